@@ -1,0 +1,228 @@
+/*
+ * ra.h -- C ABI of libra.so: the resource-aware GEMM + collective overlap hot path of
+ * arxiv/paper_2606_09200 ("Resource-aware Computation-Communication Overlap for
+ * multi-GPU ML Workloads"), hand-written CUDA for NVIDIA B200 (sm_100a).
+ *
+ * Conventions (all entry points)
+ *   - extern "C"; plain pointers and sizes; no C++ or torch types cross this boundary.
+ *   - Return value is an ra_status.  Nothing throws, aborts or prints.
+ *   - "device pointer" = address in the current CUDA device's global memory;
+ *     "host pointer"   = ordinary host memory.  Each argument says which.
+ *   - Ownership: every device buffer (operands, results, GEMM workspace, trace buffer) is
+ *     allocated and owned by the caller.  The library allocates no device memory; it lazily
+ *     caches host-side objects only (streams, events, TMA descriptors), freed by ra_shutdown().
+ *   - ra_gemm / ra_allreduce_emul / ra_alltoall_emul are ASYNCHRONOUS on `stream`
+ *     (a cudaStream_t value passed as void*; NULL = legacy default stream).  Argument errors
+ *     are detected before anything is enqueued, so a failing call has no side effects.
+ *     ra_overlap_run / ra_overlap_sweep are SYNCHRONOUS.
+ *   - Degenerate sizes: M, N or count == 0 -> RA_OK, nothing launched.  K == 0 -> C = beta*C.
+ *   - There is NO CPU fallback: without an sm_100 device every compute entry point returns
+ *     RA_ERR_ARCH (or RA_ERR_CUDA if no device/driver is present at all).
+ */
+#ifndef RA_H_
+#define RA_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define RA_MAX_RANKS 16
+
+typedef enum {
+    RA_OK = 0,
+    RA_ERR_INVALID_ARG = 1,     /* null pointer, negative dim, bad ld, misaligned pointer, P out of range, aliasing */
+    RA_ERR_UNSUPPORTED = 2,     /* valid BLAS-wise but not implemented (ld not a multiple of 8 elements, ...) */
+    RA_ERR_INFEASIBLE_KNOB = 3, /* smem_reserve_bytes / sm_budget cannot be honoured and allow_clamp == 0 */
+    RA_ERR_CUDA = 4,            /* a CUDA call failed; ra_last_cuda_error() returns the cudaError_t value */
+    RA_ERR_ARCH = 5             /* current device is not compute capability 10.x */
+} ra_status;
+
+/* Static string for a status code (never NULL). */
+const char* ra_status_str(ra_status s);
+/* cudaError_t of the most recent failing CUDA call made by this thread through the library (0 if none). */
+int ra_last_cuda_error(void);
+/* Destroys cached streams/events/descriptors.  Safe to call repeatedly. */
+void ra_shutdown(void);
+
+/* Device facts the occupancy planner uses (host out-pointers; any may be NULL).
+ * Read from cudaDeviceGetAttribute at call time -- nothing is hard-coded. */
+ra_status ra_device_info(int* sm_count, int* smem_per_sm, int* smem_per_block_optin, int* smem_reserved_per_block,
+                         int* prio_least, int* prio_greatest);
+
+/* ---------------------------------------------------------------------------------------------
+ * S3  Occupancy shaping   (section 3.1: "by tuning the GEMM tile sizes, we
+ * exploit the amount of shared memory allocated per block and therefore the number of resident
+ * GEMM blocks";  PAPER.md:116, Fig. 3: thread-block count as the second axis.)
+ *
+ * smem_reserve_bytes  >= 0.  Shared memory PER SM that the GEMM must leave unallocated so that a
+ *                     collective kernel can co-reside there.  The planner shrinks the GEMM's
+ *                     pipeline depth, then its tile, until
+ *                       ctas_per_sm * (dyn_smem_bytes + reserved_per_block) <= smem_per_sm - reserve.
+ * sm_budget           number of GEMM CTAs of the persistent grid (one CTA per SM), 1..#SMs;
+ *                     0 = all SMs.
+ * tiles_per_cta       0 = fully persistent (grid = sm_budget, each CTA loops over its tiles);
+ *                     t > 0 = bounded work: grid = ceil(n_tiles / t) and each CTA exits after
+ *                     t tiles, so a higher-priority kernel gets SMs at CTA-exit granularity
+ *                     (PAPER.md:59).  sm_budget is ignored in this mode.
+ * allow_clamp         1: an infeasible knob is clamped to the nearest feasible value and the
+ *                     plan reports what was used; 0: RA_ERR_INFEASIBLE_KNOB.
+ * ------------------------------------------------------------------------------------------- */
+typedef struct {
+    int32_t smem_reserve_bytes;
+    int32_t sm_budget;
+    int32_t tiles_per_cta;
+    int32_t allow_clamp;
+} ra_occupancy;
+
+/* What S3 decided -- for tests, logs and the sweep tables. */
+typedef struct {
+    int32_t ctas_per_sm;      /* resident GEMM CTAs per SM (cudaOccupancyMaxActiveBlocksPerMultiprocessor) */
+    int32_t grid;             /* CTAs launched */
+    int32_t stages;           /* depth of the TMA->MMA shared-memory ring */
+    int32_t tile_m, tile_n, tile_k; /* CTA tile in C's coordinates (after operand swap) */
+    int32_t split_k;          /* 1 = data-parallel tiles; >1 = stream-K (value = max parts of one tile) */
+    int32_t swap_ab;          /* 1: computed as C^T = op(B)^T op(A)^T (skinny-M path) */
+    int32_t dyn_smem_bytes;   /* dynamic shared memory per CTA, padding included */
+    int32_t smem_left_per_sm; /* smem_per_sm - ctas_per_sm*(dyn_smem_bytes + reserved_per_block) */
+    int32_t n_tiles;          /* output tiles */
+    int32_t clamped;          /* 1 if a knob was clamped */
+} ra_gemm_plan;
+
+/* Host-only: computes the plan ra_gemm would use.  `occ` NULL = defaults {0,0,0,1}. */
+ra_status ra_gemm_plan_query(int transA, int transB, int M, int N, int K, const ra_occupancy* occ, ra_gemm_plan* out);
+
+/* Bytes of device workspace ra_gemm needs for this problem and knob setting (0 if none).
+ * Only stream-K plans (split_k > 1) need one. */
+size_t ra_gemm_workspace_bytes(int transA, int transB, int M, int N, int K, const ra_occupancy* occ);
+
+/* ---------------------------------------------------------------------------------------------
+ * S1+S2  GEMM   (section 2.1:  C = alpha*op(A)*op(B) + beta*C,
+ *                A in R^{MxK}, B in R^{KxN}, C in R^{MxN}.)
+ *
+ * bf16 operands, fp32 accumulation on the tcgen05 tensor cores (accumulator in TMEM), bf16
+ * result (round-to-nearest-even).  Row-major buffers:
+ *   transA = 0: A is M x K, lda >= K          transA = 1: A is K x M, lda >= M
+ *   transB = 0: B is K x N, ldb >= N          transB = 1: B is N x K, ldb >= K
+ *   C is M x N, ldc >= N.
+ * A, B, C: device pointers, 16-byte aligned; lda, ldb, ldc multiples of 8 elements (TMA needs
+ * 16-byte row pitch), else RA_ERR_UNSUPPORTED.  C must not overlap A or B.
+ * alpha, beta: host scalars by value.  beta == 0 => C is write-only (NaN/Inf already in C do not
+ * propagate), as in BLAS.
+ * workspace: device pointer, 16-byte aligned, at least ra_gemm_workspace_bytes(...) bytes (may be
+ * NULL when that is 0).  Its contents are scratch; it must not be shared by two GEMMs in flight.
+ * Results are bit-reproducible run to run for a fixed (shape, plan): stream-K partial sums are
+ * combined in ascending-k order, never with floating-point atomics.
+ * ------------------------------------------------------------------------------------------- */
+ra_status ra_gemm(int transA, int transB, int M, int N, int K, float alpha, const void* A, int lda, const void* B,
+                  int ldb, float beta, void* C, int ldc, const ra_occupancy* occ, void* workspace,
+                  size_t workspace_bytes, void* stream);
+
+/* ---------------------------------------------------------------------------------------------
+ * S4  Allreduce stand-in   (section 2.2: "GEMM kernels compute local gradients, which
+ * are then aggregated across all GPUs using allreduce"; BASELINE.json north_star: one device,
+ * P rank buffers in HBM, fixed rank-order fp32 sum, result written back to all P buffers.)
+ *
+ *   for every e in [0,count):  s = bufs[0][e]; s = s + bufs[1][e]; ... ; s = s + bufs[P-1][e]
+ *                              (each + one IEEE-754 binary32 round-to-nearest-even add, denormals kept)
+ *                              bufs[r][e] = s  for all r.
+ * bufs: HOST array of P DEVICE pointers (copied into the kernel parameters), 1 <= P <= RA_MAX_RANKS,
+ * each 16-byte aligned, `count` floats, pairwise disjoint (overlap => RA_ERR_INVALID_ARG).
+ * sm_budget: SMs' worth of CTAs to launch (0 = all SMs).
+ * ------------------------------------------------------------------------------------------- */
+ra_status ra_allreduce_emul(float* const* bufs, int P, size_t count, int sm_budget, void* stream);
+
+/* ---------------------------------------------------------------------------------------------
+ * S5  Alltoall stand-in   ("expert-parallel workloads rely on alltoall to route
+ * tokens between devices"; BASELINE.json: P x P chunk transpose on one device.)
+ *
+ *   recv[(j*P + i)*chunk_bytes + b] = send[(i*P + j)*chunk_bytes + b]   for i,j < P, b < chunk_bytes.
+ * send, recv: device pointers, 16-byte aligned, P*P*chunk_bytes bytes each, disjoint
+ * (overlap => RA_ERR_INVALID_ARG).  chunk_bytes % 16 == 0.  1 <= P <= 256.
+ * Implemented with TMA bulk copies (global -> shared ring -> global), one issuing thread per ring.
+ * sm_budget as above.
+ * ------------------------------------------------------------------------------------------- */
+ra_status ra_alltoall_emul(const void* send, void* recv, int P, size_t chunk_bytes, int sm_budget, void* stream);
+
+/* Extended form: explicit shared-memory footprint and variant.
+ *   smem_bytes_per_cta  shared-memory ring per CTA (0 = default 64 KiB).  This is what must fit
+ *                       inside the GEMM's smem_reserve_bytes on SMs the two kernels share.
+ *   ctas_per_sm         CTAs launched per budgeted SM (0 = default).
+ *   variant             0 = TMA bulk-copy ring; 1 = plain 128-bit LDG/STG copy (no shared memory). */
+ra_status ra_alltoall_emul_ex(const void* send, void* recv, int P, size_t chunk_bytes, int sm_budget,
+                              int smem_bytes_per_cta, int ctas_per_sm, int variant, void* stream);
+
+/* ---------------------------------------------------------------------------------------------
+ * S6-S8  Overlap driver   (section 3.2: two streams per device, event dependency
+ * K_g^i -> K_c^i, K_g^{i+1} free to run concurrently with K_c^i;  PAPER.md:59, section 3.3:
+ * the communication stream gets the higher priority;  PAPER.md:108-110: TimeRatio, overlap rate.)
+ * ------------------------------------------------------------------------------------------- */
+typedef enum { RA_COLL_ALLREDUCE = 0, RA_COLL_ALLTOALL = 1, RA_COLL_NONE = 2 } ra_coll_kind;
+typedef enum { RA_MODE_SERIAL = 0, RA_MODE_OVERLAP = 1 } ra_mode;
+
+typedef struct {
+    /* GEMM K_g (same operands every iteration); set M = 0 to run the collective alone */
+    int32_t transA, transB, M, N, K;
+    float alpha, beta;
+    const void* A; int32_t lda;
+    const void* B; int32_t ldb;
+    void* C; int32_t ldc;
+    void* workspace; size_t workspace_bytes;
+    /* collective K_c */
+    int32_t kind;               /* ra_coll_kind */
+    int32_t P;
+    float* const* ar_bufs;      /* HOST array of P device pointers (allreduce, in place) */
+    size_t ar_count;
+    void* a2a_a; void* a2a_b;   /* device; iteration i copies a->b if i is even, b->a if odd */
+    size_t chunk_bytes;
+    int32_t n_iters;
+} ra_workload;
+
+typedef struct {
+    int32_t mode;               /* ra_mode */
+    ra_occupancy occ;           /* GEMM knobs */
+    int32_t coll_sm_budget;     /* 0 = all SMs */
+    int32_t coll_smem_bytes;    /* alltoall ring bytes per CTA (0 = default) */
+    int32_t coll_ctas_per_sm;   /* 0 = default */
+    int32_t coll_variant;       /* alltoall: 0 = TMA ring, 1 = LDG/STG */
+    int32_t prio_compute, prio_comm; /* cudaStreamCreateWithPriority values; equal = "priority off" */
+    int32_t dependent;          /* 1: K_c^i waits for K_g^i (the paper's schedule); 0: free-running streams */
+    int32_t record_kernel_times;/* 1: per-kernel event pairs (perturbs the schedule slightly) */
+} ra_overlap_cfg;
+
+typedef struct {
+    float total_ms;             /* GPU time, first launch to last completion, events on both streams
+                                   (ra_overlap_sweep: mean over the measured runs) */
+    float median_ms, min_ms;    /* ra_overlap_sweep: median / min over the measured runs (run: = total_ms) */
+    float gemm_ms_sum, coll_ms_sum; /* sums of per-kernel durations (record_kernel_times only, else 0) */
+    float overlap_rate;         /* sum |K_c ∩ ∪K_g| / sum |K_c|; record_kernel_times only */
+    ra_gemm_plan plan;
+    float* kernel_times;        /* optional HOST array, 4*n_iters floats: g_start, g_end, c_start, c_end (ms from t0) */
+} ra_overlap_result;
+
+/* Runs n_iters iterations under `cfg`, synchronises, fills `res` (host pointers all). */
+ra_status ra_overlap_run(const ra_workload* w, const ra_overlap_cfg* cfg, ra_overlap_result* res);
+
+/* Runs cfgs[0..n) `runs` times each, interleaved round-robin so that clock drift hits all settings
+ * alike; the first runs/3 passes are warm-up and the mean of the rest is stored in results[i].total_ms
+ * ("the first one-third of runs are considered warm-up").  *best = argmin over
+ * settings with mode == RA_MODE_OVERLAP (or over all if none).  Host pointers all. */
+ra_status ra_overlap_sweep(const ra_workload* w, const ra_overlap_cfg* cfgs, int n, int runs,
+                           ra_overlap_result* results, int* best);
+
+/* ---------------------------------------------------------------------------------------------
+ * Residency trace (evidence for "per-SM residency during overlap").  When a trace buffer is set,
+ * every CTA of every library kernel appends one record {tag, block, t_start, t_end}:
+ *   tag = kernel_id << 32 | %smid   (kernel_id: 1 = GEMM, 2 = allreduce, 3 = alltoall)
+ *   t_* = %globaltimer (ns).
+ * buf: DEVICE pointer to (1 + 4*capacity) uint64; buf[0] is the record counter (caller zeroes it).
+ * Pass NULL to disable (default).  Not thread-safe with concurrent launches from other threads.
+ * ------------------------------------------------------------------------------------------- */
+ra_status ra_set_trace(uint64_t* buf, size_t capacity);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* RA_H_ */

@@ -1,0 +1,297 @@
+"""paper_2606_09200_b200 -- thin Python binding over libra.so (the C ABI in include/ra.h).
+
+Argument marshalling only: every step of the hot path (GEMM, allreduce / alltoall stand-ins,
+overlap schedule, sweep) runs inside the library's hand-written sm_100a kernels and its C++
+driver.  PyTorch is used by callers for device memory and stream handles; this module accepts
+torch tensors (or raw integer device pointers) and passes ``tensor.data_ptr()`` through.
+
+There is no CPU fallback.  If libra.so is missing it is built with nvcc; if that fails the
+import raises.  This package never imports ``oracle``.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from ctypes import POINTER, Structure, byref, c_char_p, c_float, c_int, c_int32, c_size_t, c_uint64, c_void_p
+
+from . import build as _build
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+
+RA_OK, RA_ERR_INVALID_ARG, RA_ERR_UNSUPPORTED, RA_ERR_INFEASIBLE_KNOB, RA_ERR_CUDA, RA_ERR_ARCH = range(6)
+RA_COLL_ALLREDUCE, RA_COLL_ALLTOALL, RA_COLL_NONE = 0, 1, 2
+RA_MODE_SERIAL, RA_MODE_OVERLAP = 0, 1
+RA_MAX_RANKS = 16
+
+# every symbol include/ra.h declares (tests/test_abi.py checks the header against this and the .so)
+EXPORTS = (
+    "ra_status_str", "ra_last_cuda_error", "ra_shutdown", "ra_device_info", "ra_gemm_plan_query",
+    "ra_gemm_workspace_bytes", "ra_gemm", "ra_allreduce_emul", "ra_alltoall_emul", "ra_alltoall_emul_ex",
+    "ra_overlap_run", "ra_overlap_sweep", "ra_set_trace",
+)
+
+
+class RaError(RuntimeError):
+    def __init__(self, status: int, where: str):
+        self.status = status
+        super().__init__(f"{where}: {status_str(status)} (cuda error {last_cuda_error()})")
+
+
+class Occupancy(Structure):
+    _fields_ = [("smem_reserve_bytes", c_int32), ("sm_budget", c_int32), ("tiles_per_cta", c_int32),
+                ("allow_clamp", c_int32)]
+
+
+class GemmPlan(Structure):
+    _fields_ = [(n, c_int32) for n in ("ctas_per_sm", "grid", "stages", "tile_m", "tile_n", "tile_k", "split_k",
+                                       "swap_ab", "dyn_smem_bytes", "smem_left_per_sm", "n_tiles", "clamped")]
+
+    def as_dict(self):
+        return {n: getattr(self, n) for n, _ in self._fields_}
+
+
+class Workload(Structure):
+    _fields_ = [("transA", c_int32), ("transB", c_int32), ("M", c_int32), ("N", c_int32), ("K", c_int32),
+                ("alpha", c_float), ("beta", c_float),
+                ("A", c_void_p), ("lda", c_int32), ("B", c_void_p), ("ldb", c_int32), ("C", c_void_p), ("ldc", c_int32),
+                ("workspace", c_void_p), ("workspace_bytes", c_size_t),
+                ("kind", c_int32), ("P", c_int32), ("ar_bufs", POINTER(c_void_p)), ("ar_count", c_size_t),
+                ("a2a_a", c_void_p), ("a2a_b", c_void_p), ("chunk_bytes", c_size_t), ("n_iters", c_int32)]
+
+
+class OverlapCfg(Structure):
+    _fields_ = [("mode", c_int32), ("occ", Occupancy), ("coll_sm_budget", c_int32), ("coll_smem_bytes", c_int32),
+                ("coll_ctas_per_sm", c_int32), ("coll_variant", c_int32), ("prio_compute", c_int32),
+                ("prio_comm", c_int32), ("dependent", c_int32), ("record_kernel_times", c_int32)]
+
+
+class OverlapResult(Structure):
+    _fields_ = [("total_ms", c_float), ("median_ms", c_float), ("min_ms", c_float), ("gemm_ms_sum", c_float),
+                ("coll_ms_sum", c_float), ("overlap_rate", c_float), ("plan", GemmPlan),
+                ("kernel_times", POINTER(c_float))]
+
+
+_lib = None
+
+
+def lib_path() -> str:
+    return _build.LIB
+
+
+def _L():
+    global _lib
+    if _lib is not None:
+        return _lib
+    path = _build.build()  # no-op when up to date; raises if nvcc fails -- there is no fallback
+    lib = ctypes.CDLL(path)
+    lib.ra_status_str.restype = c_char_p
+    lib.ra_status_str.argtypes = [c_int]
+    lib.ra_last_cuda_error.restype = c_int
+    lib.ra_shutdown.restype = None
+    lib.ra_device_info.argtypes = [POINTER(c_int)] * 6
+    lib.ra_gemm_plan_query.argtypes = [c_int] * 5 + [POINTER(Occupancy), POINTER(GemmPlan)]
+    lib.ra_gemm_workspace_bytes.restype = c_size_t
+    lib.ra_gemm_workspace_bytes.argtypes = [c_int] * 5 + [POINTER(Occupancy)]
+    lib.ra_gemm.argtypes = [c_int, c_int, c_int, c_int, c_int, c_float, c_void_p, c_int, c_void_p, c_int, c_float,
+                            c_void_p, c_int, POINTER(Occupancy), c_void_p, c_size_t, c_void_p]
+    lib.ra_allreduce_emul.argtypes = [POINTER(c_void_p), c_int, c_size_t, c_int, c_void_p]
+    lib.ra_alltoall_emul.argtypes = [c_void_p, c_void_p, c_int, c_size_t, c_int, c_void_p]
+    lib.ra_alltoall_emul_ex.argtypes = [c_void_p, c_void_p, c_int, c_size_t, c_int, c_int, c_int, c_int, c_void_p]
+    lib.ra_overlap_run.argtypes = [POINTER(Workload), POINTER(OverlapCfg), POINTER(OverlapResult)]
+    lib.ra_overlap_sweep.argtypes = [POINTER(Workload), POINTER(OverlapCfg), c_int, c_int, POINTER(OverlapResult),
+                                     POINTER(c_int)]
+    lib.ra_set_trace.argtypes = [c_void_p, c_size_t]
+    for name in EXPORTS:
+        fn = getattr(lib, name)
+        if name not in ("ra_status_str", "ra_last_cuda_error", "ra_shutdown", "ra_gemm_workspace_bytes"):
+            fn.restype = c_int
+    _lib = lib
+    return lib
+
+
+# ---- helpers -----------------------------------------------------------------------------------
+def status_str(s: int) -> str:
+    return _L().ra_status_str(int(s)).decode()
+
+
+def last_cuda_error() -> int:
+    return int(_L().ra_last_cuda_error())
+
+
+def _check(s: int, where: str):
+    if s != RA_OK:
+        raise RaError(s, where)
+
+
+def _ptr(x) -> int | None:
+    """torch tensor -> device address; int/None pass through."""
+    if x is None:
+        return None
+    if isinstance(x, int):
+        return x
+    return int(x.data_ptr())
+
+
+def _stream(stream) -> int | None:
+    if stream is None:
+        try:
+            import torch
+            return int(torch.cuda.current_stream().cuda_stream) or None
+        except Exception:
+            return None
+    if isinstance(stream, int):
+        return stream or None
+    return int(stream.cuda_stream) or None
+
+
+def _occ(occ) -> Occupancy | None:
+    if occ is None or isinstance(occ, Occupancy):
+        return occ
+    return Occupancy(int(occ.get("smem_reserve_bytes", 0)), int(occ.get("sm_budget", 0)),
+                     int(occ.get("tiles_per_cta", 0)), int(occ.get("allow_clamp", 1)))
+
+
+def _occ_ref(occ):
+    o = _occ(occ)
+    return byref(o) if o is not None else None
+
+
+# ---- the C ABI, same names -----------------------------------------------------------------------
+def ra_shutdown() -> None:
+    _L().ra_shutdown()
+
+
+def ra_device_info() -> dict:
+    vals = [c_int(0) for _ in range(6)]
+    _check(_L().ra_device_info(*[byref(v) for v in vals]), "ra_device_info")
+    keys = ("sm_count", "smem_per_sm", "smem_per_block_optin", "smem_reserved_per_block", "prio_least", "prio_greatest")
+    return {k: v.value for k, v in zip(keys, vals)}
+
+
+def ra_gemm_plan_query(transA, transB, M, N, K, occ=None) -> dict:
+    plan = GemmPlan()
+    _check(_L().ra_gemm_plan_query(transA, transB, M, N, K, _occ_ref(occ), byref(plan)), "ra_gemm_plan_query")
+    return plan.as_dict()
+
+
+def ra_gemm_workspace_bytes(transA, transB, M, N, K, occ=None) -> int:
+    return int(_L().ra_gemm_workspace_bytes(transA, transB, M, N, K, _occ_ref(occ)))
+
+
+def ra_gemm(transA, transB, M, N, K, alpha, A, lda, B, ldb, beta, C, ldc, occ=None, workspace=None,
+            workspace_bytes=None, stream=None) -> None:
+    if workspace is not None and workspace_bytes is None:
+        workspace_bytes = workspace.numel() * workspace.element_size()
+    _check(_L().ra_gemm(transA, transB, M, N, K, float(alpha), _ptr(A), lda, _ptr(B), ldb, float(beta), _ptr(C), ldc,
+                        _occ_ref(occ), _ptr(workspace), int(workspace_bytes or 0), _stream(stream)), "ra_gemm")
+
+
+def _ptr_array(bufs):
+    arr = (c_void_p * len(bufs))(*[_ptr(b) for b in bufs])
+    return arr
+
+
+def ra_allreduce_emul(bufs, count=None, sm_budget=0, stream=None) -> None:
+    if count is None:
+        count = bufs[0].numel()
+    arr = _ptr_array(bufs)
+    _check(_L().ra_allreduce_emul(arr, len(bufs), int(count), int(sm_budget), _stream(stream)), "ra_allreduce_emul")
+
+
+def ra_alltoall_emul(send, recv, P, chunk_bytes, sm_budget=0, stream=None) -> None:
+    _check(_L().ra_alltoall_emul(_ptr(send), _ptr(recv), int(P), int(chunk_bytes), int(sm_budget), _stream(stream)),
+           "ra_alltoall_emul")
+
+
+def ra_alltoall_emul_ex(send, recv, P, chunk_bytes, sm_budget=0, smem_bytes_per_cta=0, ctas_per_sm=0, variant=0,
+                        stream=None) -> None:
+    _check(_L().ra_alltoall_emul_ex(_ptr(send), _ptr(recv), int(P), int(chunk_bytes), int(sm_budget),
+                                    int(smem_bytes_per_cta), int(ctas_per_sm), int(variant), _stream(stream)),
+           "ra_alltoall_emul_ex")
+
+
+def ra_set_trace(buf, capacity: int = 0) -> None:
+    _check(_L().ra_set_trace(_ptr(buf), int(capacity)), "ra_set_trace")
+
+
+def make_workload(*, gemm=None, allreduce=None, alltoall=None, n_iters=1):
+    """Marshal a workload.  gemm = dict(M,N,K,A,B,C[,alpha,beta,lda,ldb,ldc,transA,transB,workspace]);
+    allreduce = list of P fp32 tensors; alltoall = dict(a, b, P, chunk_bytes).
+    Returns (Workload, keepalive) -- keepalive holds the pointer array."""
+    w = Workload()
+    keep = []
+    if gemm is not None:
+        g = gemm
+        w.transA, w.transB = int(g.get("transA", 0)), int(g.get("transB", 1))
+        w.M, w.N, w.K = int(g["M"]), int(g["N"]), int(g["K"])
+        w.alpha, w.beta = float(g.get("alpha", 1.0)), float(g.get("beta", 0.0))
+        w.A, w.B, w.C = _ptr(g["A"]), _ptr(g["B"]), _ptr(g["C"])
+        w.lda = int(g.get("lda", w.M if w.transA else w.K))
+        w.ldb = int(g.get("ldb", w.K if w.transB else w.N))
+        w.ldc = int(g.get("ldc", w.N))
+        ws = g.get("workspace")
+        if ws is not None:
+            w.workspace = _ptr(ws)
+            w.workspace_bytes = ws.numel() * ws.element_size()
+    if allreduce is not None:
+        arr = _ptr_array(allreduce)
+        keep.append(arr)
+        w.kind, w.P = RA_COLL_ALLREDUCE, len(allreduce)
+        w.ar_bufs = ctypes.cast(arr, POINTER(c_void_p))
+        w.ar_count = int(allreduce[0].numel())
+    elif alltoall is not None:
+        w.kind, w.P = RA_COLL_ALLTOALL, int(alltoall["P"])
+        w.a2a_a, w.a2a_b = _ptr(alltoall["a"]), _ptr(alltoall["b"])
+        w.chunk_bytes = int(alltoall["chunk_bytes"])
+    else:
+        w.kind = RA_COLL_NONE
+    w.n_iters = int(n_iters)
+    return w, keep
+
+
+def make_cfg(mode=RA_MODE_OVERLAP, occ=None, coll_sm_budget=0, coll_smem_bytes=0, coll_ctas_per_sm=0, coll_variant=0,
+             prio_compute=0, prio_comm=0, dependent=1, record_kernel_times=0) -> OverlapCfg:
+    c = OverlapCfg()
+    c.mode = int(mode)
+    c.occ = _occ(occ) or Occupancy(0, 0, 0, 1)
+    c.coll_sm_budget, c.coll_smem_bytes = int(coll_sm_budget), int(coll_smem_bytes)
+    c.coll_ctas_per_sm, c.coll_variant = int(coll_ctas_per_sm), int(coll_variant)
+    c.prio_compute, c.prio_comm = int(prio_compute), int(prio_comm)
+    c.dependent, c.record_kernel_times = int(dependent), int(record_kernel_times)
+    return c
+
+
+def _result_dict(r: OverlapResult, n_iters: int, times) -> dict:
+    d = {"total_ms": r.total_ms, "median_ms": r.median_ms, "min_ms": r.min_ms, "gemm_ms_sum": r.gemm_ms_sum,
+         "coll_ms_sum": r.coll_ms_sum, "overlap_rate": r.overlap_rate, "plan": r.plan.as_dict()}
+    if times is not None:
+        d["kernel_times"] = [list(times[4 * i:4 * i + 4]) for i in range(n_iters)]
+    return d
+
+
+def ra_overlap_run(workload: Workload, cfg: OverlapCfg) -> dict:
+    res = OverlapResult()
+    times = None
+    if cfg.record_kernel_times:
+        times = (c_float * (4 * workload.n_iters))()
+        res.kernel_times = ctypes.cast(times, POINTER(c_float))
+    _check(_L().ra_overlap_run(byref(workload), byref(cfg), byref(res)), "ra_overlap_run")
+    return _result_dict(res, workload.n_iters, times)
+
+
+def ra_overlap_sweep(workload: Workload, cfgs, runs: int = 30):
+    """Returns (list of result dicts, best index)."""
+    n = len(cfgs)
+    carr = (OverlapCfg * n)(*cfgs)
+    rarr = (OverlapResult * n)()
+    keep = []
+    for i in range(n):
+        if cfgs[i].record_kernel_times:
+            t = (c_float * (4 * workload.n_iters))()
+            keep.append(t)
+            rarr[i].kernel_times = ctypes.cast(t, POINTER(c_float))
+        else:
+            keep.append(None)
+    best = c_int(-1)
+    _check(_L().ra_overlap_sweep(byref(workload), carr, n, int(runs), rarr, byref(best)), "ra_overlap_sweep")
+    return [_result_dict(rarr[i], workload.n_iters, keep[i]) for i in range(n)], best.value

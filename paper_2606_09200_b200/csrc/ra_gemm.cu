@@ -1,0 +1,719 @@
+// ra_gemm.cu -- K1: bf16 GEMM on the tcgen05 tensor cores (S1, S2, S3).
+//
+//   C[M,N] = alpha * op(A) * op(B) + beta * C          (section 2.1)
+//
+// Kernel coordinates.  The kernel multiplies two K-contiguous ("K-major") operands
+//     X : RX x K  (rows -> TMEM lanes, 128 per CTA tile, the UMMA "M" side)
+//     Y : RY x K  (rows -> TMEM columns, BN per CTA tile, the UMMA "N" side)
+// into acc[x][y] = sum_k X[x][k]*Y[y][k].  transA=0,transB=1 maps A->X, B->Y (C[x][y]); the
+// skinny-M path swaps them (B->X, A->Y, C[y][x]) so that the 128-row side is the long weight
+// dimension and tiny M costs BN = 64 columns instead of a padded 128-row tile.
+//
+// Per CTA (192 threads):
+//   warp 0   TMA producer      one elected lane: cp.async.bulk.tensor.2d into a ring of `stages`
+//                              128B-swizzled shared-memory stages, mbarrier complete_tx
+//   warp 1   MMA issuer        allocates TMEM; one elected lane issues tcgen05.mma (128 x BN x 16,
+//                              kind::f16, bf16 in / fp32 accumulate in TMEM), tcgen05.commit frees
+//                              the smem stage / publishes the accumulator
+//   warps 2-5 epilogue         tcgen05.ld (32 lanes x 32 columns per instruction) -> alpha/beta ->
+//                              cvt.rn.bf16x2.f32 -> global stores.  Two TMEM accumulators (2 x BN
+//                              columns) so the epilogue of tile i overlaps the main loop of tile i+1.
+//
+// Scheduling (S3: occupancy shaping).  grid = sm_budget persistent CTAs, one
+// per SM; pipeline depth (and, when squeezed, the tile) follows from smem_reserve_bytes.  Two
+// work decompositions, both static (no atomics in the schedule):
+//   data-parallel   CTA c owns tiles c, c+G, c+2G, ... (grouped rasterisation for L2 reuse)
+//   stream-K        the n_tiles*KB k-block units are cut into G equal contiguous ranges; a tile
+//                   whose units span several CTAs is finished by the LAST of them to arrive
+//                   (threadfence + one integer atomic per part): it sums the fp32 partials of all
+//                   parts from the workspace in ascending-k order, so the result does not depend
+//                   on arrival order and is bit-reproducible.
+#include <cuda.h>
+#include <cuda_bf16.h>
+
+#include <mutex>
+
+#include "ra_common.cuh"
+
+namespace ra {
+
+constexpr int kBM = 128;        // tile rows on the X side (UMMA M)
+constexpr int kBK = 64;         // 64 bf16 = 128 B = one swizzle-128B atom row
+constexpr int kUmmaK = 16;
+constexpr int kGemmThreads = 192;
+constexpr int kEpiThreads = 128;
+constexpr int kMaxStages = 8;
+constexpr int kBarrierBytes = 256;
+constexpr int kAlignSlack = 1024;
+constexpr int kGroupX = 16;     // rasterisation: X-tiles per group
+
+__host__ __device__ constexpr int stage_bytes(int bn) { return (kBM + bn) * kBK * 2; }
+
+struct GemmParams {
+    int RX, RY, K;
+    int tiles_x, tiles_y, n_tiles, kb_per_tile;
+    int swap;          // 0: C[x*ldc + y]   1: C[y*ldc + x]
+    int stream_k;
+    int stages;
+    float alpha, beta;
+    __nv_bfloat16* C;
+    int ldc;
+    float* partials;   // stream-K: [2*grid][BN][128] fp32
+    int* counters;     // stream-K: [n_tiles]
+    int hintX, hintY;  // L2 policy per operand: 0 normal, 1 evict_first, 2 evict_last
+};
+
+// ---- device helpers ---------------------------------------------------------------------------
+__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+
+__device__ __forceinline__ void tma_load_2d(uint32_t dst_smem, const CUtensorMap* map, int c0, int c1, uint32_t bar,
+                                            uint64_t policy) {
+    asm volatile(
+        "cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes.L2::cache_hint"
+        " [%0], [%1, {%3, %4}], [%2], %5;"
+        ::"r"(dst_smem), "l"(map), "r"(bar), "r"(c0), "r"(c1), "l"(policy)
+        : "memory");
+}
+
+// K-major, 128-byte swizzle: rows of 128 B, 8-row groups 1024 B apart (SBO), LBO unused (=1),
+// descriptor version 1 (sm_100), layout type 2 = SWIZZLE_128B.
+__device__ __forceinline__ uint64_t umma_desc_sw128(uint32_t smem_addr) {
+    uint64_t d = 0;
+    d |= (uint64_t)((smem_addr & 0x3FFFFu) >> 4);
+    d |= (uint64_t)1 << 16;
+    d |= (uint64_t)(1024 >> 4) << 32;
+    d |= (uint64_t)1 << 46;
+    d |= (uint64_t)2 << 61;
+    return d;
+}
+// kind::f16 instruction descriptor: D = fp32, A = B = bf16, both K-major, M x N.
+__host__ __device__ constexpr uint32_t umma_idesc_bf16(int m, int n) {
+    return (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(n >> 3) << 17) | ((uint32_t)(m >> 4) << 24);
+}
+__device__ __forceinline__ void umma_bf16(uint32_t tmem_d, uint64_t adesc, uint64_t bdesc, uint32_t idesc,
+                                          uint32_t accumulate) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+        "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}"
+        ::"r"(tmem_d), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate)
+        : "memory");
+}
+__device__ __forceinline__ void umma_commit(uint32_t bar) {
+    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&v)[32]) {
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
+        "{%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,"
+        "%16,%17,%18,%19,%20,%21,%22,%23,%24,%25,%26,%27,%28,%29,%30,%31}, [%32];"
+        : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
+          "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15]),
+          "=r"(v[16]), "=r"(v[17]), "=r"(v[18]), "=r"(v[19]), "=r"(v[20]), "=r"(v[21]), "=r"(v[22]), "=r"(v[23]),
+          "=r"(v[24]), "=r"(v[25]), "=r"(v[26]), "=r"(v[27]), "=r"(v[28]), "=r"(v[29]), "=r"(v[30]), "=r"(v[31])
+        : "r"(taddr));
+}
+__device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
+__device__ __forceinline__ void epi_bar_sync() { asm volatile("bar.sync 1, %0;" ::"n"(kEpiThreads) : "memory"); }
+
+__device__ __forceinline__ uint64_t make_policy(int kind) {
+    return kind == 1 ? policy_evict_first() : (kind == 2 ? policy_evict_last() : policy_evict_normal());
+}
+
+// ---- static schedule: every role walks the same sequence of (tile, kb0, kb1) segments ----------
+struct Seg {
+    int tile, kb0, kb1;
+    long long start_unit;   // stream-K: first unit of this segment
+};
+struct Sched {
+    const GemmParams& p;
+    long long u0, u1, cur;  // stream-K unit range of this CTA
+    int it;
+    __device__ Sched(const GemmParams& p_) : p(p_), it(0) {
+        if (p.stream_k) {
+            const long long U = (long long)p.n_tiles * p.kb_per_tile;
+            u0 = (long long)blockIdx.x * U / gridDim.x;
+            u1 = (long long)(blockIdx.x + 1) * U / gridDim.x;
+            cur = u0;
+        } else {
+            u0 = u1 = cur = 0;
+        }
+    }
+    __device__ bool next(Seg& s) {
+        if (p.stream_k) {
+            if (cur >= u1) return false;
+            s.tile = (int)(cur / p.kb_per_tile);
+            s.kb0 = (int)(cur - (long long)s.tile * p.kb_per_tile);
+            const long long left = u1 - cur;
+            const int room = p.kb_per_tile - s.kb0;
+            s.kb1 = s.kb0 + (int)(left < room ? left : room);
+            s.start_unit = cur;
+            cur += s.kb1 - s.kb0;
+            return true;
+        }
+        const long long t = (long long)blockIdx.x + (long long)it * gridDim.x;
+        if (t >= p.n_tiles) return false;
+        ++it;
+        s.tile = (int)t;
+        s.kb0 = 0;
+        s.kb1 = p.kb_per_tile;
+        s.start_unit = 0;
+        return true;
+    }
+};
+// grouped rasterisation: kGroupX X-tiles form a group; inside a group x runs fastest.
+__device__ __forceinline__ void tile_xy(const GemmParams& p, int tile, int& tx, int& ty) {
+    const int per_group = kGroupX * p.tiles_y;
+    const int g = tile / per_group;
+    const int first_x = g * kGroupX;
+    const int gsize = min(kGroupX, p.tiles_x - first_x);
+    const int r = tile - g * per_group;
+    tx = first_x + r % gsize;
+    ty = r / gsize;
+}
+
+// ---- epilogue pieces ---------------------------------------------------------------------------
+// 32 accumulator values acc[x][y0 .. y0+31] of row x -> C.
+__device__ __forceinline__ void store_out(const GemmParams& p, const float (&acc)[32], int x, int y0) {
+    if (x >= p.RX || y0 >= p.RY) return;
+    const float alpha = p.alpha, beta = p.beta;
+    if (!p.swap) {
+        __nv_bfloat16* row = p.C + (size_t)x * p.ldc + y0;
+        if (y0 + 32 <= p.RY) {
+            uint4 out[4];
+            uint32_t* o = reinterpret_cast<uint32_t*>(out);
+            if (beta != 0.f) {
+                uint4 cin[4];
+#pragma unroll
+                for (int v = 0; v < 4; ++v) cin[v] = *reinterpret_cast<const uint4*>(row + 8 * v);
+                const __nv_bfloat162* ci = reinterpret_cast<const __nv_bfloat162*>(cin);
+#pragma unroll
+                for (int j = 0; j < 16; ++j) {
+                    const float2 c = __bfloat1622float2(ci[j]);
+                    const __nv_bfloat162 r = __floats2bfloat162_rn(fmaf(beta, c.x, alpha * acc[2 * j]),
+                                                                   fmaf(beta, c.y, alpha * acc[2 * j + 1]));
+                    o[j] = *reinterpret_cast<const uint32_t*>(&r);
+                }
+            } else {
+#pragma unroll
+                for (int j = 0; j < 16; ++j) {
+                    const __nv_bfloat162 r = __floats2bfloat162_rn(alpha * acc[2 * j], alpha * acc[2 * j + 1]);
+                    o[j] = *reinterpret_cast<const uint32_t*>(&r);
+                }
+            }
+#pragma unroll
+            for (int v = 0; v < 4; ++v) *reinterpret_cast<uint4*>(row + 8 * v) = out[v];
+        } else {
+#pragma unroll
+            for (int j = 0; j < 32; ++j) {
+                if (y0 + j < p.RY) {
+                    float r = alpha * acc[j];
+                    if (beta != 0.f) r = fmaf(beta, __bfloat162float(row[j]), r);
+                    row[j] = __float2bfloat16_rn(r);
+                }
+            }
+        }
+    } else {
+        // transposed store: lanes of a warp hold consecutive x -> each j is one coalesced 64-byte row piece
+#pragma unroll
+        for (int j = 0; j < 32; ++j) {
+            if (y0 + j < p.RY) {
+                __nv_bfloat16* ptr = p.C + (size_t)(y0 + j) * p.ldc + x;
+                float r = alpha * acc[j];
+                if (beta != 0.f) r = fmaf(beta, __bfloat162float(*ptr), r);
+                *ptr = __float2bfloat16_rn(r);
+            }
+        }
+    }
+}
+
+template <int BN>
+__global__ void __launch_bounds__(kGemmThreads, 1)
+gemm_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constant__ CUtensorMap mapY, const GemmParams p,
+            Trace tr) {
+    constexpr int kStageBytes = stage_bytes(BN);
+    constexpr int kXBytes = kBM * kBK * 2;
+    constexpr int kTmemCols = 2 * BN;   // two accumulators (power of two for BN in {64,128,256})
+    constexpr uint32_t kIdesc = umma_idesc_bf16(kBM, BN);
+    static_assert(BN == 64 || BN == 128 || BN == 256, "BN");
+
+    extern __shared__ uint8_t smem_raw[];
+    // 1024-byte alignment for the 128B swizzle; the barrier block sits after the stages
+    const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
+    const uint32_t bar_base = smem_base + p.stages * kStageBytes;
+    auto full_bar = [&](int s) { return bar_base + 8u * s; };
+    auto empty_bar = [&](int s) { return bar_base + 8u * (kMaxStages + s); };
+    auto tfull_bar = [&](int b) { return bar_base + 8u * (2 * kMaxStages + b); };
+    auto tempty_bar = [&](int b) { return bar_base + 8u * (2 * kMaxStages + 2 + b); };
+    const uint32_t tmem_slot = bar_base + 8u * (2 * kMaxStages + 4);
+    const uint32_t flag_slot = tmem_slot + 8;
+    uint8_t* smem_gen = smem_raw + (smem_base - smem_u32(smem_raw));   // generic view of smem_base
+
+    const int warp = threadIdx.x >> 5;
+    const int lane = threadIdx.x & 31;
+    uint64_t* rec = (threadIdx.x == 0) ? trace_begin(tr, KID_GEMM) : nullptr;
+
+    if (warp == 0 && lane == 0) {
+        asm volatile("prefetch.tensormap [%0];" ::"l"(&mapX) : "memory");
+        asm volatile("prefetch.tensormap [%0];" ::"l"(&mapY) : "memory");
+        for (int s = 0; s < p.stages; ++s) {
+            mbar_init(full_bar(s), 1);
+            mbar_init(empty_bar(s), 1);
+        }
+        for (int b = 0; b < 2; ++b) {
+            mbar_init(tfull_bar(b), 1);
+            mbar_init(tempty_bar(b), kEpiThreads);
+        }
+        mbar_fence_init();
+    }
+    if (warp == 1) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(tmem_slot),
+                     "r"((uint32_t)kTmemCols)
+                     : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    }
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem_base = *reinterpret_cast<volatile uint32_t*>(smem_gen + (tmem_slot - smem_base));
+
+    if (warp == 0) {
+        // ================= TMA producer =================
+        if (lane == 0) {
+            const uint64_t polX = make_policy(p.hintX), polY = make_policy(p.hintY);
+            Sched sched(p);
+            Seg sg;
+            int stage = 0;
+            uint32_t phase = 0;
+            while (sched.next(sg)) {
+                int tx, ty;
+                tile_xy(p, sg.tile, tx, ty);
+                for (int kb = sg.kb0; kb < sg.kb1; ++kb) {
+                    mbar_wait(empty_bar(stage), phase ^ 1u);
+                    mbar_expect_tx(full_bar(stage), kStageBytes);
+                    const uint32_t sx = smem_base + stage * kStageBytes;
+                    tma_load_2d(sx, &mapX, kb * kBK, tx * kBM, full_bar(stage), polX);
+                    tma_load_2d(sx + kXBytes, &mapY, kb * kBK, ty * BN, full_bar(stage), polY);
+                    if (++stage == p.stages) { stage = 0; phase ^= 1u; }
+                }
+            }
+        }
+    } else if (warp == 1) {
+        // ================= MMA issuer =================
+        if (lane == 0) {
+            Sched sched(p);
+            Seg sg;
+            int stage = 0;
+            uint32_t phase = 0;
+            int acc_it = 0;
+            while (sched.next(sg)) {
+                const int buf = acc_it & 1;
+                const uint32_t aphase = (acc_it >> 1) & 1;
+                mbar_wait(tempty_bar(buf), aphase ^ 1u);   // epilogue has drained this accumulator
+                tc_fence_after();
+                const uint32_t tmem_d = tmem_base + (uint32_t)(buf * BN);
+                for (int kb = sg.kb0; kb < sg.kb1; ++kb) {
+                    mbar_wait(full_bar(stage), phase);     // TMA bytes have landed
+                    tc_fence_after();
+                    const uint32_t sx = smem_base + stage * kStageBytes;
+                    const uint64_t dx = umma_desc_sw128(sx);
+                    const uint64_t dy = umma_desc_sw128(sx + kXBytes);
+#pragma unroll
+                    for (int k = 0; k < kBK / kUmmaK; ++k) {
+                        // +32 B per UMMA_K step inside the swizzle atom = +2 in the (addr >> 4) field
+                        umma_bf16(tmem_d, dx + (uint64_t)(2 * k), dy + (uint64_t)(2 * k), kIdesc,
+                                  (kb > sg.kb0 || k > 0) ? 1u : 0u);
+                    }
+                    umma_commit(empty_bar(stage));         // frees the smem stage when these MMAs retire
+                    if (++stage == p.stages) { stage = 0; phase ^= 1u; }
+                }
+                umma_commit(tfull_bar(buf));               // accumulator complete
+                ++acc_it;
+            }
+        }
+    } else {
+        // ================= epilogue (warps 2..5) =================
+        const int quarter = warp & 3;                       // TMEM lane quarter this warp may read
+        const int xl = quarter * 32 + lane;                 // row inside the tile
+        const int et = threadIdx.x - 64;                    // 0..127
+        Sched sched(p);
+        Seg sg;
+        int acc_it = 0;
+        while (sched.next(sg)) {
+            const int buf = acc_it & 1;
+            const uint32_t aphase = (acc_it >> 1) & 1;
+            int tx, ty;
+            tile_xy(p, sg.tile, tx, ty);
+            const bool whole = (sg.kb0 == 0 && sg.kb1 == p.kb_per_tile);
+            const int x = tx * kBM + xl;
+            float* part = nullptr;
+            if (!whole) {
+                const int slot = 2 * (int)blockIdx.x + (sg.start_unit == sched.u0 ? 0 : 1);
+                part = p.partials + (size_t)slot * (kBM * BN);
+            }
+            mbar_wait(tfull_bar(buf), aphase);
+            tc_fence_after();
+            const uint32_t taddr = tmem_base + ((uint32_t)(quarter * 32) << 16) + (uint32_t)(buf * BN);
+#pragma unroll 1
+            for (int c = 0; c < BN / 32; ++c) {
+                uint32_t v[32];
+                tmem_ld32(taddr + c * 32, v);
+                tmem_ld_wait();
+                float acc[32];
+#pragma unroll
+                for (int j = 0; j < 32; ++j) acc[j] = __uint_as_float(v[j]);
+                if (whole) {
+                    store_out(p, acc, x, ty * BN + c * 32);
+                } else {
+#pragma unroll
+                    for (int j = 0; j < 32; ++j) __stcg(part + (size_t)(c * 32 + j) * kBM + xl, acc[j]);
+                }
+            }
+            tc_fence_before();
+            mbar_arrive(tempty_bar(buf));
+            ++acc_it;
+
+            if (!whole) {
+                // ---- stream-K fix-up: last part to arrive reduces all parts in ascending-k order ----
+                const long long U = (long long)p.n_tiles * p.kb_per_tile;
+                const long long G = gridDim.x;
+                const long long ua = (long long)sg.tile * p.kb_per_tile;          // first unit of the tile
+                const long long ub = ua + p.kb_per_tile - 1;                      // last unit of the tile
+                const int c_first = (int)(((ua + 1) * G - 1) / U);
+                const int c_last = (int)(((ub + 1) * G - 1) / U);
+                const int n_parts = c_last - c_first + 1;
+                __threadfence();
+                epi_bar_sync();
+                volatile int* flag = reinterpret_cast<volatile int*>(smem_gen + (flag_slot - smem_base));
+                if (et == 0) {
+                    const int old = atomicAdd(p.counters + sg.tile, 1);
+                    *flag = (old == n_parts - 1) ? 1 : 0;
+                }
+                epi_bar_sync();
+                const bool last = (*flag != 0);
+                epi_bar_sync();   // everyone has read the flag before a later segment overwrites it
+                if (last) {
+                    __threadfence();
+#pragma unroll 1
+                    for (int c = 0; c < BN / 32; ++c) {
+                        float acc[32];
+#pragma unroll 1
+                        for (int cc = c_first; cc <= c_last; ++cc) {
+                            const long long cu0 = (long long)cc * U / G;
+                            const long long seg_start = cu0 > ua ? cu0 : ua;
+                            const int slot = 2 * cc + (seg_start == cu0 ? 0 : 1);
+                            const float* src = p.partials + (size_t)slot * (kBM * BN) + (size_t)(c * 32) * kBM + xl;
+                            if (cc == c_first) {
+#pragma unroll
+                                for (int j = 0; j < 32; ++j) acc[j] = __ldcg(src + (size_t)j * kBM);
+                            } else {
+#pragma unroll
+                                for (int j = 0; j < 32; ++j) acc[j] = __fadd_rn(acc[j], __ldcg(src + (size_t)j * kBM));
+                            }
+                        }
+                        store_out(p, acc, x, ty * BN + c * 32);
+                    }
+                }
+            }
+        }
+    }
+
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 1) {
+        tc_fence_after();
+        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"((uint32_t)kTmemCols)
+                     : "memory");
+    }
+    if (threadIdx.x == 0) trace_end(rec);
+}
+
+// C = beta * C  (K == 0 or alpha == 0: op(A), op(B) are not referenced, as in BLAS)
+__global__ void scale_c_kernel(__nv_bfloat16* C, int M, int N, int ldc, float beta) {
+    const size_t total = (size_t)M * N;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (size_t)gridDim.x * blockDim.x) {
+        const size_t r = i / N, c = i - r * N;
+        __nv_bfloat16* ptr = C + r * ldc + c;
+        *ptr = (beta == 0.f) ? __float2bfloat16_rn(0.f) : __float2bfloat16_rn(beta * __bfloat162float(*ptr));
+    }
+}
+
+// ---- host: tensor maps -------------------------------------------------------------------------
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+static EncodeTiledFn g_encode = nullptr;
+static std::once_flag g_encode_once;
+
+static ra_status get_encode(EncodeTiledFn* fn) {
+    static cudaError_t err = cudaSuccess;
+    std::call_once(g_encode_once, [] {
+        void* f = nullptr;
+        cudaDriverEntryPointQueryResult qres;
+        err = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &f, cudaEnableDefault, &qres);
+        if (err == cudaSuccess && qres == cudaDriverEntryPointSuccess) g_encode = reinterpret_cast<EncodeTiledFn>(f);
+    });
+    if (g_encode == nullptr) return cuda_fail(err != cudaSuccess ? err : cudaErrorSymbolNotFound);
+    *fn = g_encode;
+    return RA_OK;
+}
+
+// rows x K bf16, row pitch ld elements; box = 64 (k) x box_rows, 128-byte swizzle, OOB -> zeros.
+static ra_status make_map(CUtensorMap* map, const void* base, int rows, int K, int ld, int box_rows) {
+    EncodeTiledFn enc;
+    RA_TRY(get_encode(&enc));
+    const cuuint64_t dims[2] = {(cuuint64_t)K, (cuuint64_t)rows};
+    const cuuint64_t strides[1] = {(cuuint64_t)ld * 2};
+    const cuuint32_t box[2] = {(cuuint32_t)kBK, (cuuint32_t)box_rows};
+    const cuuint32_t estr[2] = {1, 1};
+    const CUresult r = enc(map, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(base), dims, strides, box, estr,
+                           CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                           CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) {
+        g_last_cuda_error = (int)cudaErrorInvalidValue;
+        return RA_ERR_CUDA;
+    }
+    return RA_OK;
+}
+
+// ---- host: S3 planner ----------------------------------------------------------------------------
+struct Plan {
+    ra_gemm_plan pub;
+    int bn;
+    size_t counters_bytes, ws_bytes;
+};
+
+static int dyn_smem_for(int bn, int stages) { return stages * stage_bytes(bn) + kAlignSlack + kBarrierBytes; }
+
+static ra_status validate_shape(int transA, int transB, int M, int N, int K) {
+    if ((transA != 0 && transA != 1) || (transB != 0 && transB != 1)) return RA_ERR_INVALID_ARG;
+    if (M < 0 || N < 0 || K < 0) return RA_ERR_INVALID_ARG;
+    return RA_OK;
+}
+
+static ra_status make_plan(int transA, int transB, int M, int N, int K, const ra_occupancy* occ_in, Plan* out) {
+    RA_TRY(validate_shape(transA, transB, M, N, K));
+    if (transA != 0 || transB != 1) return RA_ERR_UNSUPPORTED;   // K-contiguous operands only (A13)
+    ra_occupancy occ = {0, 0, 0, 1};
+    if (occ_in) occ = *occ_in;
+    if (occ.smem_reserve_bytes < 0 || occ.sm_budget < 0 || occ.tiles_per_cta < 0) return RA_ERR_INVALID_ARG;
+
+    // device facts (B200 constants when no device is present, so plans can be queried on a CPU box)
+    int sm_count = kDefaultSmCount, smem_per_sm = kDefaultSmemPerSm, optin = kDefaultSmemPerBlockOptin,
+        reserved = kDefaultSmemReservedPerBlock;
+    {
+        DeviceInfo di;
+        if (device_info(&di) == RA_OK) {
+            sm_count = di.sm_count;
+            smem_per_sm = di.smem_per_sm;
+            optin = di.smem_per_block_optin;
+            reserved = di.smem_reserved_per_block;
+        } else {
+            g_last_cuda_error = 0;
+            (void)cudaGetLastError();
+        }
+    }
+    Plan pl{};
+    ra_gemm_plan& g = pl.pub;
+    int clamped = 0;
+
+    int budget = occ.sm_budget == 0 ? sm_count : occ.sm_budget;
+    if (budget > sm_count) {
+        if (!occ.allow_clamp) return RA_ERR_INFEASIBLE_KNOB;
+        budget = sm_count;
+        clamped = 1;
+    }
+
+    const int swap = (M <= 64 && N >= 128) ? 1 : 0;
+    const int RX = swap ? N : M, RY = swap ? M : N;
+    int bn = RY > 128 ? 256 : (RY > 64 ? 128 : 64);
+
+    // shared memory the GEMM may allocate on an SM
+    long avail = (long)smem_per_sm - occ.smem_reserve_bytes - reserved;
+    if (avail > optin) avail = optin;
+    int stages = 0;
+    for (;;) {
+        const long room = avail - kAlignSlack - kBarrierBytes;
+        stages = room > 0 ? (int)(room / stage_bytes(bn)) : 0;
+        if (stages > kMaxStages) stages = kMaxStages;
+        if (stages >= 2 || bn == 64) break;
+        bn >>= 1;   // squeeze the tile before giving up pipelining
+    }
+    if (stages < 1) {
+        if (!occ.allow_clamp) return RA_ERR_INFEASIBLE_KNOB;
+        stages = 1;
+        clamped = 1;
+    }
+    int dyn = dyn_smem_for(bn, stages);
+
+    const int tiles_x = (RX + kBM - 1) / kBM, tiles_y = (RY + bn - 1) / bn;
+    const long long n_tiles = (long long)tiles_x * tiles_y;
+    if (n_tiles > 0x7fffffffLL) return RA_ERR_UNSUPPORTED;
+    const int kb = (K + kBK - 1) / kBK;
+
+    int grid, stream_k = 0, ctas_per_sm = 1;
+    if (occ.tiles_per_cta > 0) {
+        // bounded work: more CTAs than SMs.  Residency must stay at one GEMM CTA per SM (TMEM holds
+        // two accumulators), so pad the request past half of what an SM can give.
+        grid = (int)((n_tiles + occ.tiles_per_cta - 1) / occ.tiles_per_cta);
+        const int half = (smem_per_sm - 2 * reserved) / 2 + 16;
+        if (dyn < half) {
+            if (half > avail) {
+                if (!occ.allow_clamp) return RA_ERR_INFEASIBLE_KNOB;
+                clamped = 1;
+            }
+            dyn = half;
+        }
+    } else {
+        grid = (int)(n_tiles < budget ? n_tiles : budget);
+        if (grid < 1) grid = 1;
+        // wave-quantisation efficiency of the data-parallel schedule on `budget` CTAs; below 90 %
+        // (MB: 128 tiles on 148 SMs) the k-block units are cut evenly instead (stream-K).
+        const long long U = n_tiles * kb;
+        const long long waves = (n_tiles + budget - 1) / budget;
+        const double eff = waves > 0 ? (double)n_tiles / (double)(waves * budget) : 1.0;
+        if (n_tiles > 0 && kb >= 8 && eff < 0.9) {
+            stream_k = 1;
+            grid = budget;
+            if ((long long)grid * 4 > U) grid = (int)(U / 4);   // at least 4 k-blocks per CTA
+        }
+    }
+    g.ctas_per_sm = ctas_per_sm;
+    g.grid = grid;
+    g.stages = stages;
+    g.tile_m = swap ? bn : kBM;
+    g.tile_n = swap ? kBM : bn;
+    g.tile_k = kBK;
+    g.swap_ab = swap;
+    g.dyn_smem_bytes = dyn;
+    g.smem_left_per_sm = smem_per_sm - ctas_per_sm * (dyn + reserved);
+    g.n_tiles = (int)n_tiles;
+    g.clamped = clamped;
+    g.split_k = 1;
+    pl.bn = bn;
+    if (stream_k) {
+        const long long U = n_tiles * kb;
+        // max number of CTA ranges one tile can span
+        const long long per = U / grid;   // >= 4
+        g.split_k = (int)((kb + per - 1) / per + 1);
+        pl.counters_bytes = (((size_t)n_tiles * sizeof(int)) + 1023) & ~(size_t)1023;
+        pl.ws_bytes = pl.counters_bytes + (size_t)2 * grid * kBM * bn * sizeof(float);
+    }
+    *out = pl;
+    return RA_OK;
+}
+
+template <int BN>
+static ra_status launch_gemm(const CUtensorMap& mx, const CUtensorMap& my, const GemmParams& p, int grid, int dyn,
+                             cudaStream_t stream) {
+    RA_CUDA(cudaFuncSetAttribute(gemm_kernel<BN>, cudaFuncAttributeMaxDynamicSharedMemorySize, dyn));
+    gemm_kernel<BN><<<grid, kGemmThreads, dyn, stream>>>(mx, my, p, g_trace);
+    RA_CUDA(cudaGetLastError());
+    return RA_OK;
+}
+
+ra_status gemm_launch(int transA, int transB, int M, int N, int K, float alpha, const void* A, int lda, const void* B,
+                      int ldb, float beta, void* C, int ldc, const ra_occupancy* occ, void* workspace,
+                      size_t workspace_bytes, cudaStream_t stream, ra_gemm_plan* plan_out) {
+    RA_TRY(validate_shape(transA, transB, M, N, K));
+    if (M == 0 || N == 0) return RA_OK;
+    if (A == nullptr || B == nullptr || C == nullptr) return RA_ERR_INVALID_ARG;
+    const int min_lda = transA ? M : K, min_ldb = transB ? K : N;
+    if (lda < (min_lda > 1 ? min_lda : 1) || ldb < (min_ldb > 1 ? min_ldb : 1) || ldc < N) return RA_ERR_INVALID_ARG;
+    if ((reinterpret_cast<uintptr_t>(A) & 15u) || (reinterpret_cast<uintptr_t>(B) & 15u) ||
+        (reinterpret_cast<uintptr_t>(C) & 15u))
+        return RA_ERR_INVALID_ARG;
+    if ((lda % 8) || (ldb % 8) || (ldc % 8)) return RA_ERR_UNSUPPORTED;
+    {
+        // C must not overlap A or B
+        const uintptr_t c0 = reinterpret_cast<uintptr_t>(C), c1 = c0 + ((size_t)(M - 1) * ldc + N) * 2;
+        const size_t a_elems = transA ? ((size_t)(K > 0 ? K - 1 : 0) * lda + M) : ((size_t)(M - 1) * lda + K);
+        const size_t b_elems = transB ? ((size_t)(N - 1) * ldb + K) : ((size_t)(K > 0 ? K - 1 : 0) * ldb + N);
+        const uintptr_t a0 = reinterpret_cast<uintptr_t>(A), a1 = a0 + a_elems * 2;
+        const uintptr_t b0 = reinterpret_cast<uintptr_t>(B), b1 = b0 + b_elems * 2;
+        if (K > 0 && ((c0 < a1 && a0 < c1) || (c0 < b1 && b0 < c1))) return RA_ERR_INVALID_ARG;
+    }
+    Plan pl;
+    RA_TRY(make_plan(transA, transB, M, N, K, occ, &pl));
+    if (pl.ws_bytes > 0) {
+        if (workspace == nullptr || workspace_bytes < pl.ws_bytes || (reinterpret_cast<uintptr_t>(workspace) & 15u))
+            return RA_ERR_INVALID_ARG;
+    }
+    DeviceInfo di;
+    RA_TRY(device_info(&di));
+    RA_TRY(require_sm100(di));
+    if (plan_out) *plan_out = pl.pub;
+
+    if (K == 0 || alpha == 0.f) {
+        const size_t total = (size_t)M * N;
+        const int blocks = (int)((total + 255) / 256 < (size_t)di.sm_count * 8 ? (total + 255) / 256 : (size_t)di.sm_count * 8);
+        scale_c_kernel<<<blocks, 256, 0, stream>>>(static_cast<__nv_bfloat16*>(C), M, N, ldc, beta);
+        RA_CUDA(cudaGetLastError());
+        return RA_OK;
+    }
+
+    const int swap = pl.pub.swap_ab;
+    GemmParams p{};
+    p.RX = swap ? N : M;
+    p.RY = swap ? M : N;
+    p.K = K;
+    p.tiles_x = (p.RX + kBM - 1) / kBM;
+    p.tiles_y = (p.RY + pl.bn - 1) / pl.bn;
+    p.n_tiles = pl.pub.n_tiles;
+    p.kb_per_tile = (K + kBK - 1) / kBK;
+    p.swap = swap;
+    p.stream_k = pl.pub.split_k > 1;
+    p.stages = pl.pub.stages;
+    p.alpha = alpha;
+    p.beta = beta;
+    p.C = static_cast<__nv_bfloat16*>(C);
+    p.ldc = ldc;
+    // L2 policy: an operand that is streamed exactly once (one tile along the other dimension) should
+    // not displace anything; the small operand every CTA re-reads should stay.
+    p.hintX = (p.tiles_y == 1 && p.tiles_x > 1) ? 1 : 0;
+    p.hintY = (p.tiles_y == 1 && p.tiles_x > 1) ? 2 : 0;
+    if (p.stream_k) {
+        p.counters = static_cast<int*>(workspace);
+        p.partials = reinterpret_cast<float*>(static_cast<uint8_t*>(workspace) + pl.counters_bytes);
+        RA_CUDA(cudaMemsetAsync(workspace, 0, pl.counters_bytes, stream));
+    }
+    const void* X = swap ? B : A;
+    const void* Y = swap ? A : B;
+    const int ldx = swap ? ldb : lda, ldy = swap ? lda : ldb;
+    CUtensorMap mx, my;
+    RA_TRY(make_map(&mx, X, p.RX, K, ldx, kBM));
+    RA_TRY(make_map(&my, Y, p.RY, K, ldy, pl.bn));
+    switch (pl.bn) {
+        case 64: return launch_gemm<64>(mx, my, p, pl.pub.grid, pl.pub.dyn_smem_bytes, stream);
+        case 128: return launch_gemm<128>(mx, my, p, pl.pub.grid, pl.pub.dyn_smem_bytes, stream);
+        case 256: return launch_gemm<256>(mx, my, p, pl.pub.grid, pl.pub.dyn_smem_bytes, stream);
+    }
+    return RA_ERR_UNSUPPORTED;
+}
+
+}  // namespace ra
+
+extern "C" {
+
+ra_status ra_gemm_plan_query(int transA, int transB, int M, int N, int K, const ra_occupancy* occ, ra_gemm_plan* out) {
+    if (out == nullptr) return RA_ERR_INVALID_ARG;
+    ra::Plan pl;
+    RA_TRY(ra::make_plan(transA, transB, M, N, K, occ, &pl));
+    *out = pl.pub;
+    return RA_OK;
+}
+
+size_t ra_gemm_workspace_bytes(int transA, int transB, int M, int N, int K, const ra_occupancy* occ) {
+    ra::Plan pl;
+    if (ra::make_plan(transA, transB, M, N, K, occ, &pl) != RA_OK) return 0;
+    return pl.ws_bytes;
+}
+
+ra_status ra_gemm(int transA, int transB, int M, int N, int K, float alpha, const void* A, int lda, const void* B,
+                  int ldb, float beta, void* C, int ldc, const ra_occupancy* occ, void* workspace,
+                  size_t workspace_bytes, void* stream) {
+    return ra::gemm_launch(transA, transB, M, N, K, alpha, A, lda, B, ldb, beta, C, ldc, occ, workspace,
+                           workspace_bytes, static_cast<cudaStream_t>(stream), nullptr);
+}
+
+}  // extern "C"
