@@ -111,8 +111,19 @@ __device__ __forceinline__ bool mbar_try_wait(uint32_t bar, uint32_t parity) {
         : "memory");
     return ok != 0;
 }
+// Bounded wait: a protocol bug (wrong phase, lost arrive) must surface as a trapped launch
+// (cudaErrorLaunchFailure -> RA_ERR_CUDA), never as a hung GPU.  The clock is only read on the
+// slow path (every 4096 failed probes), so the common case costs nothing.
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+    if (mbar_try_wait(bar, parity)) return;
+    uint64_t t0 = 0;
+    uint32_t spins = 0;
     while (!mbar_try_wait(bar, parity)) {
+        if ((++spins & 4095u) == 0) {
+            const uint64_t now = globaltimer();
+            if (t0 == 0) t0 = now;
+            else if (now - t0 > 5000000000ull) __trap();   // 5 s
+        }
     }
 }
 

@@ -1,0 +1,141 @@
+"""CPU-only checks of the boundary: libra.so loads, exports every symbol include/ra.h declares, the planner
+(host logic of S3) behaves, argument errors are reported before any CUDA call, and nothing in the product
+imports the oracle."""
+import ctypes
+import os
+import re
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def ra():
+    import paper_2606_09200_b200 as m
+    return m
+
+
+def _header_functions():
+    src = open(os.path.join(ROOT, "include", "ra.h")).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    return sorted(set(re.findall(r"\b(ra_[a-z0-9_]+)\s*\(", src)))
+
+
+def test_library_exports_every_declared_symbol(ra):
+    lib = ctypes.CDLL(ra.lib_path())
+    names = _header_functions()
+    assert {"ra_gemm", "ra_allreduce_emul", "ra_alltoall_emul", "ra_overlap_run"} <= set(names)
+    for n in names:
+        assert hasattr(lib, n), n
+    assert sorted(ra.EXPORTS) == names            # the binding covers exactly the header
+
+
+def test_status_strings(ra):
+    assert [ra.status_str(i) for i in range(6)] == ["RA_OK", "RA_ERR_INVALID_ARG", "RA_ERR_UNSUPPORTED",
+                                                     "RA_ERR_INFEASIBLE_KNOB", "RA_ERR_CUDA", "RA_ERR_ARCH"]
+
+
+def test_struct_layouts_match_header(ra):
+    # sizes computed by hand from include/ra.h (LP64)
+    assert ctypes.sizeof(ra.Occupancy) == 16
+    assert ctypes.sizeof(ra.GemmPlan) == 48
+    assert ctypes.sizeof(ra.Workload) == 152
+    assert ctypes.sizeof(ra.OverlapCfg) == 4 + 16 + 8 * 4
+    assert ctypes.sizeof(ra.OverlapResult) == 24 + 48 + 8
+
+
+KB = 1024
+
+
+@pytest.mark.parametrize("shape", [(8192, 8192, 8192), (64, 16384, 16384), (256, 256, 256), (200, 136, 72)])
+@pytest.mark.parametrize("reserve", [0, 32 * KB, 64 * KB, 96 * KB, 128 * KB, 160 * KB, 200 * KB])
+@pytest.mark.parametrize("budget", [0, 74, 110, 148])
+def test_plan_honours_reserve_and_budget(ra, shape, reserve, budget):
+    M, N, K = shape
+    p = ra.ra_gemm_plan_query(0, 1, M, N, K, dict(smem_reserve_bytes=reserve, sm_budget=budget))
+    assert p["smem_left_per_sm"] >= reserve, p                     # S3: the GEMM leaves the reserve unallocated
+    assert p["stages"] >= 1 and p["tile_k"] == 64
+    assert p["grid"] <= (budget or 148)
+    assert p["dyn_smem_bytes"] <= 227 * KB
+    tiles = -(-M // p["tile_m"]) * -(-N // p["tile_n"])
+    assert p["n_tiles"] == tiles
+    ws = ra.ra_gemm_workspace_bytes(0, 1, M, N, K, dict(smem_reserve_bytes=reserve, sm_budget=budget))
+    assert (ws > 0) == (p["split_k"] > 1)
+
+
+def test_plan_depth_shrinks_with_reserve(ra):
+    stages = [ra.ra_gemm_plan_query(0, 1, 8192, 8192, 8192, dict(smem_reserve_bytes=r * KB))["stages"] for r in (0, 64, 112)]
+    assert stages == sorted(stages, reverse=True) and stages[0] == 4
+    mb = [ra.ra_gemm_plan_query(0, 1, 64, 16384, 16384, dict(smem_reserve_bytes=r * KB)) for r in (0, 64, 128, 200)]
+    assert [p["stages"] for p in mb] == sorted((p["stages"] for p in mb), reverse=True)
+    assert all(p["swap_ab"] == 1 and p["tile_m"] == 64 for p in mb)
+    assert mb[0]["split_k"] > 1                                     # 128 tiles on 148 SMs -> stream-K
+
+
+def test_plan_infeasible_knob(ra):
+    with pytest.raises(ra.RaError) as e:
+        ra.ra_gemm_plan_query(0, 1, 512, 512, 512, dict(smem_reserve_bytes=226 * KB, allow_clamp=0))
+    assert e.value.status == ra.RA_ERR_INFEASIBLE_KNOB
+    p = ra.ra_gemm_plan_query(0, 1, 512, 512, 512, dict(smem_reserve_bytes=226 * KB, allow_clamp=1))
+    assert p["clamped"] == 1 and p["stages"] == 1
+    with pytest.raises(ra.RaError):
+        ra.ra_gemm_plan_query(0, 1, 512, 512, 512, dict(sm_budget=1000, allow_clamp=0))
+    assert ra.ra_gemm_plan_query(0, 1, 512, 512, 512, dict(sm_budget=1000))["clamped"] == 1
+
+
+def test_bounded_work_mode_grid(ra):
+    p = ra.ra_gemm_plan_query(0, 1, 8192, 8192, 8192, dict(tiles_per_cta=4))
+    assert p["grid"] == 2048 // 4 and p["split_k"] == 1
+    assert 2 * (p["dyn_smem_bytes"] + 1024) > 228 * KB               # a second GEMM CTA cannot fit on the SM
+
+
+def test_argument_errors_need_no_gpu(ra):
+    fake = 0x10000
+    lib = ra._L()
+    P = ctypes.POINTER(ctypes.c_void_p)
+    arr = (ctypes.c_void_p * 2)(fake, fake + 4096)
+    assert lib.ra_allreduce_emul(None, 2, 16, 0, None) == ra.RA_ERR_INVALID_ARG
+    assert lib.ra_allreduce_emul(arr, 0, 16, 0, None) == ra.RA_ERR_INVALID_ARG
+    assert lib.ra_allreduce_emul(arr, 2, 4096, 0, None) == ra.RA_ERR_INVALID_ARG        # buffers overlap
+    assert lib.ra_allreduce_emul((ctypes.c_void_p * 2)(fake + 4, fake + 4096), 2, 16, 0, None) == ra.RA_ERR_INVALID_ARG
+    assert lib.ra_allreduce_emul(arr, 2, 0, 0, None) == ra.RA_OK                        # count == 0: nothing to do
+    assert lib.ra_alltoall_emul(fake, fake + 64, 2, 64, 0, None) == ra.RA_ERR_INVALID_ARG  # overlap
+    assert lib.ra_alltoall_emul(fake, fake + 4096, 2, 24, 0, None) == ra.RA_ERR_INVALID_ARG
+    assert lib.ra_alltoall_emul(fake, fake + 4096, 2, 0, 0, None) == ra.RA_OK
+    g = dict(transA=0, transB=1, M=32, N=32, K=64, alpha=1.0, A=fake, lda=64, B=fake + (1 << 20), ldb=64, beta=0.0,
+             C=fake + (2 << 20), ldc=32)
+    for kw, st in [(dict(M=-1), 1), (dict(transA=2), 1), (dict(A=None), 1), (dict(lda=8), 1), (dict(ldc=24), 1),
+                   (dict(ldc=36), 2), (dict(A=fake + 2), 1), (dict(transB=0, ldb=64), 2), (dict(M=0), 0)]:
+        a = dict(g, **kw)
+        s = lib.ra_gemm(a["transA"], a["transB"], a["M"], a["N"], a["K"], a["alpha"], a["A"], a["lda"], a["B"], a["ldb"],
+                        a["beta"], a["C"], a["ldc"], None, None, 0, None)
+        assert s == st, (kw, s)
+    assert lib.ra_overlap_run(None, None, None) == ra.RA_ERR_INVALID_ARG
+
+
+def test_compute_fails_loudly_without_device(ra):
+    try:
+        import torch
+        if torch.cuda.is_available():
+            pytest.skip("GPU present")
+    except ImportError:
+        pass
+    arr = (ctypes.c_void_p * 2)(0x10000, 0x20000)
+    s = ra._L().ra_allreduce_emul(arr, 2, 16, 0, None)
+    assert s in (ra.RA_ERR_CUDA, ra.RA_ERR_ARCH)                    # no CPU fallback
+    assert ra.status_str(s).startswith("RA_ERR")
+
+
+def test_product_never_imports_oracle():
+    pkg = os.path.join(ROOT, "paper_2606_09200_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                txt = open(os.path.join(dirpath, f)).read()
+                assert not re.search(r"^\s*(import|from)\s+oracle\b", txt, flags=re.M), f
+                assert "liboracle" not in txt and "oracle.c" not in txt, f
+    for f in os.listdir(os.path.join(ROOT, "oracle")):
+        if f.endswith((".py", ".c")):
+            txt = open(os.path.join(ROOT, "oracle", f)).read()
+            assert "import paper_2606_09200_b200" not in txt and "ra.h" not in txt

@@ -1,0 +1,39 @@
+"""N>1 path of bench.py on CPU: world_size-2 gloo (replicas only -- the hot path does not shard, so there is
+no data-path collective; torch.distributed only provides the barrier and the max-over-ranks of the step time)."""
+import json
+import os
+import socket
+import subprocess
+import sys
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def _free_port():
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        return s.getsockname()[1]
+
+
+def _torchrun(script_args, nproc=2, timeout=600):
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={nproc}", "--master-addr", "127.0.0.1",
+           "--master-port", str(_free_port())] + script_args
+    env = dict(os.environ, CUDA_VISIBLE_DEVICES="", OMP_NUM_THREADS="2")
+    return subprocess.run(cmd, cwd=ROOT, env=env, capture_output=True, text=True, timeout=timeout)
+
+
+def test_gloo_world2_barrier_and_max():
+    r = _torchrun([os.path.join("tests", "_dist_worker.py")])
+    assert r.returncode == 0, r.stderr[-2000:]
+    assert "DIST_OK world=2 max=2.5 value=64.0" in r.stdout
+
+
+def test_reference_arm_world2_prints_one_line():
+    r = _torchrun(["bench.py", "--impl", "reference", "--gpus", "2", "--steps", "1", "--warmup", "0", "--config", "tiny"])
+    assert r.returncode == 0, r.stderr[-2000:]
+    lines = [ln for ln in r.stdout.splitlines() if ln.startswith("{")]
+    assert len(lines) == 1                       # rank 0 alone prints
+    d = json.loads(lines[0])
+    assert d["impl"] == "reference" and d["unit"] == "iter/s" and d["value"] > 0
+    assert d["cpu_baseline"]["kind"] == "oracle" and d["e2e"]["h2d_bytes_per_step"] == 0
+    assert d["config"]["workload"] == "tiny" and d["gpu_launches"] == 0

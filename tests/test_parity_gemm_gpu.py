@@ -1,0 +1,199 @@
+"""GPU parity: K1 tcgen05 GEMM vs the CPU oracle, through the C ABI.
+
+Acceptance (BASELINE.json north_star): max |gpu - ref| / (|alpha| ||opA(i,:)|| ||opB(:,j)|| + |beta||Cin|) <= 1e-2;
+bit-exact where the arithmetic is exact (identity, integer-valued inputs, power-of-two alpha).
+"""
+import numpy as np
+import pytest
+
+import oracle
+import ra_inputs
+from helpers import GEMM_TOL, gemm_norm_err, to_dev, to_host
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def ra():
+    import paper_2606_09200_b200 as m
+    return m
+
+
+def run_gemm(ra, M, N, K, A, B, alpha=1.0, beta=0.0, Cin=None, occ=None, lda=None, ldb=None, ldc=None, fill=None):
+    """A: [M, lda] bits, B: [N, ldb] bits (transA=0, transB=1).  Returns C bits [M, N]."""
+    import torch
+    lda = lda or K
+    ldb = ldb or K
+    ldc = ldc or N
+    dA, dB = to_dev(A), to_dev(B)
+    if Cin is not None:
+        dC = to_dev(Cin)
+    else:
+        dC = torch.full((M, ldc), 0x7FC0 if fill is None else fill, dtype=torch.int16, device="cuda")  # NaN-filled
+    ws_bytes = ra.ra_gemm_workspace_bytes(0, 1, M, N, K, occ)
+    ws = torch.empty(max(ws_bytes, 16), dtype=torch.uint8, device="cuda")
+    ra.ra_gemm(0, 1, M, N, K, alpha, dA, lda, dB, ldb, beta, dC, ldc, occ=occ, workspace=ws)
+    torch.cuda.synchronize()
+    out = to_host(dC, np.uint16).reshape(M, ldc)
+    return out[:, :N].copy(), out
+
+
+def _up8(x):
+    return (x + 7) // 8 * 8
+
+
+def check(ra, M, N, K, seed, alpha=1.0, beta=0.0, occ=None):
+    # leading dimensions rounded up to the 8-element pitch TMA needs; the pad columns hold data too
+    # (so a kernel that ignored ld would read/write the wrong elements)
+    lda = ldb = _up8(K) + (8 if K % 16 else 0)
+    ldc = _up8(N)
+    A = ra_inputs.normal_bf16((M, lda), seed, ra_inputs.STREAM_A)
+    B = ra_inputs.normal_bf16((N, ldb), seed, ra_inputs.STREAM_B)
+    Cin = ra_inputs.normal_bf16((M, ldc), seed, ra_inputs.STREAM_C) if beta != 0.0 else None
+    ref, _ = oracle.gemm(0, 1, M, N, K, alpha, A, B, beta, Cin, lda=lda, ldb=ldb, ldc=ldc)
+    rowA, colB = oracle.gemm_norms(0, 1, M, N, K, A, B, lda=lda, ldb=ldb)
+    got, full = run_gemm(ra, M, N, K, A, B, alpha, beta, Cin, occ, lda=lda, ldb=ldb, ldc=ldc)
+    cin_view = Cin[:, :N] if Cin is not None else None
+    err = gemm_norm_err(got, ref, rowA, colB, alpha, beta, cin_view)
+    assert err <= GEMM_TOL, f"normalised error {err} for {M}x{N}x{K} plan {ra.ra_gemm_plan_query(0, 1, M, N, K, occ)}"
+    if Cin is not None and ldc > N:
+        assert np.array_equal(full[:, N:], Cin[:, N:]), "pad columns of C were modified"
+    return err
+
+
+def test_tiny_config(ra):
+    cfg = ra_inputs.CONFIGS[0]
+    A, B = ra_inputs.gemm_operands(cfg)
+    ref, _ = oracle.gemm(0, 1, cfg.M, cfg.N, cfg.K, 1.0, A, B)
+    rowA, colB = oracle.gemm_norms(0, 1, cfg.M, cfg.N, cfg.K, A, B)
+    got, _ = run_gemm(ra, cfg.M, cfg.N, cfg.K, A, B)
+    assert gemm_norm_err(got, ref, rowA, colB) <= GEMM_TOL
+
+
+@pytest.mark.parametrize("M,N,K", [
+    (128, 256, 64), (128, 64, 128), (256, 512, 256),          # whole tiles, each BN
+    (200, 136, 72), (1, 8, 8), (130, 260, 200), (77, 40, 1000),  # ragged M, N, K tails
+    (384, 768, 4096),                                          # several tiles per CTA? (6 tiles)
+    (64, 1024, 2048), (17, 640, 1536), (64, 128, 512),         # skinny-M: operand swap (+ stream-K)
+    (300, 200, 8192),                                          # stream-K on the non-swapped path
+])
+def test_shapes(ra, M, N, K):
+    check(ra, M, N, K, seed=1000 + M + N + K)
+
+
+@pytest.mark.parametrize("alpha,beta", [(1.0, 1.0), (-0.5, 2.0), (2.0, -0.5), (0.0, 1.0), (0.0, 0.0), (1.0, 0.0)])
+@pytest.mark.parametrize("M,N,K", [(200, 136, 72), (64, 1024, 2048)])
+def test_alpha_beta(ra, alpha, beta, M, N, K):
+    check(ra, M, N, K, seed=5, alpha=alpha, beta=beta)
+
+
+def test_identity_bit_exact(ra):
+    # A = I  =>  C == B^T exactly (every product exact, every sum adds zeros).
+    n = 256
+    eye = ra_inputs.f32_to_bf16_bits_exact(np.eye(n, dtype=np.float32))
+    Bm = ra_inputs.normal_bf16((384, n), 11, ra_inputs.STREAM_B)        # B is N x K
+    got, _ = run_gemm(ra, n, 384, n, eye, Bm)
+    assert np.array_equal(got, Bm.T)
+    got, _ = run_gemm(ra, 384, n, n, Bm, eye)                           # B = I  =>  C == A
+    assert np.array_equal(got, Bm)
+
+
+@pytest.mark.parametrize("M,N,K", [(256, 256, 256), (200, 520, 4096), (64, 2048, 16384), (128, 256, 16384)])
+def test_integer_exact(ra, M, N, K):
+    # entries in {-2..2}: all partial sums are integers < 2^24 -> fp32 accumulation is exact in any order,
+    # so the bf16 result must equal the oracle's bf16 rounding bit for bit (strongest layout/index pin).
+    A = ra_inputs.smallint_bf16((M, K), 31, ra_inputs.STREAM_A)
+    B = ra_inputs.smallint_bf16((N, K), 31, ra_inputs.STREAM_B)
+    _, ref16 = oracle.gemm(0, 1, M, N, K, 1.0, A, B)
+    got, _ = run_gemm(ra, M, N, K, A, B)
+    assert np.array_equal(got, ref16)
+
+
+def test_ones_closed_form(ra):
+    for K in (256, 8192):
+        one = ra_inputs.f32_to_bf16_bits_exact(np.ones((130, K), np.float32))
+        got, _ = run_gemm(ra, 130, 130, K, one, one)
+        assert np.all(ra_inputs.bf16_bits_to_f32(got) == np.float32(K))
+
+
+def test_beta0_ignores_nan_in_c_and_respects_ldc(ra):
+    M, N, K, ldc = 100, 72, 256, 96
+    A = ra_inputs.normal_bf16((M, K), 3, ra_inputs.STREAM_A)
+    B = ra_inputs.normal_bf16((N, K), 3, ra_inputs.STREAM_B)
+    got, full = run_gemm(ra, M, N, K, A, B, ldc=ldc)
+    assert not np.any((got & 0x7FFF) > 0x7F80)              # no NaN leaked from the NaN-filled C
+    assert np.all(full[:, N:] == 0x7FC0)                    # padding columns untouched
+    ref, _ = oracle.gemm(0, 1, M, N, K, 1.0, A, B)
+    rowA, colB = oracle.gemm_norms(0, 1, M, N, K, A, B)
+    assert gemm_norm_err(got, ref, rowA, colB) <= GEMM_TOL
+
+
+def test_alpha_power_of_two_linearity(ra):
+    M, N, K = 192, 320, 512
+    A = ra_inputs.normal_bf16((M, K), 9, ra_inputs.STREAM_A)
+    B = ra_inputs.normal_bf16((N, K), 9, ra_inputs.STREAM_B)
+    c1, _ = run_gemm(ra, M, N, K, A, B, alpha=1.0)
+    c2, _ = run_gemm(ra, M, N, K, A, B, alpha=2.0)
+    assert np.array_equal(ra_inputs.bf16_bits_to_f32(c2), 2.0 * ra_inputs.bf16_bits_to_f32(c1))
+
+
+@pytest.mark.parametrize("occ", [
+    dict(smem_reserve_bytes=0, sm_budget=74), dict(smem_reserve_bytes=64 * 1024, sm_budget=148),
+    dict(smem_reserve_bytes=128 * 1024, sm_budget=110), dict(smem_reserve_bytes=160 * 1024, sm_budget=92),
+    dict(smem_reserve_bytes=200 * 1024, sm_budget=148), dict(tiles_per_cta=1), dict(tiles_per_cta=3, smem_reserve_bytes=32 * 1024),
+    dict(sm_budget=1), dict(sm_budget=7),
+])
+@pytest.mark.parametrize("M,N,K", [(512, 768, 1024), (64, 2048, 4096)])
+def test_knobs_do_not_change_results(ra, occ, M, N, K):
+    # PAPER.md:47 "without modifying kernel logic": occupancy shaping must not change what is computed.
+    plan = ra.ra_gemm_plan_query(0, 1, M, N, K, occ)
+    assert plan["smem_left_per_sm"] >= occ.get("smem_reserve_bytes", 0) or plan["clamped"]
+    check(ra, M, N, K, seed=77, occ=occ)
+
+
+def test_run_to_run_reproducible_stream_k(ra):
+    M, N, K = 64, 4096, 8192
+    assert ra.ra_gemm_plan_query(0, 1, M, N, K)["split_k"] > 1
+    A = ra_inputs.normal_bf16((M, K), 21, ra_inputs.STREAM_A)
+    B = ra_inputs.normal_bf16((N, K), 21, ra_inputs.STREAM_B)
+    first, _ = run_gemm(ra, M, N, K, A, B)
+    for _ in range(5):
+        again, _ = run_gemm(ra, M, N, K, A, B)
+        assert np.array_equal(first, again)
+
+
+def test_budget_bit_identical_data_parallel(ra):
+    # sm_budget / tiles_per_cta only change which CTA computes a tile.
+    M, N, K = 1024, 1024, 512
+    A = ra_inputs.normal_bf16((M, K), 22, ra_inputs.STREAM_A)
+    B = ra_inputs.normal_bf16((N, K), 22, ra_inputs.STREAM_B)
+    base, _ = run_gemm(ra, M, N, K, A, B, occ=dict(sm_budget=32))
+    for occ in (dict(sm_budget=16), dict(sm_budget=8, smem_reserve_bytes=100 * 1024), dict(tiles_per_cta=2)):
+        plan = ra.ra_gemm_plan_query(0, 1, M, N, K, occ)
+        if plan["split_k"] > 1 or plan["tile_n"] != 256:
+            continue
+        got, _ = run_gemm(ra, M, N, K, A, B, occ=occ)
+        assert np.array_equal(base, got)
+
+
+def test_errors(ra):
+    import torch
+    a = torch.zeros(64 * 64, dtype=torch.int16, device="cuda")
+    b = torch.zeros(64 * 64, dtype=torch.int16, device="cuda")
+    c = torch.zeros(64 * 64, dtype=torch.int16, device="cuda")
+    for kw, st in [
+        (dict(transA=1), ra.RA_ERR_UNSUPPORTED), (dict(lda=60), ra.RA_ERR_INVALID_ARG), (dict(lda=68), ra.RA_ERR_UNSUPPORTED),
+        (dict(M=-1), ra.RA_ERR_INVALID_ARG), (dict(C=a), ra.RA_ERR_INVALID_ARG),
+    ]:
+        args = dict(transA=0, transB=1, M=32, N=32, K=64, alpha=1.0, A=a, lda=64, B=b, ldb=64, beta=0.0, C=c, ldc=64)
+        args.update(kw)
+        with pytest.raises(ra.RaError) as e:
+            ra.ra_gemm(**args)
+        assert e.value.status == st, kw
+    ra.ra_gemm(0, 1, 0, 32, 64, 1.0, a, 64, b, 64, 0.0, c, 64)     # M == 0: nothing to do
+    # K == 0: C = beta*C
+    c.fill_(0x3F80)  # 1.0
+    ra.ra_gemm(0, 1, 32, 32, 0, 1.0, a, 8, b, 8, 2.0, c, 64)
+    torch.cuda.synchronize()
+    out = to_host(c, np.uint16).reshape(64, 64)
+    assert np.all(out[:32, :32] == 0x4000) and np.all(out[:32, 32:] == 0x3F80)
