@@ -190,12 +190,23 @@ def cfg_label(kw):
 def kernels_alone(ra, cfg, d, h, peaks, n_iters):
     """Each kernel by itself (CUDA events inside the library, on the stream the kernel runs on)."""
     out = {}
+    # burst: single launches with idle gaps, best of 10 (how MEASURED_PEAKS.json's burst figure was taken)
+    w1, keep1 = make_workload(ra, cfg, d, 1, coll=False)
+    burst = []
+    for _ in range(12):
+        time.sleep(0.05)
+        burst.append(ra.ra_overlap_run(w1, ra.make_cfg(mode=0))["total_ms"])
+    gb_ms = min(burst[2:])
+    out["gemm_ms_burst"] = gb_ms
+    out["gemm_tflops_burst"] = cfg.gemm_flops / gb_ms / 1e9
+    out["gemm_frac_of_bf16_peak_burst"] = out["gemm_tflops_burst"] / peaks["bf16_tflops"]
+    # sustained: back-to-back launches (power-capped regime)
     w, keep = make_workload(ra, cfg, d, n_iters, coll=False)
     res, _ = ra.ra_overlap_sweep(w, [ra.make_cfg(mode=0)], runs=6)
     g_ms = res[0]["total_ms"] / n_iters
     out["gemm_ms"] = g_ms
     out["gemm_tflops"] = cfg.gemm_flops / g_ms / 1e9
-    out["gemm_frac_of_bf16_peak_burst"] = out["gemm_tflops"] / peaks["bf16_tflops"]
+    out["gemm_frac_of_bf16_peak_sustained"] = out["gemm_tflops"] / peaks["bf16_tflops_sustained"]
     out["gemm_gbs"] = cfg.gemm_bytes / g_ms / 1e6
     out["gemm_frac_of_hbm_peak"] = out["gemm_gbs"] / peaks["hbm_gbs"]
     out["gemm_plan"] = res[0]["plan"]
@@ -413,7 +424,7 @@ def run_ours(args, cfg):
         ach = flops / gemm_in_step_ms / 1e9
         roof = {"kernel": "ra::gemm_kernel", "bound": "tensor", "achieved": ach, "peak": peaks["bf16_tflops_sustained"], "unit": "TFLOP/s",
                 "frac": ach / peaks["bf16_tflops_sustained"], "traffic": None, "peak_source": f"{peaks['source']} (sustained: kernel timed inside a long overlapped step)",
-                "launch_ms": gemm_in_step_ms, "alone": {"achieved": alone["gemm_tflops"], "peak": peaks["bf16_tflops"], "frac": alone["gemm_frac_of_bf16_peak_burst"], "peak_kind": "burst"}}
+                "launch_ms": gemm_in_step_ms, "alone": {"achieved": alone["gemm_tflops_burst"], "peak": peaks["bf16_tflops"], "frac": alone["gemm_frac_of_bf16_peak_burst"], "peak_kind": "burst (best of 10 single launches)"}}
     else:
         ach = gbytes / gemm_in_step_ms / 1e6
         roof = {"kernel": "ra::gemm_kernel", "bound": "hbm", "achieved": ach, "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": ach / peaks["hbm_gbs"],

@@ -111,8 +111,8 @@ def test_integer_exact(ra, M, N, K):
 
 def test_ones_closed_form(ra):
     for K in (256, 8192):
-        one = ra_inputs.f32_to_bf16_bits_exact(np.ones((130, K), np.float32))
-        got, _ = run_gemm(ra, 130, 130, K, one, one)
+        one = ra_inputs.f32_to_bf16_bits_exact(np.ones((136, K), np.float32))
+        got, _ = run_gemm(ra, 130, 136, K, one, one)
         assert np.all(ra_inputs.bf16_bits_to_f32(got) == np.float32(K))
 
 
