@@ -75,6 +75,8 @@ typedef struct {
     int32_t sm_budget;
     int32_t tiles_per_cta;
     int32_t allow_clamp;
+    int32_t cta_group;        /* 0 = planner decides; 1 = single-CTA tiles (128 x N); 2 = CTA pairs (tcgen05
+                                 cta_group::2, 256 x 256 tiles, 2-CTA clusters) where the shape allows */
 } ra_occupancy;
 
 /* What S3 decided -- for tests, logs and the sweep tables. */
@@ -89,9 +91,10 @@ typedef struct {
     int32_t smem_left_per_sm; /* smem_per_sm - ctas_per_sm*(dyn_smem_bytes + reserved_per_block) */
     int32_t n_tiles;          /* output tiles */
     int32_t clamped;          /* 1 if a knob was clamped */
+    int32_t cta_group;        /* 1, or 2 = CTA pairs: `grid` counts CTAs (2 per tile), sm_budget rounded down to even */
 } ra_gemm_plan;
 
-/* Host-only: computes the plan ra_gemm would use.  `occ` NULL = defaults {0,0,0,1}. */
+/* Host-only: computes the plan ra_gemm would use.  `occ` NULL = defaults {0,0,0,1,0}. */
 ra_status ra_gemm_plan_query(int transA, int transB, int M, int N, int K, const ra_occupancy* occ, ra_gemm_plan* out);
 
 /* Bytes of device workspace ra_gemm needs for this problem and knob setting (0 if none).

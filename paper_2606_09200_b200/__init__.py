@@ -39,12 +39,12 @@ class RaError(RuntimeError):
 
 class Occupancy(Structure):
     _fields_ = [("smem_reserve_bytes", c_int32), ("sm_budget", c_int32), ("tiles_per_cta", c_int32),
-                ("allow_clamp", c_int32)]
+                ("allow_clamp", c_int32), ("cta_group", c_int32)]
 
 
 class GemmPlan(Structure):
     _fields_ = [(n, c_int32) for n in ("ctas_per_sm", "grid", "stages", "tile_m", "tile_n", "tile_k", "split_k",
-                                       "swap_ab", "dyn_smem_bytes", "smem_left_per_sm", "n_tiles", "clamped")]
+                                       "swap_ab", "dyn_smem_bytes", "smem_left_per_sm", "n_tiles", "clamped", "cta_group")]
 
     def as_dict(self):
         return {n: getattr(self, n) for n, _ in self._fields_}
@@ -148,7 +148,7 @@ def _occ(occ) -> Occupancy | None:
     if occ is None or isinstance(occ, Occupancy):
         return occ
     return Occupancy(int(occ.get("smem_reserve_bytes", 0)), int(occ.get("sm_budget", 0)),
-                     int(occ.get("tiles_per_cta", 0)), int(occ.get("allow_clamp", 1)))
+                     int(occ.get("tiles_per_cta", 0)), int(occ.get("allow_clamp", 1)), int(occ.get("cta_group", 0)))
 
 
 def _occ_ref(occ):
@@ -253,7 +253,7 @@ def make_cfg(mode=RA_MODE_OVERLAP, occ=None, coll_sm_budget=0, coll_smem_bytes=0
              prio_compute=0, prio_comm=0, dependent=1, record_kernel_times=0) -> OverlapCfg:
     c = OverlapCfg()
     c.mode = int(mode)
-    c.occ = _occ(occ) or Occupancy(0, 0, 0, 1)
+    c.occ = _occ(occ) or Occupancy(0, 0, 0, 1, 0)
     c.coll_sm_budget, c.coll_smem_bytes = int(coll_sm_budget), int(coll_smem_bytes)
     c.coll_ctas_per_sm, c.coll_variant = int(coll_ctas_per_sm), int(coll_variant)
     c.prio_compute, c.prio_comm = int(prio_compute), int(prio_comm)

@@ -47,7 +47,8 @@ constexpr int kBarrierBytes = 256;
 constexpr int kAlignSlack = 1024;
 constexpr int kGroupX = 16;     // rasterisation: X-tiles per group
 
-__host__ __device__ constexpr int stage_bytes(int bn) { return (kBM + bn) * kBK * 2; }
+// bytes of one pipeline stage in ONE CTA: 128 rows of X + bn/cg rows of Y, 64 bf16 each
+__host__ __device__ constexpr int stage_bytes(int bn, int cg) { return (kBM + bn / cg) * kBK * 2; }
 
 struct GemmParams {
     int RX, RY, K;
@@ -67,13 +68,47 @@ struct GemmParams {
 __device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
 
+// ---- cluster (CTA pair) helpers ------------------------------------------------------------------
+__device__ __forceinline__ uint32_t cluster_ctarank() {
+    uint32_t r;
+    asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
+    return r;
+}
+__device__ __forceinline__ void cluster_sync_all() {
+    asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory");
+    asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+// shared::cluster address of the same shared-memory offset in CTA `rank` of the cluster
+__device__ __forceinline__ uint32_t mapa(uint32_t addr, uint32_t rank) {
+    uint32_t r;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(addr), "r"(rank));
+    return r;
+}
+// arrive (+ expect_tx) on a barrier given by its shared::cluster address (may live in the peer CTA)
+__device__ __forceinline__ void mbar_expect_tx_cluster(uint32_t bar_cluster, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cluster.b64 _, [%0], %1;" ::"r"(bar_cluster), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_cluster(uint32_t bar_cluster) {
+    asm volatile("mbarrier.arrive.shared::cluster.b64 _, [%0];" ::"r"(bar_cluster) : "memory");
+}
+
+// TMA tile load.  CG == 2: the .cta_group::2 form, whose mbarrier may live in the peer (leader) CTA.
+template <int CG>
 __device__ __forceinline__ void tma_load_2d(uint32_t dst_smem, const CUtensorMap* map, int c0, int c1, uint32_t bar,
                                             uint64_t policy) {
-    asm volatile(
-        "cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes.L2::cache_hint"
-        " [%0], [%1, {%3, %4}], [%2], %5;"
-        ::"r"(dst_smem), "l"(map), "r"(bar), "r"(c0), "r"(c1), "l"(policy)
-        : "memory");
+    if constexpr (CG == 1) {
+        asm volatile(
+            "cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes.L2::cache_hint"
+            " [%0], [%1, {%3, %4}], [%2], %5;"
+            ::"r"(dst_smem), "l"(map), "r"(bar), "r"(c0), "r"(c1), "l"(policy)
+            : "memory");
+    } else {
+        asm volatile(
+            "cp.async.bulk.tensor.2d.cta_group::2.shared::cluster.global.tile.mbarrier::complete_tx::bytes.L2::cache_hint"
+            " [%0], [%1, {%3, %4}], [%2], %5;"
+            ::"r"(dst_smem), "l"(map), "r"(bar), "r"(c0), "r"(c1), "l"(policy)
+            : "memory");
+    }
 }
 
 // K-major, 128-byte swizzle: rows of 128 B, 8-row groups 1024 B apart (SBO), LBO unused (=1),
@@ -91,16 +126,37 @@ __device__ __forceinline__ uint64_t umma_desc_sw128(uint32_t smem_addr) {
 __host__ __device__ constexpr uint32_t umma_idesc_bf16(int m, int n) {
     return (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(n >> 3) << 17) | ((uint32_t)(m >> 4) << 24);
 }
+// D[tmem] (+)= X[smem] * Y[smem]^T.  CG == 2: one instruction drives the tensor cores of both SMs of the
+// pair (M = 256: rows 0-127 from the leader's X stage, 128-255 from the peer's; Y split N/2 + N/2).
+template <int CG>
 __device__ __forceinline__ void umma_bf16(uint32_t tmem_d, uint64_t adesc, uint64_t bdesc, uint32_t idesc,
                                           uint32_t accumulate) {
-    asm volatile(
-        "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
-        "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}"
-        ::"r"(tmem_d), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate)
-        : "memory");
+    if constexpr (CG == 1) {
+        asm volatile(
+            "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+            "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}"
+            ::"r"(tmem_d), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate)
+            : "memory");
+    } else {
+        asm volatile(
+            "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+            "tcgen05.mma.cta_group::2.kind::f16 [%0], %1, %2, %3, p;\n\t}"
+            ::"r"(tmem_d), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate)
+            : "memory");
+    }
 }
+// mbarrier arrive when all MMAs issued so far have retired.  CG == 2: multicast to the same barrier
+// offset in both CTAs of the pair.
+template <int CG>
 __device__ __forceinline__ void umma_commit(uint32_t bar) {
-    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
+    if constexpr (CG == 1) {
+        asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
+    } else {
+        asm volatile(
+            "tcgen05.commit.cta_group::2.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;"
+            ::"r"(bar), "h"((uint16_t)3)
+            : "memory");
+    }
 }
 __device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&v)[32]) {
     asm volatile(
@@ -127,13 +183,14 @@ struct Seg {
 };
 struct Sched {
     const GemmParams& p;
-    long long u0, u1, cur;  // stream-K unit range of this CTA
+    long long u0, u1, cur;  // stream-K unit range of this worker
     int it;
-    __device__ Sched(const GemmParams& p_) : p(p_), it(0) {
+    int wid, nw;            // worker (CTA, or CTA pair) index and count
+    __device__ Sched(const GemmParams& p_, int wid_, int nw_) : p(p_), it(0), wid(wid_), nw(nw_) {
         if (p.stream_k) {
             const long long U = (long long)p.n_tiles * p.kb_per_tile;
-            u0 = (long long)blockIdx.x * U / gridDim.x;
-            u1 = (long long)(blockIdx.x + 1) * U / gridDim.x;
+            u0 = (long long)wid * U / nw;
+            u1 = (long long)(wid + 1) * U / nw;
             cur = u0;
         } else {
             u0 = u1 = cur = 0;
@@ -151,7 +208,7 @@ struct Sched {
             cur += s.kb1 - s.kb0;
             return true;
         }
-        const long long t = (long long)blockIdx.x + (long long)it * gridDim.x;
+        const long long t = (long long)wid + (long long)it * nw;
         if (t >= p.n_tiles) return false;
         ++it;
         s.tile = (int)t;
@@ -227,18 +284,25 @@ __device__ __forceinline__ void store_out(const GemmParams& p, const float (&acc
     }
 }
 
-template <int BN>
+template <int BN, int CG>
 __global__ void __launch_bounds__(kGemmThreads, 1)
 gemm_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constant__ CUtensorMap mapY, const GemmParams p,
             Trace tr) {
-    constexpr int kStageBytes = stage_bytes(BN);
+    // CG == 2: the CTA pair of a 2-cluster works on one 256 x BN tile.  Each CTA stages its own 128 rows of X
+    // and its own BN/2 rows of Y; the leader (cluster rank 0) issues tcgen05.mma.cta_group::2, which reads both
+    // CTAs' stages and writes rows [128*rank, 128*rank+128) of the accumulator into each CTA's TMEM.
+    constexpr int kYRows = BN / CG;
     constexpr int kXBytes = kBM * kBK * 2;
+    constexpr int kStageBytes = kXBytes + kYRows * kBK * 2;
     constexpr int kTmemCols = 2 * BN;   // two accumulators (power of two for BN in {64,128,256})
-    constexpr uint32_t kIdesc = umma_idesc_bf16(kBM, BN);
+    constexpr uint32_t kIdesc = umma_idesc_bf16(kBM * CG, BN);
     static_assert(BN == 64 || BN == 128 || BN == 256, "BN");
+    static_assert(CG == 1 || CG == 2, "CG");
+    static_assert(kStageBytes == stage_bytes(BN, CG), "stage size");
 
     extern __shared__ uint8_t smem_raw[];
-    // 1024-byte alignment for the 128B swizzle; the barrier block sits after the stages
+    // 1024-byte alignment for the 128B swizzle; the barrier block sits after the stages.  Both CTAs of a pair
+    // compute identical offsets (same kernel, same dynamic-smem base), which cta_group::2 relies on.
     const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
     const uint32_t bar_base = smem_base + p.stages * kStageBytes;
     auto full_bar = [&](int s) { return bar_base + 8u * s; };
@@ -251,57 +315,74 @@ gemm_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constant__ CU
 
     const int warp = threadIdx.x >> 5;
     const int lane = threadIdx.x & 31;
+    const uint32_t rank = (CG == 2) ? cluster_ctarank() : 0u;          // 0 = leader
+    const int wid = (int)(blockIdx.x / CG), nw = (int)(gridDim.x / CG);
     uint64_t* rec = (threadIdx.x == 0) ? trace_begin(tr, KID_GEMM) : nullptr;
 
     if (warp == 0 && lane == 0) {
         asm volatile("prefetch.tensormap [%0];" ::"l"(&mapX) : "memory");
         asm volatile("prefetch.tensormap [%0];" ::"l"(&mapY) : "memory");
         for (int s = 0; s < p.stages; ++s) {
-            mbar_init(full_bar(s), 1);
-            mbar_init(empty_bar(s), 1);
+            mbar_init(full_bar(s), CG);           // one arrive.expect_tx per producer of the pair
+            mbar_init(empty_bar(s), 1);           // one tcgen05.commit (multicast to both CTAs when CG == 2)
         }
         for (int b = 0; b < 2; ++b) {
             mbar_init(tfull_bar(b), 1);
-            mbar_init(tempty_bar(b), kEpiThreads);
+            mbar_init(tempty_bar(b), 4 * CG);     // one arrive per epilogue warp of the pair
         }
         mbar_fence_init();
     }
     if (warp == 1) {
-        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(tmem_slot),
-                     "r"((uint32_t)kTmemCols)
-                     : "memory");
-        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+        if constexpr (CG == 1) {
+            asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(tmem_slot),
+                         "r"((uint32_t)kTmemCols) : "memory");
+            asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+        } else {
+            asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(tmem_slot),
+                         "r"((uint32_t)kTmemCols) : "memory");
+            asm volatile("tcgen05.relinquish_alloc_permit.cta_group::2.sync.aligned;" ::: "memory");
+        }
     }
     tc_fence_before();
-    __syncthreads();
+    if constexpr (CG == 2) cluster_sync_all();    // the peer's barriers exist before anything remote touches them
+    else __syncthreads();
     tc_fence_after();
     const uint32_t tmem_base = *reinterpret_cast<volatile uint32_t*>(smem_gen + (tmem_slot - smem_base));
 
     if (warp == 0) {
-        // ================= TMA producer =================
+        // ================= TMA producer (one per CTA) =================
         if (lane == 0) {
             const uint64_t polX = make_policy(p.hintX), polY = make_policy(p.hintY);
-            Sched sched(p);
+            Sched sched(p, wid, nw);
             Seg sg;
             int stage = 0;
             uint32_t phase = 0;
             while (sched.next(sg)) {
                 int tx, ty;
                 tile_xy(p, sg.tile, tx, ty);
+                const int x0 = tx * (kBM * CG) + (int)rank * kBM;
+                const int y0 = ty * BN + (int)rank * kYRows;
                 for (int kb = sg.kb0; kb < sg.kb1; ++kb) {
-                    mbar_wait(empty_bar(stage), phase ^ 1u);
-                    mbar_expect_tx(full_bar(stage), kStageBytes);
+                    mbar_wait(empty_bar(stage), phase ^ 1u);           // local: MMAs reading this stage retired
                     const uint32_t sx = smem_base + stage * kStageBytes;
-                    tma_load_2d(sx, &mapX, kb * kBK, tx * kBM, full_bar(stage), polX);
-                    tma_load_2d(sx + kXBytes, &mapY, kb * kBK, ty * BN, full_bar(stage), polY);
+                    if constexpr (CG == 1) {
+                        mbar_expect_tx(full_bar(stage), kStageBytes);
+                        tma_load_2d<1>(sx, &mapX, kb * kBK, x0, full_bar(stage), polX);
+                        tma_load_2d<1>(sx + kXBytes, &mapY, kb * kBK, y0, full_bar(stage), polY);
+                    } else {
+                        const uint32_t lead_full = mapa(full_bar(stage), 0);   // the leader's barrier collects both halves
+                        mbar_expect_tx_cluster(lead_full, kStageBytes);
+                        tma_load_2d<2>(sx, &mapX, kb * kBK, x0, lead_full, polX);
+                        tma_load_2d<2>(sx + kXBytes, &mapY, kb * kBK, y0, lead_full, polY);
+                    }
                     if (++stage == p.stages) { stage = 0; phase ^= 1u; }
                 }
             }
         }
     } else if (warp == 1) {
-        // ================= MMA issuer =================
-        if (lane == 0) {
-            Sched sched(p);
+        // ================= MMA issuer (leader CTA only) =================
+        if (lane == 0 && rank == 0) {
+            Sched sched(p, wid, nw);
             Seg sg;
             int stage = 0;
             uint32_t phase = 0;
@@ -309,11 +390,11 @@ gemm_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constant__ CU
             while (sched.next(sg)) {
                 const int buf = acc_it & 1;
                 const uint32_t aphase = (acc_it >> 1) & 1;
-                mbar_wait(tempty_bar(buf), aphase ^ 1u);   // epilogue has drained this accumulator
+                mbar_wait(tempty_bar(buf), aphase ^ 1u);   // every epilogue warp (of the pair) drained this accumulator
                 tc_fence_after();
                 const uint32_t tmem_d = tmem_base + (uint32_t)(buf * BN);
                 for (int kb = sg.kb0; kb < sg.kb1; ++kb) {
-                    mbar_wait(full_bar(stage), phase);     // TMA bytes have landed
+                    mbar_wait(full_bar(stage), phase);     // TMA bytes (of both CTAs) have landed
                     tc_fence_after();
                     const uint32_t sx = smem_base + stage * kStageBytes;
                     const uint64_t dx = umma_desc_sw128(sx);
@@ -321,22 +402,22 @@ gemm_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constant__ CU
 #pragma unroll
                     for (int k = 0; k < kBK / kUmmaK; ++k) {
                         // +32 B per UMMA_K step inside the swizzle atom = +2 in the (addr >> 4) field
-                        umma_bf16(tmem_d, dx + (uint64_t)(2 * k), dy + (uint64_t)(2 * k), kIdesc,
-                                  (kb > sg.kb0 || k > 0) ? 1u : 0u);
+                        umma_bf16<CG>(tmem_d, dx + (uint64_t)(2 * k), dy + (uint64_t)(2 * k), kIdesc,
+                                      (kb > sg.kb0 || k > 0) ? 1u : 0u);
                     }
-                    umma_commit(empty_bar(stage));         // frees the smem stage when these MMAs retire
+                    umma_commit<CG>(empty_bar(stage));     // frees the smem stage (in both CTAs) when these MMAs retire
                     if (++stage == p.stages) { stage = 0; phase ^= 1u; }
                 }
-                umma_commit(tfull_bar(buf));               // accumulator complete
+                umma_commit<CG>(tfull_bar(buf));           // accumulator complete (signals both CTAs' epilogues)
                 ++acc_it;
             }
         }
     } else {
-        // ================= epilogue (warps 2..5) =================
+        // ================= epilogue (warps 2..5 of every CTA) =================
         const int quarter = warp & 3;                       // TMEM lane quarter this warp may read
-        const int xl = quarter * 32 + lane;                 // row inside the tile
+        const int xl = quarter * 32 + lane;                 // row inside this CTA's 128-row slab
         const int et = threadIdx.x - 64;                    // 0..127
-        Sched sched(p);
+        Sched sched(p, wid, nw);
         Seg sg;
         int acc_it = 0;
         while (sched.next(sg)) {
@@ -345,10 +426,10 @@ gemm_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constant__ CU
             int tx, ty;
             tile_xy(p, sg.tile, tx, ty);
             const bool whole = (sg.kb0 == 0 && sg.kb1 == p.kb_per_tile);
-            const int x = tx * kBM + xl;
+            const int x = tx * (kBM * CG) + (int)rank * kBM + xl;
             float* part = nullptr;
             if (!whole) {
-                const int slot = 2 * (int)blockIdx.x + (sg.start_unit == sched.u0 ? 0 : 1);
+                const int slot = 2 * wid + (sg.start_unit == sched.u0 ? 0 : 1);
                 part = p.partials + (size_t)slot * (kBM * BN);
             }
             mbar_wait(tfull_bar(buf), aphase);
@@ -369,14 +450,19 @@ gemm_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constant__ CU
                     for (int j = 0; j < 32; ++j) __stcg(part + (size_t)(c * 32 + j) * kBM + xl, acc[j]);
                 }
             }
+            // this warp's quarter of the accumulator is drained: tell the (leader's) MMA issuer
             tc_fence_before();
-            mbar_arrive(tempty_bar(buf));
+            __syncwarp();
+            if (lane == 0) {
+                if constexpr (CG == 1) mbar_arrive(tempty_bar(buf));
+                else mbar_arrive_cluster(mapa(tempty_bar(buf), 0));
+            }
             ++acc_it;
 
             if (!whole) {
-                // ---- stream-K fix-up: last part to arrive reduces all parts in ascending-k order ----
+                // ---- stream-K fix-up (CG == 1 only): last part to arrive reduces all parts in ascending-k order ----
                 const long long U = (long long)p.n_tiles * p.kb_per_tile;
-                const long long G = gridDim.x;
+                const long long G = nw;
                 const long long ua = (long long)sg.tile * p.kb_per_tile;          // first unit of the tile
                 const long long ub = ua + p.kb_per_tile - 1;                      // last unit of the tile
                 const int c_first = (int)(((ua + 1) * G - 1) / U);
@@ -418,12 +504,16 @@ gemm_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constant__ CU
         }
     }
 
+    // teardown: nobody may exit (or free TMEM) while the peer can still signal its barriers / read its stages
     tc_fence_before();
-    __syncthreads();
+    if constexpr (CG == 2) cluster_sync_all();
+    else __syncthreads();
     if (warp == 1) {
         tc_fence_after();
-        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"((uint32_t)kTmemCols)
-                     : "memory");
+        if constexpr (CG == 1)
+            asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"((uint32_t)kTmemCols) : "memory");
+        else
+            asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"((uint32_t)kTmemCols) : "memory");
     }
     if (threadIdx.x == 0) trace_end(rec);
 }
@@ -483,8 +573,6 @@ struct Plan {
     size_t counters_bytes, ws_bytes;
 };
 
-static int dyn_smem_for(int bn, int stages) { return stages * stage_bytes(bn) + kAlignSlack + kBarrierBytes; }
-
 static ra_status validate_shape(int transA, int transB, int M, int N, int K) {
     if ((transA != 0 && transA != 1) || (transB != 0 && transB != 1)) return RA_ERR_INVALID_ARG;
     if (M < 0 || N < 0 || K < 0) return RA_ERR_INVALID_ARG;
@@ -494,7 +582,7 @@ static ra_status validate_shape(int transA, int transB, int M, int N, int K) {
 static ra_status make_plan(int transA, int transB, int M, int N, int K, const ra_occupancy* occ_in, Plan* out) {
     RA_TRY(validate_shape(transA, transB, M, N, K));
     if (transA != 0 || transB != 1) return RA_ERR_UNSUPPORTED;   // K-contiguous operands only (A13)
-    ra_occupancy occ = {0, 0, 0, 1};
+    ra_occupancy occ = {0, 0, 0, 1, 0};
     if (occ_in) occ = *occ_in;
     if (occ.smem_reserve_bytes < 0 || occ.sm_budget < 0 || occ.tiles_per_cta < 0) return RA_ERR_INVALID_ARG;
 
@@ -527,15 +615,39 @@ static ra_status make_plan(int transA, int transB, int M, int N, int K, const ra
     const int swap = (M <= 64 && N >= 128) ? 1 : 0;
     const int RX = swap ? N : M, RY = swap ? M : N;
     int bn = RY > 128 ? 256 : (RY > 64 ? 128 : 64);
+    const int kb = (K + kBK - 1) / kBK;
+    if (occ.cta_group < 0 || occ.cta_group > 2) return RA_ERR_INVALID_ARG;
 
     // shared memory the GEMM may allocate on an SM
     long avail = (long)smem_per_sm - occ.smem_reserve_bytes - reserved;
     if (avail > optin) avail = optin;
+    const long room = avail - kAlignSlack - kBarrierBytes;
+    auto stages_for = [&](int bn_, int cg_) {
+        int s = room > 0 ? (int)(room / stage_bytes(bn_, cg_)) : 0;
+        return s > kMaxStages ? kMaxStages : s;
+    };
+    auto wave_eff = [](long long tiles, int workers) {
+        const long long waves = (tiles + workers - 1) / workers;
+        return waves > 0 ? (double)tiles / (double)(waves * workers) : 1.0;
+    };
+
+    // CTA pairs (cta_group::2, 256 x 256 tiles): each SM stages 128 rows of X and 128 of Y per k-block instead of
+    // 128 + 256, i.e. 1/3 less L2->SM traffic per flop.  Used for the data-parallel schedule on large problems.
+    int cg = 1;
+    if (occ.cta_group != 1 && !swap && bn == 256 && RX >= 256 && budget >= 2 && stages_for(256, 2) >= 2) {
+        const long long t2 = (long long)((RX + 2 * kBM - 1) / (2 * kBM)) * ((RY + bn - 1) / bn);
+        // measured on B200: pairs at 86 % wave efficiency (4096^3) still beat single-CTA stream-K by 28 %
+        const bool sk_wanted = occ.tiles_per_cta == 0 && kb >= 8 && wave_eff(t2, budget / 2) < 0.7;
+        if (!sk_wanted || occ.cta_group == 2) cg = 2;
+    }
+    if (occ.cta_group == 2 && cg != 2) {
+        if (!occ.allow_clamp) return RA_ERR_INFEASIBLE_KNOB;
+        clamped = 1;
+    }
+
     int stages = 0;
     for (;;) {
-        const long room = avail - kAlignSlack - kBarrierBytes;
-        stages = room > 0 ? (int)(room / stage_bytes(bn)) : 0;
-        if (stages > kMaxStages) stages = kMaxStages;
+        stages = stages_for(bn, cg);
         if (stages >= 2 || bn == 64) break;
         bn >>= 1;   // squeeze the tile before giving up pipelining
     }
@@ -544,18 +656,18 @@ static ra_status make_plan(int transA, int transB, int M, int N, int K, const ra
         stages = 1;
         clamped = 1;
     }
-    int dyn = dyn_smem_for(bn, stages);
+    int dyn = stages * stage_bytes(bn, cg) + kAlignSlack + kBarrierBytes;
 
-    const int tiles_x = (RX + kBM - 1) / kBM, tiles_y = (RY + bn - 1) / bn;
+    const int tile_x = kBM * cg;
+    const int tiles_x = (RX + tile_x - 1) / tile_x, tiles_y = (RY + bn - 1) / bn;
     const long long n_tiles = (long long)tiles_x * tiles_y;
-    if (n_tiles > 0x7fffffffLL) return RA_ERR_UNSUPPORTED;
-    const int kb = (K + kBK - 1) / kBK;
+    if (n_tiles > 0x3fffffffLL) return RA_ERR_UNSUPPORTED;
 
     int grid, stream_k = 0, ctas_per_sm = 1;
     if (occ.tiles_per_cta > 0) {
         // bounded work: more CTAs than SMs.  Residency must stay at one GEMM CTA per SM (TMEM holds
         // two accumulators), so pad the request past half of what an SM can give.
-        grid = (int)((n_tiles + occ.tiles_per_cta - 1) / occ.tiles_per_cta);
+        grid = cg * (int)((n_tiles + occ.tiles_per_cta - 1) / occ.tiles_per_cta);
         const int half = (smem_per_sm - 2 * reserved) / 2 + 16;
         if (dyn < half) {
             if (half > avail) {
@@ -565,23 +677,26 @@ static ra_status make_plan(int transA, int transB, int M, int N, int K, const ra
             dyn = half;
         }
     } else {
-        grid = (int)(n_tiles < budget ? n_tiles : budget);
-        if (grid < 1) grid = 1;
-        // wave-quantisation efficiency of the data-parallel schedule on `budget` CTAs; below 90 %
-        // (MB: 128 tiles on 148 SMs) the k-block units are cut evenly instead (stream-K).
+        const int workers = budget / cg;                 // CTAs, or CTA pairs
+        int w = (int)(n_tiles < workers ? n_tiles : workers);
+        if (w < 1) w = 1;
+        // wave-quantisation efficiency of the data-parallel schedule.  Several waves with a ragged last one
+        // (< 90 %): cut the k-block units evenly instead (stream-K, single-CTA tiles only).  A single partial
+        // wave (MB: 128 tiles on 148 SMs = 86 %) stays data-parallel down to 80 %: one tile per CTA and no
+        // partials measured 4 % faster than stream-K on all 148 SMs, since 128 SMs already saturate HBM.
         const long long U = n_tiles * kb;
-        const long long waves = (n_tiles + budget - 1) / budget;
-        const double eff = waves > 0 ? (double)n_tiles / (double)(waves * budget) : 1.0;
-        if (n_tiles > 0 && kb >= 8 && eff < 0.9) {
+        const double eff = wave_eff(n_tiles, workers);
+        if (cg == 1 && n_tiles > 0 && kb >= 8 && eff < (n_tiles <= workers ? 0.8 : 0.9)) {
             stream_k = 1;
-            grid = budget;
-            if ((long long)grid * 4 > U) grid = (int)(U / 4);   // at least 4 k-blocks per CTA
+            w = workers;
+            if ((long long)w * 4 > U) w = (int)(U / 4);   // at least 4 k-blocks per CTA
         }
+        grid = w * cg;
     }
     g.ctas_per_sm = ctas_per_sm;
     g.grid = grid;
     g.stages = stages;
-    g.tile_m = swap ? bn : kBM;
+    g.tile_m = swap ? bn : tile_x;
     g.tile_n = swap ? kBM : bn;
     g.tile_k = kBK;
     g.swap_ab = swap;
@@ -590,6 +705,7 @@ static ra_status make_plan(int transA, int transB, int M, int N, int K, const ra
     g.n_tiles = (int)n_tiles;
     g.clamped = clamped;
     g.split_k = 1;
+    g.cta_group = cg;
     pl.bn = bn;
     if (stream_k) {
         const long long U = n_tiles * kb;
@@ -603,12 +719,28 @@ static ra_status make_plan(int transA, int transB, int M, int N, int K, const ra
     return RA_OK;
 }
 
-template <int BN>
+template <int BN, int CG>
 static ra_status launch_gemm(const CUtensorMap& mx, const CUtensorMap& my, const GemmParams& p, int grid, int dyn,
                              cudaStream_t stream) {
-    RA_CUDA(cudaFuncSetAttribute(gemm_kernel<BN>, cudaFuncAttributeMaxDynamicSharedMemorySize, dyn));
-    gemm_kernel<BN><<<grid, kGemmThreads, dyn, stream>>>(mx, my, p, g_trace);
-    RA_CUDA(cudaGetLastError());
+    RA_CUDA(cudaFuncSetAttribute(gemm_kernel<BN, CG>, cudaFuncAttributeMaxDynamicSharedMemorySize, dyn));
+    if constexpr (CG == 1) {
+        gemm_kernel<BN, 1><<<grid, kGemmThreads, dyn, stream>>>(mx, my, p, g_trace);
+        RA_CUDA(cudaGetLastError());
+        return RA_OK;
+    }
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3((unsigned)grid);
+    cfg.blockDim = dim3(kGemmThreads);
+    cfg.dynamicSmemBytes = (size_t)dyn;
+    cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = CG;
+    attr[0].val.clusterDim.y = 1;
+    attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    RA_CUDA(cudaLaunchKernelEx(&cfg, gemm_kernel<BN, CG>, mx, my, p, g_trace));
     return RA_OK;
 }
 
@@ -657,7 +789,8 @@ ra_status gemm_launch(int transA, int transB, int M, int N, int K, float alpha, 
     p.RX = swap ? N : M;
     p.RY = swap ? M : N;
     p.K = K;
-    p.tiles_x = (p.RX + kBM - 1) / kBM;
+    const int cg = pl.pub.cta_group;
+    p.tiles_x = (p.RX + kBM * cg - 1) / (kBM * cg);
     p.tiles_y = (p.RY + pl.bn - 1) / pl.bn;
     p.n_tiles = pl.pub.n_tiles;
     p.kb_per_tile = (K + kBK - 1) / kBK;
@@ -682,11 +815,12 @@ ra_status gemm_launch(int transA, int transB, int M, int N, int K, float alpha, 
     const int ldx = swap ? ldb : lda, ldy = swap ? lda : ldb;
     CUtensorMap mx, my;
     RA_TRY(make_map(&mx, X, p.RX, K, ldx, kBM));
-    RA_TRY(make_map(&my, Y, p.RY, K, ldy, pl.bn));
+    RA_TRY(make_map(&my, Y, p.RY, K, ldy, pl.bn / cg));
+    if (cg == 2) return launch_gemm<256, 2>(mx, my, p, pl.pub.grid, pl.pub.dyn_smem_bytes, stream);
     switch (pl.bn) {
-        case 64: return launch_gemm<64>(mx, my, p, pl.pub.grid, pl.pub.dyn_smem_bytes, stream);
-        case 128: return launch_gemm<128>(mx, my, p, pl.pub.grid, pl.pub.dyn_smem_bytes, stream);
-        case 256: return launch_gemm<256>(mx, my, p, pl.pub.grid, pl.pub.dyn_smem_bytes, stream);
+        case 64: return launch_gemm<64, 1>(mx, my, p, pl.pub.grid, pl.pub.dyn_smem_bytes, stream);
+        case 128: return launch_gemm<128, 1>(mx, my, p, pl.pub.grid, pl.pub.dyn_smem_bytes, stream);
+        case 256: return launch_gemm<256, 1>(mx, my, p, pl.pub.grid, pl.pub.dyn_smem_bytes, stream);
     }
     return RA_ERR_UNSUPPORTED;
 }

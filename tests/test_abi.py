@@ -38,11 +38,11 @@ def test_status_strings(ra):
 
 def test_struct_layouts_match_header(ra):
     # sizes computed by hand from include/ra.h (LP64)
-    assert ctypes.sizeof(ra.Occupancy) == 16
-    assert ctypes.sizeof(ra.GemmPlan) == 48
+    assert ctypes.sizeof(ra.Occupancy) == 20
+    assert ctypes.sizeof(ra.GemmPlan) == 52
     assert ctypes.sizeof(ra.Workload) == 152
-    assert ctypes.sizeof(ra.OverlapCfg) == 4 + 16 + 8 * 4
-    assert ctypes.sizeof(ra.OverlapResult) == 24 + 48 + 8
+    assert ctypes.sizeof(ra.OverlapCfg) == 4 + 20 + 8 * 4
+    assert ctypes.sizeof(ra.OverlapResult) == 24 + 52 + 4 + 8
 
 
 KB = 1024
@@ -66,11 +66,14 @@ def test_plan_honours_reserve_and_budget(ra, shape, reserve, budget):
 
 def test_plan_depth_shrinks_with_reserve(ra):
     stages = [ra.ra_gemm_plan_query(0, 1, 8192, 8192, 8192, dict(smem_reserve_bytes=r * KB))["stages"] for r in (0, 64, 112)]
-    assert stages == sorted(stages, reverse=True) and stages[0] == 4
+    assert stages == sorted(stages, reverse=True) and stages[0] == 7
     mb = [ra.ra_gemm_plan_query(0, 1, 64, 16384, 16384, dict(smem_reserve_bytes=r * KB)) for r in (0, 64, 128, 200)]
     assert [p["stages"] for p in mb] == sorted((p["stages"] for p in mb), reverse=True)
     assert all(p["swap_ab"] == 1 and p["tile_m"] == 64 for p in mb)
-    assert mb[0]["split_k"] > 1                                     # 128 tiles on 148 SMs -> stream-K
+    assert mb[0]["split_k"] == 1 and mb[0]["grid"] == 128           # one tile per CTA on 128 of the 148 SMs
+    for b in (74, 92, 110):                                         # ragged multi-wave -> stream-K on exactly b CTAs
+        p = ra.ra_gemm_plan_query(0, 1, 64, 16384, 16384, dict(sm_budget=b))
+        assert p["split_k"] > 1 and p["grid"] == b
 
 
 def test_plan_infeasible_knob(ra):

@@ -109,6 +109,33 @@ def test_integer_exact(ra, M, N, K):
     assert np.array_equal(got, ref16)
 
 
+@pytest.mark.parametrize("M,N,K", [(256, 256, 64), (512, 512, 256), (1000, 520, 200), (384, 768, 4096), (2048, 2048, 512),
+                                   (257, 264, 72), (4096, 1024, 1024)])
+@pytest.mark.parametrize("occ", [dict(cta_group=2), dict(cta_group=2, sm_budget=9, smem_reserve_bytes=128 * 1024),
+                                 dict(cta_group=2, tiles_per_cta=1)])
+def test_cta_pairs(ra, M, N, K, occ):
+    """tcgen05 cta_group::2 path (2-CTA clusters, 256 x 256 tiles), forced on shapes the planner would not pick it for."""
+    plan = ra.ra_gemm_plan_query(0, 1, M, N, K, occ)
+    assert plan["cta_group"] == 2 and plan["tile_m"] == 256 and plan["grid"] % 2 == 0, plan
+    check(ra, M, N, K, seed=4000 + M + N + K, occ=occ)
+
+
+def test_cta_pairs_integer_exact_and_bit_identical_to_single(ra):
+    M, N, K = 1024, 768, 2048
+    A = ra_inputs.smallint_bf16((M, K), 41, ra_inputs.STREAM_A)
+    B = ra_inputs.smallint_bf16((N, K), 41, ra_inputs.STREAM_B)
+    _, ref16 = oracle.gemm(0, 1, M, N, K, 1.0, A, B)
+    got2, _ = run_gemm(ra, M, N, K, A, B, occ=dict(cta_group=2))
+    assert np.array_equal(got2, ref16)
+    # same per-element K order (k-blocks ascending, one accumulator) => pairs and single CTAs agree bit for bit
+    An = ra_inputs.normal_bf16((M, K), 42, ra_inputs.STREAM_A)
+    Bn = ra_inputs.normal_bf16((N, K), 42, ra_inputs.STREAM_B)
+    c2, _ = run_gemm(ra, M, N, K, An, Bn, occ=dict(cta_group=2, sm_budget=148))
+    c1, _ = run_gemm(ra, M, N, K, An, Bn, occ=dict(cta_group=1, sm_budget=24))
+    assert ra.ra_gemm_plan_query(0, 1, M, N, K, dict(cta_group=1, sm_budget=24))["split_k"] == 1
+    assert np.array_equal(c1, c2)
+
+
 def test_ones_closed_form(ra):
     for K in (256, 8192):
         one = ra_inputs.f32_to_bf16_bits_exact(np.ones((136, K), np.float32))
