@@ -70,7 +70,7 @@ class ClockSampler:
         try:
             self.tmp = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
             self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
-                                          "-lms", "100", "-i", str(self.gpu)], stdout=self.tmp, stderr=subprocess.DEVNULL)
+                                          "-lms", "20", "-i", str(self.gpu)], stdout=self.tmp, stderr=subprocess.DEVNULL)
         except Exception:
             self.proc = None
 
@@ -174,9 +174,18 @@ def sweep_candidates(ra, cfg, quick: bool):
     for r in reserves:
         for b in budgets:
             for prio in (0, hi):
-                for csb in ({0, info["sm_count"] - b} if b < info["sm_count"] else {0}):
-                    cands.append(dict(mode=1, occ=dict(smem_reserve_bytes=r, sm_budget=b), prio_compute=0, prio_comm=prio,
-                                      coll_sm_budget=csb, coll_smem_bytes=min(max(r, 32 * KB), 64 * KB) if r else 0))
+                for csb in sorted({0, info["sm_count"] - b} if b < info["sm_count"] else {0}):
+                    base = dict(mode=1, occ=dict(smem_reserve_bytes=r, sm_budget=b), prio_compute=0, prio_comm=prio, coll_sm_budget=csb)
+                    if cfg.coll == "alltoall":
+                        # TMA ring sized to fit INSIDE the reserve (ring + 1 KiB system + barriers), and the
+                        # shared-memory-free LDG/STG variant, which can co-reside on a full GEMM SM
+                        if r >= 20 * KB:
+                            cands.append(dict(base, coll_variant=0, coll_smem_bytes=min(r - 4 * KB, 64 * KB), coll_ctas_per_sm=1))
+                        elif b < info["sm_count"]:
+                            cands.append(dict(base, coll_variant=0))
+                        cands.append(dict(base, coll_variant=1))
+                    else:
+                        cands.append(base)
     return cands
 
 
@@ -184,7 +193,47 @@ def cfg_label(kw):
     o = kw.get("occ", {})
     return {"smem_reserve_bytes": o.get("smem_reserve_bytes", 0), "sm_budget": o.get("sm_budget", 0),
             "tiles_per_cta": o.get("tiles_per_cta", 0), "priority": "on" if kw.get("prio_comm", 0) != kw.get("prio_compute", 0) else "off",
-            "coll_sm_budget": kw.get("coll_sm_budget", 0), "coll_smem_bytes": kw.get("coll_smem_bytes", 0)}
+            "coll_sm_budget": kw.get("coll_sm_budget", 0), "coll_smem_bytes": kw.get("coll_smem_bytes", 0),
+            "coll_variant": kw.get("coll_variant", 0), "coll_ctas_per_sm": kw.get("coll_ctas_per_sm", 0)}
+
+
+def residency_map(ra, w, cfg_kw, n_sms):
+    """Per-SM residency during one overlapped step, from the library's %smid/%globaltimer trace
+    (ra_set_trace): every CTA of every kernel logs {kernel id, SM, start, end}.  Evidence for co-residency:
+    how much of the collective's CTA-time ran on an SM that hosted a GEMM CTA at the same instant."""
+    import torch
+    cap = 1 << 16
+    buf = torch.zeros(1 + 4 * cap, dtype=torch.int64, device="cuda")
+    ra.ra_set_trace(buf, cap)
+    try:
+        ra.ra_overlap_run(w, ra.make_cfg(**cfg_kw))
+        torch.cuda.synchronize()
+    finally:
+        ra.ra_set_trace(None, 0)
+    hbuf = buf.cpu().numpy().view(np.uint64)
+    n = int(min(int(hbuf[0]), cap))
+    rec = hbuf[1:1 + 4 * n].reshape(n, 4)
+    kid = (rec[:, 0] >> np.uint64(32)).astype(np.int64)
+    sm = (rec[:, 0] & np.uint64(0xFFFFFFFF)).astype(np.int64)
+    t0, t1 = rec[:, 2].astype(np.int64), rec[:, 3].astype(np.int64)
+    g, c = kid == 1, kid != 1
+    out = {"records": n, "gemm_ctas": int(g.sum()), "coll_ctas": int(c.sum()),
+           "gemm_sms_used": int(len(set(sm[g]))), "coll_sms_used": int(len(set(sm[c])))}
+    co, tot = 0, 0
+    per_sm_g = {}
+    for s_, a, b in zip(sm[g], t0[g], t1[g]):
+        per_sm_g.setdefault(int(s_), []).append((int(a), int(b)))
+    for s_, a, b in zip(sm[c], t0[c], t1[c]):
+        tot += int(b - a)
+        for (ga, gb) in per_sm_g.get(int(s_), ()):
+            lo, hi = max(a, ga), min(b, gb)
+            if hi > lo:
+                co += int(hi - lo)
+    out["coll_cta_time_coresident_with_gemm_frac"] = (co / tot) if tot else None
+    span = (t1.max() - t0.min()) if n else 0
+    out["gemm_sm_busy_frac"] = float((t1[g] - t0[g]).sum() / (span * n_sms)) if span else None
+    out["coll_mean_cta_us"] = float((t1[c] - t0[c]).mean() / 1e3) if c.any() else None
+    return out
 
 
 def kernels_alone(ra, cfg, d, h, peaks, n_iters):
@@ -354,6 +403,8 @@ def run_ours(args, cfg):
             norm_time = on / off
 
     alone = kernels_alone(ra, cfg, d, h, peaks, n_iters)
+    residency = residency_map(ra, w, best_kw, ra.ra_device_info()["sm_count"])
+    reset_collective(cfg, d, h)
 
     # ---- timed region: exactly K steps of the overlapped hot path at the picked setting ----
     best_cfg = ra.make_cfg(**dict(best_kw, record_kernel_times=1))
@@ -455,7 +506,7 @@ def run_ours(args, cfg):
         "overlap_vs_roofline": {"burst": over_ms / comb["bf16_tflops"], "sustained": over_ms / comb["bf16_tflops_sustained"]},
         "peaks": peaks, "roofline": roof, "cpu_baseline": cpu,
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
-        "gpu_launches": args.steps * n_iters * 2, "clocks": clocks, "wall_ms_timed_region": wall_ms, "paper_context": PAPER_CONTEXT,
+        "residency": residency, "gpu_launches": args.steps * n_iters * 2, "clocks": clocks, "wall_ms_timed_region": wall_ms, "paper_context": PAPER_CONTEXT,
     }
     if args.table:
         with open(args.table, "w") as f:

@@ -136,6 +136,8 @@ ra_status ra_gemm(int transA, int transB, int M, int N, int K, float alpha, cons
  * sm_budget: SMs' worth of CTAs to launch (0 = all SMs).
  * ------------------------------------------------------------------------------------------- */
 ra_status ra_allreduce_emul(float* const* bufs, int P, size_t count, int sm_budget, void* stream);
+/* Extended form: ctas_per_sm = CTAs (256 threads each) launched per budgeted SM, 1..4 (0 = default 2). */
+ra_status ra_allreduce_emul_ex(float* const* bufs, int P, size_t count, int sm_budget, int ctas_per_sm, void* stream);
 
 /* ---------------------------------------------------------------------------------------------
  * S5  Alltoall stand-in   ("expert-parallel workloads rely on alltoall to route
@@ -188,7 +190,7 @@ typedef struct {
     ra_occupancy occ;           /* GEMM knobs */
     int32_t coll_sm_budget;     /* 0 = all SMs */
     int32_t coll_smem_bytes;    /* alltoall ring bytes per CTA (0 = default) */
-    int32_t coll_ctas_per_sm;   /* 0 = default */
+    int32_t coll_ctas_per_sm;   /* collective CTAs per budgeted SM; 0 = default */
     int32_t coll_variant;       /* alltoall: 0 = TMA ring, 1 = LDG/STG */
     int32_t prio_compute, prio_comm; /* cudaStreamCreateWithPriority values; equal = "priority off" */
     int32_t dependent;          /* 1: K_c^i waits for K_g^i (the paper's schedule); 0: free-running streams */

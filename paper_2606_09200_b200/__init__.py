@@ -26,7 +26,8 @@ RA_MAX_RANKS = 16
 # every symbol include/ra.h declares (tests/test_abi.py checks the header against this and the .so)
 EXPORTS = (
     "ra_status_str", "ra_last_cuda_error", "ra_shutdown", "ra_device_info", "ra_gemm_plan_query",
-    "ra_gemm_workspace_bytes", "ra_gemm", "ra_allreduce_emul", "ra_alltoall_emul", "ra_alltoall_emul_ex",
+    "ra_gemm_workspace_bytes", "ra_gemm", "ra_allreduce_emul", "ra_allreduce_emul_ex", "ra_alltoall_emul",
+    "ra_alltoall_emul_ex",
     "ra_overlap_run", "ra_overlap_sweep", "ra_set_trace",
 )
 
@@ -95,6 +96,7 @@ def _L():
     lib.ra_gemm.argtypes = [c_int, c_int, c_int, c_int, c_int, c_float, c_void_p, c_int, c_void_p, c_int, c_float,
                             c_void_p, c_int, POINTER(Occupancy), c_void_p, c_size_t, c_void_p]
     lib.ra_allreduce_emul.argtypes = [POINTER(c_void_p), c_int, c_size_t, c_int, c_void_p]
+    lib.ra_allreduce_emul_ex.argtypes = [POINTER(c_void_p), c_int, c_size_t, c_int, c_int, c_void_p]
     lib.ra_alltoall_emul.argtypes = [c_void_p, c_void_p, c_int, c_size_t, c_int, c_void_p]
     lib.ra_alltoall_emul_ex.argtypes = [c_void_p, c_void_p, c_int, c_size_t, c_int, c_int, c_int, c_int, c_void_p]
     lib.ra_overlap_run.argtypes = [POINTER(Workload), POINTER(OverlapCfg), POINTER(OverlapResult)]
@@ -196,6 +198,14 @@ def ra_allreduce_emul(bufs, count=None, sm_budget=0, stream=None) -> None:
         count = bufs[0].numel()
     arr = _ptr_array(bufs)
     _check(_L().ra_allreduce_emul(arr, len(bufs), int(count), int(sm_budget), _stream(stream)), "ra_allreduce_emul")
+
+
+def ra_allreduce_emul_ex(bufs, count=None, sm_budget=0, ctas_per_sm=0, stream=None) -> None:
+    if count is None:
+        count = bufs[0].numel()
+    arr = _ptr_array(bufs)
+    _check(_L().ra_allreduce_emul_ex(arr, len(bufs), int(count), int(sm_budget), int(ctas_per_sm), _stream(stream)),
+           "ra_allreduce_emul_ex")
 
 
 def ra_alltoall_emul(send, recv, P, chunk_bytes, sm_budget=0, stream=None) -> None:

@@ -17,8 +17,13 @@ struct ArPtrs {
     float* p[RA_MAX_RANKS];
 };
 
-constexpr int kArThreads = 512;
-constexpr int kArCtasPerSm = 2;
+// 256 threads x <= 64 registers: 2 warps x 2048 registers per SM sub-partition.  The register file is
+// split four ways (16 K registers per sub-partition), and a resident tcgen05 GEMM CTA (6 warps x 160
+// registers) leaves only 6 K free in two of them -- a 512-thread CTA (8 K per sub-partition) measured
+// 0.03 % co-residency with the GEMM (bench.py residency map), a 256-thread CTA fits.
+constexpr int kArThreads = 256;
+constexpr int kArCtasPerSm = 4;          // launch bound (registers); the default grid uses kArDefaultCtasPerSm
+constexpr int kArDefaultCtasPerSm = 2;
 
 __device__ __forceinline__ float4 ld_stream(const float4* p) {
     float4 v;
@@ -86,9 +91,9 @@ static cudaError_t launch_ar(const ArPtrs& ptrs, size_t count, int grid, cudaStr
     return cudaGetLastError();
 }
 
-ra_status allreduce_launch(float* const* bufs, int P, size_t count, int sm_budget, cudaStream_t stream) {
+ra_status allreduce_launch(float* const* bufs, int P, size_t count, int sm_budget, int ctas_per_sm, cudaStream_t stream) {
     if (bufs == nullptr || P < 1 || P > RA_MAX_RANKS) return RA_ERR_INVALID_ARG;
-    if (sm_budget < 0) return RA_ERR_INVALID_ARG;
+    if (sm_budget < 0 || ctas_per_sm < 0 || ctas_per_sm > kArCtasPerSm) return RA_ERR_INVALID_ARG;
     ArPtrs ptrs{};
     for (int r = 0; r < P; ++r) {
         if (bufs[r] == nullptr || (reinterpret_cast<uintptr_t>(bufs[r]) & 15u)) return RA_ERR_INVALID_ARG;
@@ -110,7 +115,7 @@ ra_status allreduce_launch(float* const* bufs, int P, size_t count, int sm_budge
     const size_t nvec = count >> 2;
     size_t want = (nvec + kArThreads - 1) / kArThreads;
     if (want == 0) want = 1;
-    size_t grid = (size_t)sms * kArCtasPerSm;
+    size_t grid = (size_t)sms * (ctas_per_sm ? ctas_per_sm : kArDefaultCtasPerSm);
     if (grid > want) grid = want;
 
     cudaError_t e;
@@ -128,6 +133,11 @@ ra_status allreduce_launch(float* const* bufs, int P, size_t count, int sm_budge
 
 }  // namespace ra
 
-extern "C" ra_status ra_allreduce_emul(float* const* bufs, int P, size_t count, int sm_budget, void* stream) {
-    return ra::allreduce_launch(bufs, P, count, sm_budget, static_cast<cudaStream_t>(stream));
+extern "C" {
+ra_status ra_allreduce_emul(float* const* bufs, int P, size_t count, int sm_budget, void* stream) {
+    return ra::allreduce_launch(bufs, P, count, sm_budget, 0, static_cast<cudaStream_t>(stream));
+}
+ra_status ra_allreduce_emul_ex(float* const* bufs, int P, size_t count, int sm_budget, int ctas_per_sm, void* stream) {
+    return ra::allreduce_launch(bufs, P, count, sm_budget, ctas_per_sm, static_cast<cudaStream_t>(stream));
+}
 }
