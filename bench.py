@@ -184,6 +184,8 @@ def sweep_candidates(ra, cfg, quick: bool):
                         elif b < info["sm_count"]:
                             cands.append(dict(base, coll_variant=0))
                         cands.append(dict(base, coll_variant=1))
+                        if csb == 0:
+                            cands.append(dict(base, coll_variant=2))     # copy engines: no SM residency at all
                     else:
                         cands.append(base)
     return cands

@@ -155,7 +155,8 @@ ra_status ra_alltoall_emul(const void* send, void* recv, int P, size_t chunk_byt
  *   smem_bytes_per_cta  shared-memory ring per CTA (0 = default 64 KiB).  This is what must fit
  *                       inside the GEMM's smem_reserve_bytes on SMs the two kernels share.
  *   ctas_per_sm         CTAs launched per budgeted SM (0 = default).
- *   variant             0 = TMA bulk-copy ring; 1 = plain 128-bit LDG/STG copy (no shared memory). */
+ *   variant             0 = TMA bulk-copy ring; 1 = plain 128-bit LDG/STG copy (no shared memory);
+ *                       2 = copy engines (P*P cudaMemcpyAsync device-to-device copies, no SM residency). */
 ra_status ra_alltoall_emul_ex(const void* send, void* recv, int P, size_t chunk_bytes, int sm_budget,
                               int smem_bytes_per_cta, int ctas_per_sm, int variant, void* stream);
 
@@ -191,7 +192,7 @@ typedef struct {
     int32_t coll_sm_budget;     /* 0 = all SMs */
     int32_t coll_smem_bytes;    /* alltoall ring bytes per CTA (0 = default) */
     int32_t coll_ctas_per_sm;   /* collective CTAs per budgeted SM; 0 = default */
-    int32_t coll_variant;       /* alltoall: 0 = TMA ring, 1 = LDG/STG */
+    int32_t coll_variant;       /* alltoall: 0 = TMA ring, 1 = LDG/STG, 2 = copy engines */
     int32_t prio_compute, prio_comm; /* cudaStreamCreateWithPriority values; equal = "priority off" */
     int32_t dependent;          /* 1: K_c^i waits for K_g^i (the paper's schedule); 0: free-running streams */
     int32_t record_kernel_times;/* 1: per-kernel event pairs (perturbs the schedule slightly) */

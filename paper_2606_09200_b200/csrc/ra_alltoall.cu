@@ -8,6 +8,7 @@
 // so the SM's LSU and register file stay idle -- the only SM resource the kernel holds is its
 // shared-memory ring, which is exactly what the GEMM's smem_reserve_bytes knob makes room for.
 // Variant 1 is a plain 128-bit LDG/STG copy with no shared memory.  Neither touches TMEM.
+// Variant 2 uses no SM at all: one cudaMemcpyAsync (copy engine) per chunk.
 #include "ra_common.cuh"
 
 namespace ra {
@@ -145,7 +146,7 @@ alltoall_ldg_kernel(const A2aParams p, Trace tr) {
 ra_status alltoall_launch(const void* send, void* recv, int P, size_t chunk_bytes, int sm_budget,
                           int smem_bytes_per_cta, int ctas_per_sm, int variant, cudaStream_t stream) {
     if (send == nullptr || recv == nullptr || P < 1 || P > 256) return RA_ERR_INVALID_ARG;
-    if (sm_budget < 0 || smem_bytes_per_cta < 0 || ctas_per_sm < 0 || (variant != 0 && variant != 1))
+    if (sm_budget < 0 || smem_bytes_per_cta < 0 || ctas_per_sm < 0 || (variant < 0 || variant > 2))
         return RA_ERR_INVALID_ARG;
     if ((reinterpret_cast<uintptr_t>(send) & 15u) || (reinterpret_cast<uintptr_t>(recv) & 15u)) return RA_ERR_INVALID_ARG;
     if (chunk_bytes % 16 != 0) return RA_ERR_INVALID_ARG;
@@ -159,6 +160,19 @@ ra_status alltoall_launch(const void* send, void* recv, int P, size_t chunk_byte
     DeviceInfo di;
     RA_TRY(device_info(&di));
     RA_TRY(require_sm100(di));
+    if (variant == 2) {
+        // SM-free variant (the mechanism of ConCCL): the device's copy engines move the chunks;
+        // no CTA is ever resident, so the GEMM's occupancy knobs are irrelevant to it.  One plain
+        // cudaMemcpyAsync per chunk (i,j) -> (j,i), P*P copies enqueued on `stream`.
+        const char* s8 = static_cast<const char*>(send);
+        char* r8 = static_cast<char*>(recv);
+        for (int i = 0; i < P; ++i) {
+            for (int j = 0; j < P; ++j)
+                RA_CUDA(cudaMemcpyAsync(r8 + ((size_t)j * P + i) * chunk_bytes, s8 + ((size_t)i * P + j) * chunk_bytes,
+                                        chunk_bytes, cudaMemcpyDeviceToDevice, stream));
+        }
+        return RA_OK;
+    }
     const int sms = (sm_budget == 0 || sm_budget > di.sm_count) ? di.sm_count : sm_budget;
 
     A2aParams p{};

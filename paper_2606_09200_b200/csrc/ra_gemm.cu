@@ -45,7 +45,6 @@ constexpr int kEpiThreads = 128;
 constexpr int kMaxStages = 8;
 constexpr int kBarrierBytes = 256;
 constexpr int kAlignSlack = 1024;
-constexpr int kGroupX = 16;     // rasterisation: X-tiles per group
 
 // bytes of one pipeline stage in ONE CTA: 128 rows of X + bn/cg rows of Y, 64 bf16 each
 __host__ __device__ constexpr int stage_bytes(int bn, int cg) { return (kBM + bn / cg) * kBK * 2; }
@@ -62,6 +61,7 @@ struct GemmParams {
     float* partials;   // stream-K: [2*grid][BN][128] fp32
     int* counters;     // stream-K: [n_tiles]
     int hintX, hintY;  // L2 policy per operand: 0 normal, 1 evict_first, 2 evict_last
+    int group_x;       // rasterisation: X-tiles per group
 };
 
 // ---- device helpers ---------------------------------------------------------------------------
@@ -218,12 +218,12 @@ struct Sched {
         return true;
     }
 };
-// grouped rasterisation: kGroupX X-tiles form a group; inside a group x runs fastest.
+// grouped rasterisation: group_x X-tiles form a group; inside a group x runs fastest.
 __device__ __forceinline__ void tile_xy(const GemmParams& p, int tile, int& tx, int& ty) {
-    const int per_group = kGroupX * p.tiles_y;
+    const int per_group = p.group_x * p.tiles_y;
     const int g = tile / per_group;
-    const int first_x = g * kGroupX;
-    const int gsize = min(kGroupX, p.tiles_x - first_x);
+    const int first_x = g * p.group_x;
+    const int gsize = min(p.group_x, p.tiles_x - first_x);
     const int r = tile - g * per_group;
     tx = first_x + r % gsize;
     ty = r / gsize;
@@ -805,6 +805,18 @@ ra_status gemm_launch(int transA, int transB, int M, int N, int K, float alpha, 
     // not displace anything; the small operand every CTA re-reads should stay.
     p.hintX = (p.tiles_y == 1 && p.tiles_x > 1) ? 1 : 0;
     p.hintY = (p.tiles_y == 1 && p.tiles_x > 1) ? 2 : 0;
+    {
+        // Rasterisation.  The W workers of one wave cover a gx x gy block of tiles and march through K together, so
+        // the wave reads (gx*tile_x + gy*BN) rows of K from DRAM once and shares them through L2; with 16 KiB rows
+        // (K = 8192) a wave's footprint (~69 MB) already exceeds what L2 keeps across waves (measured: no cross-wave
+        // reuse), so DRAM traffic ~ waves * (gx*tile_x + gy*BN) rows.  Minimised, subject to gx*gy = W, at
+        // gx = sqrt(W*BN/tile_x): 8 for 74 pairs of 256x256, 16-17 for 148 CTAs of 128x256.
+        const int workers = pl.pub.grid / cg;
+        int gx = 1;
+        while ((long long)(gx + 1) * (gx + 1) * (kBM * cg) <= (long long)workers * pl.bn) ++gx;
+        if (gx > p.tiles_x) gx = p.tiles_x;
+        p.group_x = gx < 1 ? 1 : gx;
+    }
     if (p.stream_k) {
         p.counters = static_cast<int*>(workspace);
         p.partials = reinterpret_cast<float*>(static_cast<uint8_t*>(workspace) + pl.counters_bytes);

@@ -97,7 +97,7 @@ def _run_alltoall(ra, send_np, P, chunk_bytes, **kw):
     return to_host(r, send_np.dtype), s, r
 
 
-@pytest.mark.parametrize("variant", [0, 1])
+@pytest.mark.parametrize("variant", [0, 1, 2])
 @pytest.mark.parametrize("P,chunk", [(1, 16), (2, 48), (3, 1024), (4, 16 * 1024), (8, 16 * 1024 + 16),
                                       (8, 100 * 1024 + 32), (5, 1 << 20)])
 def test_alltoall_tagged(ra, variant, P, chunk):
@@ -107,7 +107,7 @@ def test_alltoall_tagged(ra, variant, P, chunk):
     _assert_bits_equal(got, ref)
 
 
-@pytest.mark.parametrize("variant", [0, 1])
+@pytest.mark.parametrize("variant", [0, 1, 2])
 def test_alltoall_random_bits_and_involution(ra, variant):
     import torch
     cfg = ra_inputs.CONFIGS[3]
