@@ -111,7 +111,8 @@ size_t ra_gemm_workspace_bytes(int transA, int transB, int M, int N, int K, cons
  *   transB = 0: B is K x N, ldb >= N          transB = 1: B is N x K, ldb >= K
  *   C is M x N, ldc >= N.
  * A, B, C: device pointers, 16-byte aligned; lda, ldb, ldc multiples of 8 elements (TMA needs
- * 16-byte row pitch), else RA_ERR_UNSUPPORTED.  C must not overlap A or B.
+ * 16-byte row pitch), else RA_ERR_UNSUPPORTED.  C must not overlap A or B.  All four (transA, transB)
+ * combinations are implemented (K-contiguous operands use K-major, the others MN-major UMMA descriptors).
  * alpha, beta: host scalars by value.  beta == 0 => C is write-only (NaN/Inf already in C do not
  * propagate), as in BLAS.
  * workspace: device pointer, 16-byte aligned, at least ra_gemm_workspace_bytes(...) bytes (may be

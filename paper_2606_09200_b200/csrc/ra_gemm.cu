@@ -62,6 +62,7 @@ struct GemmParams {
     int* counters;     // stream-K: [n_tiles]
     int hintX, hintY;  // L2 policy per operand: 0 normal, 1 evict_first, 2 evict_last
     int group_x;       // rasterisation: X-tiles per group
+    int xmn, ymn;      // operand storage: 0 = K-contiguous rows (K-major), 1 = row index contiguous (MN-major)
 };
 
 // ---- device helpers ---------------------------------------------------------------------------
@@ -122,7 +123,20 @@ __device__ __forceinline__ uint64_t umma_desc_sw128(uint32_t smem_addr) {
     d |= (uint64_t)2 << 61;
     return d;
 }
-// kind::f16 instruction descriptor: D = fp32, A = B = bf16, both K-major, M x N.
+// MN-major, 128-byte swizzle.  The stage holds one 8 KiB box per 64 rows (TMA box = 64 rows x 64 k, the 64 rows
+// contiguous = one 128-byte line per k): canonical layout ((8,8,m),(8,k)) : ((1,8,LBO),(64,SBO)) elements, i.e.
+// 8 k-lines of 128 B form a 1024-B swizzle atom; SBO = 1024 B between 8-k groups, LBO = 8192 B between 64-row boxes.
+// One UMMA (K = 16) spans two k groups, so the k step advances the start address by 2048 B.
+__device__ __forceinline__ uint64_t umma_desc_sw128_mn(uint32_t smem_addr) {
+    uint64_t d = 0;
+    d |= (uint64_t)((smem_addr & 0x3FFFFu) >> 4);
+    d |= (uint64_t)(8192 >> 4) << 16;
+    d |= (uint64_t)(1024 >> 4) << 32;
+    d |= (uint64_t)1 << 46;
+    d |= (uint64_t)2 << 61;
+    return d;
+}
+// kind::f16 instruction descriptor: D = fp32, A = B = bf16, M x N; bit 15 / 16 = A / B is MN-major.
 __host__ __device__ constexpr uint32_t umma_idesc_bf16(int m, int n) {
     return (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(n >> 3) << 17) | ((uint32_t)(m >> 4) << 24);
 }
@@ -365,15 +379,27 @@ gemm_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constant__ CU
                 for (int kb = sg.kb0; kb < sg.kb1; ++kb) {
                     mbar_wait(empty_bar(stage), phase ^ 1u);           // local: MMAs reading this stage retired
                     const uint32_t sx = smem_base + stage * kStageBytes;
+                    uint32_t bar;
                     if constexpr (CG == 1) {
-                        mbar_expect_tx(full_bar(stage), kStageBytes);
-                        tma_load_2d<1>(sx, &mapX, kb * kBK, x0, full_bar(stage), polX);
-                        tma_load_2d<1>(sx + kXBytes, &mapY, kb * kBK, y0, full_bar(stage), polY);
+                        bar = full_bar(stage);
+                        mbar_expect_tx(bar, kStageBytes);
                     } else {
-                        const uint32_t lead_full = mapa(full_bar(stage), 0);   // the leader's barrier collects both halves
-                        mbar_expect_tx_cluster(lead_full, kStageBytes);
-                        tma_load_2d<2>(sx, &mapX, kb * kBK, x0, lead_full, polX);
-                        tma_load_2d<2>(sx + kXBytes, &mapY, kb * kBK, y0, lead_full, polY);
+                        bar = mapa(full_bar(stage), 0);               // the leader's barrier collects both halves
+                        mbar_expect_tx_cluster(bar, kStageBytes);
+                    }
+                    // K-major operand: one box (64 k x rows).  MN-major operand: one box (64 rows x 64 k) per 64 rows.
+                    if (!p.xmn) {
+                        tma_load_2d<CG>(sx, &mapX, kb * kBK, x0, bar, polX);
+                    } else {
+#pragma unroll
+                        for (int b = 0; b < kBM / 64; ++b) tma_load_2d<CG>(sx + b * 8192, &mapX, x0 + 64 * b, kb * kBK, bar, polX);
+                    }
+                    if (!p.ymn) {
+                        tma_load_2d<CG>(sx + kXBytes, &mapY, kb * kBK, y0, bar, polY);
+                    } else {
+#pragma unroll
+                        for (int b = 0; b < kYRows / 64; ++b)
+                            tma_load_2d<CG>(sx + kXBytes + b * 8192, &mapY, y0 + 64 * b, kb * kBK, bar, polY);
                     }
                     if (++stage == p.stages) { stage = 0; phase ^= 1u; }
                 }
@@ -387,6 +413,8 @@ gemm_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constant__ CU
             int stage = 0;
             uint32_t phase = 0;
             int acc_it = 0;
+            const uint32_t idesc = kIdesc | ((uint32_t)p.xmn << 15) | ((uint32_t)p.ymn << 16);
+            const int kx_step = p.xmn ? (2048 >> 4) : (32 >> 4), ky_step = p.ymn ? (2048 >> 4) : (32 >> 4);
             while (sched.next(sg)) {
                 const int buf = acc_it & 1;
                 const uint32_t aphase = (acc_it >> 1) & 1;
@@ -397,12 +425,12 @@ gemm_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constant__ CU
                     mbar_wait(full_bar(stage), phase);     // TMA bytes (of both CTAs) have landed
                     tc_fence_after();
                     const uint32_t sx = smem_base + stage * kStageBytes;
-                    const uint64_t dx = umma_desc_sw128(sx);
-                    const uint64_t dy = umma_desc_sw128(sx + kXBytes);
+                    const uint64_t dx = p.xmn ? umma_desc_sw128_mn(sx) : umma_desc_sw128(sx);
+                    const uint64_t dy = p.ymn ? umma_desc_sw128_mn(sx + kXBytes) : umma_desc_sw128(sx + kXBytes);
 #pragma unroll
                     for (int k = 0; k < kBK / kUmmaK; ++k) {
-                        // +32 B per UMMA_K step inside the swizzle atom = +2 in the (addr >> 4) field
-                        umma_bf16<CG>(tmem_d, dx + (uint64_t)(2 * k), dy + (uint64_t)(2 * k), kIdesc,
+                        // per UMMA_K step: K-major +32 B inside the swizzle atom, MN-major +2 k-groups of 1024 B
+                        umma_bf16<CG>(tmem_d, dx + (uint64_t)(kx_step * k), dy + (uint64_t)(ky_step * k), idesc,
                                       (kb > sg.kb0 || k > 0) ? 1u : 0u);
                     }
                     umma_commit<CG>(empty_bar(stage));     // frees the smem stage (in both CTAs) when these MMAs retire
@@ -548,13 +576,14 @@ static ra_status get_encode(EncodeTiledFn* fn) {
     return RA_OK;
 }
 
-// rows x K bf16, row pitch ld elements; box = 64 (k) x box_rows, 128-byte swizzle, OOB -> zeros.
-static ra_status make_map(CUtensorMap* map, const void* base, int rows, int K, int ld, int box_rows) {
+// K-major operand: rows x K bf16, row pitch ld; box = 64 (k) x box_rows.  MN-major operand: K x rows bf16 (rows
+// contiguous), pitch ld; box = 64 (rows) x 64 (k).  128-byte swizzle, OOB -> zeros.
+static ra_status make_map(CUtensorMap* map, const void* base, int rows, int K, int ld, int box_rows, int mn_major) {
     EncodeTiledFn enc;
     RA_TRY(get_encode(&enc));
-    const cuuint64_t dims[2] = {(cuuint64_t)K, (cuuint64_t)rows};
+    const cuuint64_t dims[2] = {(cuuint64_t)(mn_major ? rows : K), (cuuint64_t)(mn_major ? K : rows)};
     const cuuint64_t strides[1] = {(cuuint64_t)ld * 2};
-    const cuuint32_t box[2] = {(cuuint32_t)kBK, (cuuint32_t)box_rows};
+    const cuuint32_t box[2] = {(cuuint32_t)(mn_major ? 64 : kBK), (cuuint32_t)(mn_major ? kBK : box_rows)};
     const cuuint32_t estr[2] = {1, 1};
     const CUresult r = enc(map, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(base), dims, strides, box, estr,
                            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
@@ -581,7 +610,6 @@ static ra_status validate_shape(int transA, int transB, int M, int N, int K) {
 
 static ra_status make_plan(int transA, int transB, int M, int N, int K, const ra_occupancy* occ_in, Plan* out) {
     RA_TRY(validate_shape(transA, transB, M, N, K));
-    if (transA != 0 || transB != 1) return RA_ERR_UNSUPPORTED;   // K-contiguous operands only (A13)
     ra_occupancy occ = {0, 0, 0, 1, 0};
     if (occ_in) occ = *occ_in;
     if (occ.smem_reserve_bytes < 0 || occ.sm_budget < 0 || occ.tiles_per_cta < 0) return RA_ERR_INVALID_ARG;
@@ -826,8 +854,12 @@ ra_status gemm_launch(int transA, int transB, int M, int N, int K, float alpha, 
     const void* Y = swap ? A : B;
     const int ldx = swap ? ldb : lda, ldy = swap ? lda : ldb;
     CUtensorMap mx, my;
-    RA_TRY(make_map(&mx, X, p.RX, K, ldx, kBM));
-    RA_TRY(make_map(&my, Y, p.RY, K, ldy, pl.bn / cg));
+    // op(A)(i,k): K-contiguous iff transA == 0;  op(B)(k,j): K-contiguous iff transB == 1
+    const int a_mn = transA ? 1 : 0, b_mn = transB ? 0 : 1;
+    p.xmn = swap ? b_mn : a_mn;
+    p.ymn = swap ? a_mn : b_mn;
+    RA_TRY(make_map(&mx, X, p.RX, K, ldx, kBM, p.xmn));
+    RA_TRY(make_map(&my, Y, p.RY, K, ldy, pl.bn / cg, p.ymn));
     if (cg == 2) return launch_gemm<256, 2>(mx, my, p, pl.pub.grid, pl.pub.dyn_smem_bytes, stream);
     switch (pl.bn) {
         case 64: return launch_gemm<64, 1>(mx, my, p, pl.pub.grid, pl.pub.dyn_smem_bytes, stream);

@@ -109,7 +109,7 @@ def test_argument_errors_need_no_gpu(ra):
     g = dict(transA=0, transB=1, M=32, N=32, K=64, alpha=1.0, A=fake, lda=64, B=fake + (1 << 20), ldb=64, beta=0.0,
              C=fake + (2 << 20), ldc=32)
     for kw, st in [(dict(M=-1), 1), (dict(transA=2), 1), (dict(A=None), 1), (dict(lda=8), 1), (dict(ldc=24), 1),
-                   (dict(ldc=36), 2), (dict(A=fake + 2), 1), (dict(transB=0, ldb=64), 2), (dict(M=0), 0)]:
+                   (dict(ldc=36), 2), (dict(A=fake + 2), 1), (dict(transB=0, ldb=24), 1), (dict(transA=1, lda=24), 1), (dict(M=0), 0)]:
         a = dict(g, **kw)
         s = lib.ra_gemm(a["transA"], a["transB"], a["M"], a["N"], a["K"], a["alpha"], a["A"], a["lda"], a["B"], a["ldb"],
                         a["beta"], a["C"], a["ldc"], None, None, 0, None)

@@ -19,20 +19,21 @@ def ra():
     return m
 
 
-def run_gemm(ra, M, N, K, A, B, alpha=1.0, beta=0.0, Cin=None, occ=None, lda=None, ldb=None, ldc=None, fill=None):
-    """A: [M, lda] bits, B: [N, ldb] bits (transA=0, transB=1).  Returns C bits [M, N]."""
+def run_gemm(ra, M, N, K, A, B, alpha=1.0, beta=0.0, Cin=None, occ=None, lda=None, ldb=None, ldc=None, fill=None,
+             transA=0, transB=1):
+    """A, B: bit arrays in the storage the trans flags describe.  Returns C bits [M, N] and the full [M, ldc] buffer."""
     import torch
-    lda = lda or K
-    ldb = ldb or K
+    lda = lda or (M if transA else K)
+    ldb = ldb or (K if transB else N)
     ldc = ldc or N
     dA, dB = to_dev(A), to_dev(B)
     if Cin is not None:
         dC = to_dev(Cin)
     else:
         dC = torch.full((M, ldc), 0x7FC0 if fill is None else fill, dtype=torch.int16, device="cuda")  # NaN-filled
-    ws_bytes = ra.ra_gemm_workspace_bytes(0, 1, M, N, K, occ)
+    ws_bytes = ra.ra_gemm_workspace_bytes(transA, transB, M, N, K, occ)
     ws = torch.empty(max(ws_bytes, 16), dtype=torch.uint8, device="cuda")
-    ra.ra_gemm(0, 1, M, N, K, alpha, dA, lda, dB, ldb, beta, dC, ldc, occ=occ, workspace=ws)
+    ra.ra_gemm(transA, transB, M, N, K, alpha, dA, lda, dB, ldb, beta, dC, ldc, occ=occ, workspace=ws)
     torch.cuda.synchronize()
     out = to_host(dC, np.uint16).reshape(M, ldc)
     return out[:, :N].copy(), out
@@ -42,23 +43,49 @@ def _up8(x):
     return (x + 7) // 8 * 8
 
 
-def check(ra, M, N, K, seed, alpha=1.0, beta=0.0, occ=None):
+def check(ra, M, N, K, seed, alpha=1.0, beta=0.0, occ=None, transA=0, transB=1):
     # leading dimensions rounded up to the 8-element pitch TMA needs; the pad columns hold data too
     # (so a kernel that ignored ld would read/write the wrong elements)
-    lda = ldb = _up8(K) + (8 if K % 16 else 0)
+    def pad(x):
+        return _up8(x) + (8 if x % 16 else 0)
+    lda = pad(M) if transA else pad(K)
+    ldb = pad(K) if transB else pad(N)
     ldc = _up8(N)
-    A = ra_inputs.normal_bf16((M, lda), seed, ra_inputs.STREAM_A)
-    B = ra_inputs.normal_bf16((N, ldb), seed, ra_inputs.STREAM_B)
+    A = ra_inputs.normal_bf16((K if transA else M, lda), seed, ra_inputs.STREAM_A)
+    B = ra_inputs.normal_bf16((N if transB else K, ldb), seed, ra_inputs.STREAM_B)
     Cin = ra_inputs.normal_bf16((M, ldc), seed, ra_inputs.STREAM_C) if beta != 0.0 else None
-    ref, _ = oracle.gemm(0, 1, M, N, K, alpha, A, B, beta, Cin, lda=lda, ldb=ldb, ldc=ldc)
-    rowA, colB = oracle.gemm_norms(0, 1, M, N, K, A, B, lda=lda, ldb=ldb)
-    got, full = run_gemm(ra, M, N, K, A, B, alpha, beta, Cin, occ, lda=lda, ldb=ldb, ldc=ldc)
+    ref, _ = oracle.gemm(transA, transB, M, N, K, alpha, A, B, beta, Cin, lda=lda, ldb=ldb, ldc=ldc)
+    rowA, colB = oracle.gemm_norms(transA, transB, M, N, K, A, B, lda=lda, ldb=ldb)
+    got, full = run_gemm(ra, M, N, K, A, B, alpha, beta, Cin, occ, lda=lda, ldb=ldb, ldc=ldc, transA=transA, transB=transB)
     cin_view = Cin[:, :N] if Cin is not None else None
     err = gemm_norm_err(got, ref, rowA, colB, alpha, beta, cin_view)
-    assert err <= GEMM_TOL, f"normalised error {err} for {M}x{N}x{K} plan {ra.ra_gemm_plan_query(0, 1, M, N, K, occ)}"
+    assert err <= GEMM_TOL, (f"normalised error {err} for {M}x{N}x{K} trans {transA}{transB} "
+                             f"plan {ra.ra_gemm_plan_query(transA, transB, M, N, K, occ)}")
     if Cin is not None and ldc > N:
         assert np.array_equal(full[:, N:], Cin[:, N:]), "pad columns of C were modified"
     return err
+
+
+@pytest.mark.parametrize("transA,transB", [(0, 0), (1, 0), (1, 1)])
+@pytest.mark.parametrize("M,N,K,occ", [
+    (128, 256, 64, None), (200, 136, 72, None), (130, 260, 200, None), (384, 768, 2048, None),     # single-CTA tiles
+    (64, 1024, 2048, None), (17, 640, 1536, None),                                                  # operand swap (+ stream-K)
+    (512, 512, 256, dict(cta_group=2)), (1000, 520, 200, dict(cta_group=2)), (2048, 2048, 512, dict(cta_group=2)),  # CTA pairs
+    (300, 200, 4096, None),                                                                         # stream-K
+])
+def test_all_trans_combinations(ra, transA, transB, M, N, K, occ):
+    """op(A), op(B) of PAPER.md:28: every storage order of both operands (MN-major UMMA descriptors + TMA boxes)."""
+    check(ra, M, N, K, seed=7000 + M + N + K, occ=occ, transA=transA, transB=transB)
+
+
+@pytest.mark.parametrize("transA,transB", [(0, 0), (1, 0), (1, 1)])
+def test_trans_integer_exact(ra, transA, transB):
+    M, N, K = 384, 520, 1024
+    A = ra_inputs.smallint_bf16((K, M) if transA else (M, K), 51, ra_inputs.STREAM_A)
+    B = ra_inputs.smallint_bf16((N, K) if transB else (K, N), 51, ra_inputs.STREAM_B)
+    _, ref16 = oracle.gemm(transA, transB, M, N, K, 1.0, A, B)
+    got, _ = run_gemm(ra, M, N, K, A, B, transA=transA, transB=transB)
+    assert np.array_equal(got, ref16)
 
 
 def test_tiny_config(ra):
@@ -209,7 +236,7 @@ def test_errors(ra):
     b = torch.zeros(64 * 64, dtype=torch.int16, device="cuda")
     c = torch.zeros(64 * 64, dtype=torch.int16, device="cuda")
     for kw, st in [
-        (dict(transA=1), ra.RA_ERR_UNSUPPORTED), (dict(lda=60), ra.RA_ERR_INVALID_ARG), (dict(lda=68), ra.RA_ERR_UNSUPPORTED),
+        (dict(transA=1, lda=24), ra.RA_ERR_INVALID_ARG), (dict(lda=60), ra.RA_ERR_INVALID_ARG), (dict(lda=68), ra.RA_ERR_UNSUPPORTED),
         (dict(M=-1), ra.RA_ERR_INVALID_ARG), (dict(C=a), ra.RA_ERR_INVALID_ARG),
     ]:
         args = dict(transA=0, transB=1, M=32, N=32, K=64, alpha=1.0, A=a, lda=64, B=b, ldb=64, beta=0.0, C=c, ldc=64)
