@@ -40,12 +40,13 @@ class RaError(RuntimeError):
 
 class Occupancy(Structure):
     _fields_ = [("smem_reserve_bytes", c_int32), ("sm_budget", c_int32), ("tiles_per_cta", c_int32),
-                ("allow_clamp", c_int32), ("cta_group", c_int32)]
+                ("allow_clamp", c_int32), ("cta_group", c_int32), ("m_blocks", c_int32)]
 
 
 class GemmPlan(Structure):
     _fields_ = [(n, c_int32) for n in ("ctas_per_sm", "grid", "stages", "tile_m", "tile_n", "tile_k", "split_k",
-                                       "swap_ab", "dyn_smem_bytes", "smem_left_per_sm", "n_tiles", "clamped", "cta_group")]
+                                       "swap_ab", "dyn_smem_bytes", "smem_left_per_sm", "n_tiles", "clamped", "cta_group",
+                                       "m_blocks")]
 
     def as_dict(self):
         return {n: getattr(self, n) for n, _ in self._fields_}
@@ -150,7 +151,8 @@ def _occ(occ) -> Occupancy | None:
     if occ is None or isinstance(occ, Occupancy):
         return occ
     return Occupancy(int(occ.get("smem_reserve_bytes", 0)), int(occ.get("sm_budget", 0)),
-                     int(occ.get("tiles_per_cta", 0)), int(occ.get("allow_clamp", 1)), int(occ.get("cta_group", 0)))
+                     int(occ.get("tiles_per_cta", 0)), int(occ.get("allow_clamp", 1)), int(occ.get("cta_group", 0)),
+                     int(occ.get("m_blocks", 0)))
 
 
 def _occ_ref(occ):

@@ -46,8 +46,8 @@ constexpr int kMaxStages = 8;
 constexpr int kBarrierBytes = 256;
 constexpr int kAlignSlack = 1024;
 
-// bytes of one pipeline stage in ONE CTA: 128 rows of X + bn/cg rows of Y, 64 bf16 each
-__host__ __device__ constexpr int stage_bytes(int bn, int cg) { return (kBM + bn / cg) * kBK * 2; }
+// bytes of one pipeline stage in ONE CTA: 128*xh rows of X + bn/cg rows of Y, 64 bf16 each
+__host__ __device__ constexpr int stage_bytes(int bn, int cg, int xh) { return (kBM * xh + bn / cg) * kBK * 2; }
 
 struct GemmParams {
     int RX, RY, K;
@@ -298,21 +298,30 @@ __device__ __forceinline__ void store_out(const GemmParams& p, const float (&acc
     }
 }
 
-template <int BN, int CG>
+template <int BN, int CG, int XH>
 __global__ void __launch_bounds__(kGemmThreads, 1)
 gemm_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constant__ CUtensorMap mapY, const GemmParams p,
             Trace tr) {
     // CG == 2: the CTA pair of a 2-cluster works on one 256 x BN tile.  Each CTA stages its own 128 rows of X
     // and its own BN/2 rows of Y; the leader (cluster rank 0) issues tcgen05.mma.cta_group::2, which reads both
     // CTAs' stages and writes rows [128*rank, 128*rank+128) of the accumulator into each CTA's TMEM.
+    //
+    // XH == 2 ("big" tiles): every CTA owns 256 rows of X as two 128-row blocks that share one Y stage, i.e. two
+    // MMAs per k-step into two accumulators (TMEM columns [0,BN) and [BN,2BN)).  A pair then covers 512 x 256 and
+    // stages 256 + 128 rows per k-block instead of 2 x (128 + 128): 25 % less L2->SM traffic per flop, which is
+    // what bounds the 256 x 256 pair tile (64 B/clk/SM).  The price: both accumulators belong to the current
+    // tile, so the epilogue overlaps only the first k-blocks of the next tile (see the MMA issuer).
     constexpr int kYRows = BN / CG;
-    constexpr int kXBytes = kBM * kBK * 2;
+    constexpr int kXHalfBytes = kBM * kBK * 2;
+    constexpr int kXBytes = XH * kXHalfBytes;
     constexpr int kStageBytes = kXBytes + kYRows * kBK * 2;
-    constexpr int kTmemCols = 2 * BN;   // two accumulators (power of two for BN in {64,128,256})
+    constexpr int kTmemCols = 2 * BN;   // XH == 1: two accumulators (double buffer); XH == 2: the two X blocks of one tile
+    constexpr int kTileX = kBM * XH * CG;
     constexpr uint32_t kIdesc = umma_idesc_bf16(kBM * CG, BN);
     static_assert(BN == 64 || BN == 128 || BN == 256, "BN");
     static_assert(CG == 1 || CG == 2, "CG");
-    static_assert(kStageBytes == stage_bytes(BN, CG), "stage size");
+    static_assert(XH == 1 || XH == 2, "XH");
+    static_assert(kStageBytes == stage_bytes(BN, CG, XH), "stage size");
 
     extern __shared__ uint8_t smem_raw[];
     // 1024-byte alignment for the 128B swizzle; the barrier block sits after the stages.  Both CTAs of a pair
@@ -374,7 +383,7 @@ gemm_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constant__ CU
             while (sched.next(sg)) {
                 int tx, ty;
                 tile_xy(p, sg.tile, tx, ty);
-                const int x0 = tx * (kBM * CG) + (int)rank * kBM;
+                const int x0 = tx * kTileX + (int)rank * (kBM * XH);
                 const int y0 = ty * BN + (int)rank * kYRows;
                 for (int kb = sg.kb0; kb < sg.kb1; ++kb) {
                     mbar_wait(empty_bar(stage), phase ^ 1u);           // local: MMAs reading this stage retired
@@ -392,7 +401,7 @@ gemm_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constant__ CU
                         tma_load_2d<CG>(sx, &mapX, kb * kBK, x0, bar, polX);
                     } else {
 #pragma unroll
-                        for (int b = 0; b < kBM / 64; ++b) tma_load_2d<CG>(sx + b * 8192, &mapX, x0 + 64 * b, kb * kBK, bar, polX);
+                        for (int b = 0; b < kBM * XH / 64; ++b) tma_load_2d<CG>(sx + b * 8192, &mapX, x0 + 64 * b, kb * kBK, bar, polX);
                     }
                     if (!p.ymn) {
                         tma_load_2d<CG>(sx + kXBytes, &mapY, kb * kBK, y0, bar, polY);
@@ -416,27 +425,40 @@ gemm_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constant__ CU
             const uint32_t idesc = kIdesc | ((uint32_t)p.xmn << 15) | ((uint32_t)p.ymn << 16);
             const int kx_step = p.xmn ? (2048 >> 4) : (32 >> 4), ky_step = p.ymn ? (2048 >> 4) : (32 >> 4);
             while (sched.next(sg)) {
-                const int buf = acc_it & 1;
-                const uint32_t aphase = (acc_it >> 1) & 1;
-                mbar_wait(tempty_bar(buf), aphase ^ 1u);   // every epilogue warp (of the pair) drained this accumulator
-                tc_fence_after();
-                const uint32_t tmem_d = tmem_base + (uint32_t)(buf * BN);
+                // XH == 1: accumulator acc_it & 1 (double buffer).  XH == 2: block h of the tile accumulates in
+                // columns [h*BN, h*BN + BN); each block has its own "drained" barrier so block 0 of this tile can
+                // start while the epilogue is still reading block 1 of the previous one.
+                const int buf = (XH == 1) ? (acc_it & 1) : 0;
+                const uint32_t aphase = (XH == 1) ? ((acc_it >> 1) & 1) : (acc_it & 1);
+                if constexpr (XH == 1) {
+                    mbar_wait(tempty_bar(buf), aphase ^ 1u);   // every epilogue warp (of the pair) drained this accumulator
+                    tc_fence_after();
+                }
                 for (int kb = sg.kb0; kb < sg.kb1; ++kb) {
                     mbar_wait(full_bar(stage), phase);     // TMA bytes (of both CTAs) have landed
                     tc_fence_after();
                     const uint32_t sx = smem_base + stage * kStageBytes;
-                    const uint64_t dx = p.xmn ? umma_desc_sw128_mn(sx) : umma_desc_sw128(sx);
                     const uint64_t dy = p.ymn ? umma_desc_sw128_mn(sx + kXBytes) : umma_desc_sw128(sx + kXBytes);
 #pragma unroll
-                    for (int k = 0; k < kBK / kUmmaK; ++k) {
-                        // per UMMA_K step: K-major +32 B inside the swizzle atom, MN-major +2 k-groups of 1024 B
-                        umma_bf16<CG>(tmem_d, dx + (uint64_t)(kx_step * k), dy + (uint64_t)(ky_step * k), idesc,
-                                      (kb > sg.kb0 || k > 0) ? 1u : 0u);
+                    for (int h = 0; h < XH; ++h) {
+                        if (XH == 2 && kb == sg.kb0) {
+                            mbar_wait(tempty_bar(h), aphase ^ 1u);
+                            tc_fence_after();
+                        }
+                        const uint32_t sxh = sx + h * kXHalfBytes;
+                        const uint64_t dx = p.xmn ? umma_desc_sw128_mn(sxh) : umma_desc_sw128(sxh);
+                        const uint32_t tmem_d = tmem_base + (uint32_t)((XH == 1 ? buf : h) * BN);
+#pragma unroll
+                        for (int k = 0; k < kBK / kUmmaK; ++k) {
+                            // per UMMA_K step: K-major +32 B inside the swizzle atom, MN-major +2 k-groups of 1024 B
+                            umma_bf16<CG>(tmem_d, dx + (uint64_t)(kx_step * k), dy + (uint64_t)(ky_step * k), idesc,
+                                          (kb > sg.kb0 || k > 0) ? 1u : 0u);
+                        }
                     }
                     umma_commit<CG>(empty_bar(stage));     // frees the smem stage (in both CTAs) when these MMAs retire
                     if (++stage == p.stages) { stage = 0; phase ^= 1u; }
                 }
-                umma_commit<CG>(tfull_bar(buf));           // accumulator complete (signals both CTAs' epilogues)
+                umma_commit<CG>(tfull_bar(buf));           // accumulator(s) complete (signals both CTAs' epilogues)
                 ++acc_it;
             }
         }
@@ -449,12 +471,12 @@ gemm_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constant__ CU
         Seg sg;
         int acc_it = 0;
         while (sched.next(sg)) {
-            const int buf = acc_it & 1;
-            const uint32_t aphase = (acc_it >> 1) & 1;
+            const int buf = (XH == 1) ? (acc_it & 1) : 0;
+            const uint32_t aphase = (XH == 1) ? ((acc_it >> 1) & 1) : (acc_it & 1);
             int tx, ty;
             tile_xy(p, sg.tile, tx, ty);
             const bool whole = (sg.kb0 == 0 && sg.kb1 == p.kb_per_tile);
-            const int x = tx * (kBM * CG) + (int)rank * kBM + xl;
+            const int x = tx * kTileX + (int)rank * (kBM * XH) + xl;   // row of X block 0
             float* part = nullptr;
             if (!whole) {
                 const int slot = 2 * wid + (sg.start_unit == sched.u0 ? 0 : 1);
@@ -462,28 +484,32 @@ gemm_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constant__ CU
             }
             mbar_wait(tfull_bar(buf), aphase);
             tc_fence_after();
-            const uint32_t taddr = tmem_base + ((uint32_t)(quarter * 32) << 16) + (uint32_t)(buf * BN);
 #pragma unroll 1
-            for (int c = 0; c < BN / 32; ++c) {
-                uint32_t v[32];
-                tmem_ld32(taddr + c * 32, v);
-                tmem_ld_wait();
-                float acc[32];
+            for (int h = 0; h < XH; ++h) {
+                const int acc_idx = (XH == 1) ? buf : h;
+                const uint32_t taddr = tmem_base + ((uint32_t)(quarter * 32) << 16) + (uint32_t)(acc_idx * BN);
+#pragma unroll 1
+                for (int c = 0; c < BN / 32; ++c) {
+                    uint32_t v[32];
+                    tmem_ld32(taddr + c * 32, v);
+                    tmem_ld_wait();
+                    float acc[32];
 #pragma unroll
-                for (int j = 0; j < 32; ++j) acc[j] = __uint_as_float(v[j]);
-                if (whole) {
-                    store_out(p, acc, x, ty * BN + c * 32);
-                } else {
+                    for (int j = 0; j < 32; ++j) acc[j] = __uint_as_float(v[j]);
+                    if (whole) {
+                        store_out(p, acc, x + h * kBM, ty * BN + c * 32);
+                    } else {
 #pragma unroll
-                    for (int j = 0; j < 32; ++j) __stcg(part + (size_t)(c * 32 + j) * kBM + xl, acc[j]);
+                        for (int j = 0; j < 32; ++j) __stcg(part + (size_t)(c * 32 + j) * kBM + xl, acc[j]);
+                    }
                 }
-            }
-            // this warp's quarter of the accumulator is drained: tell the (leader's) MMA issuer
-            tc_fence_before();
-            __syncwarp();
-            if (lane == 0) {
-                if constexpr (CG == 1) mbar_arrive(tempty_bar(buf));
-                else mbar_arrive_cluster(mapa(tempty_bar(buf), 0));
+                // this warp's quarter of the accumulator is drained: tell the (leader's) MMA issuer
+                tc_fence_before();
+                __syncwarp();
+                if (lane == 0) {
+                    if constexpr (CG == 1) mbar_arrive(tempty_bar(acc_idx));
+                    else mbar_arrive_cluster(mapa(tempty_bar(acc_idx), 0));
+                }
             }
             ++acc_it;
 
@@ -610,7 +636,7 @@ static ra_status validate_shape(int transA, int transB, int M, int N, int K) {
 
 static ra_status make_plan(int transA, int transB, int M, int N, int K, const ra_occupancy* occ_in, Plan* out) {
     RA_TRY(validate_shape(transA, transB, M, N, K));
-    ra_occupancy occ = {0, 0, 0, 1, 0};
+    ra_occupancy occ = {0, 0, 0, 1, 0, 0};
     if (occ_in) occ = *occ_in;
     if (occ.smem_reserve_bytes < 0 || occ.sm_budget < 0 || occ.tiles_per_cta < 0) return RA_ERR_INVALID_ARG;
 
@@ -645,13 +671,14 @@ static ra_status make_plan(int transA, int transB, int M, int N, int K, const ra
     int bn = RY > 128 ? 256 : (RY > 64 ? 128 : 64);
     const int kb = (K + kBK - 1) / kBK;
     if (occ.cta_group < 0 || occ.cta_group > 2) return RA_ERR_INVALID_ARG;
+    if (occ.m_blocks < 0 || occ.m_blocks > 2) return RA_ERR_INVALID_ARG;
 
     // shared memory the GEMM may allocate on an SM
     long avail = (long)smem_per_sm - occ.smem_reserve_bytes - reserved;
     if (avail > optin) avail = optin;
     const long room = avail - kAlignSlack - kBarrierBytes;
-    auto stages_for = [&](int bn_, int cg_) {
-        int s = room > 0 ? (int)(room / stage_bytes(bn_, cg_)) : 0;
+    auto stages_for = [&](int bn_, int cg_, int xh_) {
+        int s = room > 0 ? (int)(room / stage_bytes(bn_, cg_, xh_)) : 0;
         return s > kMaxStages ? kMaxStages : s;
     };
     auto wave_eff = [](long long tiles, int workers) {
@@ -662,7 +689,7 @@ static ra_status make_plan(int transA, int transB, int M, int N, int K, const ra
     // CTA pairs (cta_group::2, 256 x 256 tiles): each SM stages 128 rows of X and 128 of Y per k-block instead of
     // 128 + 256, i.e. 1/3 less L2->SM traffic per flop.  Used for the data-parallel schedule on large problems.
     int cg = 1;
-    if (occ.cta_group != 1 && !swap && bn == 256 && RX >= 256 && budget >= 2 && stages_for(256, 2) >= 2) {
+    if (occ.cta_group != 1 && !swap && bn == 256 && RX >= 256 && budget >= 2 && stages_for(256, 2, 1) >= 2) {
         const long long t2 = (long long)((RX + 2 * kBM - 1) / (2 * kBM)) * ((RY + bn - 1) / bn);
         // measured on B200: pairs at 86 % wave efficiency (4096^3) still beat single-CTA stream-K by 28 %
         const bool sk_wanted = occ.tiles_per_cta == 0 && kb >= 8 && wave_eff(t2, budget / 2) < 0.7;
@@ -673,9 +700,25 @@ static ra_status make_plan(int transA, int transB, int M, int N, int K, const ra
         clamped = 1;
     }
 
+    // Big tiles (two 128-row X blocks per CTA sharing one Y stage; a pair covers 512 x 256): 48 B/clk/SM of
+    // operand traffic instead of 64, which is the L2->SM limit the 256 x 256 pair tile runs into (the tensor pipe
+    // was 85-88 % busy; cuBLAS's 256x256-per-CTA kernel 96 %).  Needs >= 3 stages of 48 KiB and enough tiles that
+    // the coarser wave quantisation does not eat the gain.
+    int xh = 1;
+    if (cg == 2 && occ.m_blocks != 1 && RX >= 4 * kBM && stages_for(256, 2, 2) >= 3 && occ.tiles_per_cta == 0) {
+        const long long t1 = (long long)((RX + 2 * kBM - 1) / (2 * kBM)) * ((RY + bn - 1) / bn);
+        const long long t2 = (long long)((RX + 4 * kBM - 1) / (4 * kBM)) * ((RY + bn - 1) / bn);
+        const double e1 = wave_eff(t1, budget / 2) * 0.88, e2 = wave_eff(t2, budget / 2) * 0.96;
+        if (e2 >= e1 || occ.m_blocks == 2) xh = 2;
+    }
+    if (occ.m_blocks == 2 && xh != 2) {
+        if (!occ.allow_clamp) return RA_ERR_INFEASIBLE_KNOB;
+        clamped = 1;
+    }
+
     int stages = 0;
     for (;;) {
-        stages = stages_for(bn, cg);
+        stages = stages_for(bn, cg, xh);
         if (stages >= 2 || bn == 64) break;
         bn >>= 1;   // squeeze the tile before giving up pipelining
     }
@@ -684,9 +727,9 @@ static ra_status make_plan(int transA, int transB, int M, int N, int K, const ra
         stages = 1;
         clamped = 1;
     }
-    int dyn = stages * stage_bytes(bn, cg) + kAlignSlack + kBarrierBytes;
+    int dyn = stages * stage_bytes(bn, cg, xh) + kAlignSlack + kBarrierBytes;
 
-    const int tile_x = kBM * cg;
+    const int tile_x = kBM * cg * xh;
     const int tiles_x = (RX + tile_x - 1) / tile_x, tiles_y = (RY + bn - 1) / bn;
     const long long n_tiles = (long long)tiles_x * tiles_y;
     if (n_tiles > 0x3fffffffLL) return RA_ERR_UNSUPPORTED;
@@ -734,6 +777,7 @@ static ra_status make_plan(int transA, int transB, int M, int N, int K, const ra
     g.clamped = clamped;
     g.split_k = 1;
     g.cta_group = cg;
+    g.m_blocks = xh;
     pl.bn = bn;
     if (stream_k) {
         const long long U = n_tiles * kb;
@@ -747,12 +791,12 @@ static ra_status make_plan(int transA, int transB, int M, int N, int K, const ra
     return RA_OK;
 }
 
-template <int BN, int CG>
+template <int BN, int CG, int XH>
 static ra_status launch_gemm(const CUtensorMap& mx, const CUtensorMap& my, const GemmParams& p, int grid, int dyn,
                              cudaStream_t stream) {
-    RA_CUDA(cudaFuncSetAttribute(gemm_kernel<BN, CG>, cudaFuncAttributeMaxDynamicSharedMemorySize, dyn));
+    RA_CUDA(cudaFuncSetAttribute(gemm_kernel<BN, CG, XH>, cudaFuncAttributeMaxDynamicSharedMemorySize, dyn));
     if constexpr (CG == 1) {
-        gemm_kernel<BN, 1><<<grid, kGemmThreads, dyn, stream>>>(mx, my, p, g_trace);
+        gemm_kernel<BN, 1, XH><<<grid, kGemmThreads, dyn, stream>>>(mx, my, p, g_trace);
         RA_CUDA(cudaGetLastError());
         return RA_OK;
     }
@@ -768,7 +812,7 @@ static ra_status launch_gemm(const CUtensorMap& mx, const CUtensorMap& my, const
     attr[0].val.clusterDim.z = 1;
     cfg.attrs = attr;
     cfg.numAttrs = 1;
-    RA_CUDA(cudaLaunchKernelEx(&cfg, gemm_kernel<BN, CG>, mx, my, p, g_trace));
+    RA_CUDA(cudaLaunchKernelEx(&cfg, gemm_kernel<BN, CG, XH>, mx, my, p, g_trace));
     return RA_OK;
 }
 
@@ -817,8 +861,9 @@ ra_status gemm_launch(int transA, int transB, int M, int N, int K, float alpha, 
     p.RX = swap ? N : M;
     p.RY = swap ? M : N;
     p.K = K;
-    const int cg = pl.pub.cta_group;
-    p.tiles_x = (p.RX + kBM * cg - 1) / (kBM * cg);
+    const int cg = pl.pub.cta_group, xh = pl.pub.m_blocks;
+    const int tile_x = kBM * cg * xh;
+    p.tiles_x = (p.RX + tile_x - 1) / tile_x;
     p.tiles_y = (p.RY + pl.bn - 1) / pl.bn;
     p.n_tiles = pl.pub.n_tiles;
     p.kb_per_tile = (K + kBK - 1) / kBK;
@@ -841,7 +886,7 @@ ra_status gemm_launch(int transA, int transB, int M, int N, int K, float alpha, 
         // gx = sqrt(W*BN/tile_x): 8 for 74 pairs of 256x256, 16-17 for 148 CTAs of 128x256.
         const int workers = pl.pub.grid / cg;
         int gx = 1;
-        while ((long long)(gx + 1) * (gx + 1) * (kBM * cg) <= (long long)workers * pl.bn) ++gx;
+        while ((long long)(gx + 1) * (gx + 1) * tile_x <= (long long)workers * pl.bn) ++gx;
         if (gx > p.tiles_x) gx = p.tiles_x;
         p.group_x = gx < 1 ? 1 : gx;
     }
@@ -858,13 +903,14 @@ ra_status gemm_launch(int transA, int transB, int M, int N, int K, float alpha, 
     const int a_mn = transA ? 1 : 0, b_mn = transB ? 0 : 1;
     p.xmn = swap ? b_mn : a_mn;
     p.ymn = swap ? a_mn : b_mn;
-    RA_TRY(make_map(&mx, X, p.RX, K, ldx, kBM, p.xmn));
+    RA_TRY(make_map(&mx, X, p.RX, K, ldx, kBM * xh, p.xmn));
     RA_TRY(make_map(&my, Y, p.RY, K, ldy, pl.bn / cg, p.ymn));
-    if (cg == 2) return launch_gemm<256, 2>(mx, my, p, pl.pub.grid, pl.pub.dyn_smem_bytes, stream);
+    if (cg == 2 && xh == 2) return launch_gemm<256, 2, 2>(mx, my, p, pl.pub.grid, pl.pub.dyn_smem_bytes, stream);
+    if (cg == 2) return launch_gemm<256, 2, 1>(mx, my, p, pl.pub.grid, pl.pub.dyn_smem_bytes, stream);
     switch (pl.bn) {
-        case 64: return launch_gemm<64, 1>(mx, my, p, pl.pub.grid, pl.pub.dyn_smem_bytes, stream);
-        case 128: return launch_gemm<128, 1>(mx, my, p, pl.pub.grid, pl.pub.dyn_smem_bytes, stream);
-        case 256: return launch_gemm<256, 1>(mx, my, p, pl.pub.grid, pl.pub.dyn_smem_bytes, stream);
+        case 64: return launch_gemm<64, 1, 1>(mx, my, p, pl.pub.grid, pl.pub.dyn_smem_bytes, stream);
+        case 128: return launch_gemm<128, 1, 1>(mx, my, p, pl.pub.grid, pl.pub.dyn_smem_bytes, stream);
+        case 256: return launch_gemm<256, 1, 1>(mx, my, p, pl.pub.grid, pl.pub.dyn_smem_bytes, stream);
     }
     return RA_ERR_UNSUPPORTED;
 }

@@ -38,11 +38,11 @@ def test_status_strings(ra):
 
 def test_struct_layouts_match_header(ra):
     # sizes computed by hand from include/ra.h (LP64)
-    assert ctypes.sizeof(ra.Occupancy) == 20
-    assert ctypes.sizeof(ra.GemmPlan) == 52
+    assert ctypes.sizeof(ra.Occupancy) == 24
+    assert ctypes.sizeof(ra.GemmPlan) == 56
     assert ctypes.sizeof(ra.Workload) == 152
-    assert ctypes.sizeof(ra.OverlapCfg) == 4 + 20 + 8 * 4
-    assert ctypes.sizeof(ra.OverlapResult) == 24 + 52 + 4 + 8
+    assert ctypes.sizeof(ra.OverlapCfg) == 4 + 24 + 8 * 4
+    assert ctypes.sizeof(ra.OverlapResult) == 24 + 56 + 8
 
 
 KB = 1024
@@ -66,7 +66,14 @@ def test_plan_honours_reserve_and_budget(ra, shape, reserve, budget):
 
 def test_plan_depth_shrinks_with_reserve(ra):
     stages = [ra.ra_gemm_plan_query(0, 1, 8192, 8192, 8192, dict(smem_reserve_bytes=r * KB))["stages"] for r in (0, 64, 112)]
-    assert stages == sorted(stages, reverse=True) and stages[0] == 7
+    assert stages == sorted(stages, reverse=True) and stages[0] == 4          # big tiles: 4 x 48 KiB
+    p0 = ra.ra_gemm_plan_query(0, 1, 8192, 8192, 8192)
+    assert p0["m_blocks"] == 2 and p0["tile_m"] == 512 and p0["cta_group"] == 2 and p0["n_tiles"] == 512
+    p1 = ra.ra_gemm_plan_query(0, 1, 8192, 8192, 8192, dict(m_blocks=1))
+    assert p1["m_blocks"] == 1 and p1["tile_m"] == 256 and p1["stages"] == 7     # 7 x 32 KiB
+    # too little shared memory for three 48 KiB stages -> back to one block per CTA
+    p2 = ra.ra_gemm_plan_query(0, 1, 8192, 8192, 8192, dict(smem_reserve_bytes=112 * KB))
+    assert p2["m_blocks"] == 1 and p2["smem_left_per_sm"] >= 112 * KB
     mb = [ra.ra_gemm_plan_query(0, 1, 64, 16384, 16384, dict(smem_reserve_bytes=r * KB)) for r in (0, 64, 128, 200)]
     assert [p["stages"] for p in mb] == sorted((p["stages"] for p in mb), reverse=True)
     assert all(p["swap_ab"] == 1 and p["tile_m"] == 64 for p in mb)

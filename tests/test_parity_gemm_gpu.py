@@ -138,13 +138,46 @@ def test_integer_exact(ra, M, N, K):
 
 @pytest.mark.parametrize("M,N,K", [(256, 256, 64), (512, 512, 256), (1000, 520, 200), (384, 768, 4096), (2048, 2048, 512),
                                    (257, 264, 72), (4096, 1024, 1024)])
-@pytest.mark.parametrize("occ", [dict(cta_group=2), dict(cta_group=2, sm_budget=9, smem_reserve_bytes=128 * 1024),
+@pytest.mark.parametrize("occ", [dict(cta_group=2, m_blocks=1), dict(cta_group=2, m_blocks=1, sm_budget=9, smem_reserve_bytes=128 * 1024),
                                  dict(cta_group=2, tiles_per_cta=1)])
 def test_cta_pairs(ra, M, N, K, occ):
     """tcgen05 cta_group::2 path (2-CTA clusters, 256 x 256 tiles), forced on shapes the planner would not pick it for."""
     plan = ra.ra_gemm_plan_query(0, 1, M, N, K, occ)
     assert plan["cta_group"] == 2 and plan["tile_m"] == 256 and plan["grid"] % 2 == 0, plan
     check(ra, M, N, K, seed=4000 + M + N + K, occ=occ)
+
+
+@pytest.mark.parametrize("M,N,K", [(512, 256, 64), (1000, 520, 200), (2048, 2048, 512), (700, 264, 4096), (4096, 1024, 1024),
+                                   (513, 264, 72)])
+@pytest.mark.parametrize("occ", [dict(cta_group=2, m_blocks=2), dict(cta_group=2, m_blocks=2, sm_budget=10, smem_reserve_bytes=64 * 1024)])
+def test_big_tiles(ra, M, N, K, occ):
+    """m_blocks = 2: two 128-row MMA blocks per CTA share one B stage (512 x 256 tiles per CTA pair, single accumulator set)."""
+    plan = ra.ra_gemm_plan_query(0, 1, M, N, K, occ)
+    assert plan["cta_group"] == 2 and plan["m_blocks"] == 2 and plan["tile_m"] == 512 and plan["stages"] >= 3, plan
+    check(ra, M, N, K, seed=4500 + M + N + K, occ=occ)
+
+
+@pytest.mark.parametrize("transA,transB", [(0, 0), (1, 0), (1, 1)])
+def test_big_tiles_trans(ra, transA, transB):
+    check(ra, 1032, 520, 328, seed=4600 + 2 * transA + transB, occ=dict(cta_group=2, m_blocks=2), transA=transA, transB=transB)
+    check(ra, 1024, 512, 256, seed=4610 + 2 * transA + transB, alpha=-0.5, beta=2.0, occ=dict(cta_group=2, m_blocks=2),
+          transA=transA, transB=transB)
+
+
+def test_big_tiles_integer_exact_and_bit_identical(ra):
+    M, N, K = 2048, 768, 2048
+    A = ra_inputs.smallint_bf16((M, K), 43, ra_inputs.STREAM_A)
+    B = ra_inputs.smallint_bf16((N, K), 43, ra_inputs.STREAM_B)
+    _, ref16 = oracle.gemm(0, 1, M, N, K, 1.0, A, B)
+    got2, _ = run_gemm(ra, M, N, K, A, B, occ=dict(cta_group=2, m_blocks=2))
+    assert np.array_equal(got2, ref16)
+    # same per-element K order => big tiles, pair tiles and single-CTA tiles agree bit for bit (DESIGN.md A12)
+    An = ra_inputs.normal_bf16((M, K), 44, ra_inputs.STREAM_A)
+    Bn = ra_inputs.normal_bf16((N, K), 44, ra_inputs.STREAM_B)
+    c4, _ = run_gemm(ra, M, N, K, An, Bn, occ=dict(cta_group=2, m_blocks=2))
+    c2, _ = run_gemm(ra, M, N, K, An, Bn, occ=dict(cta_group=2, m_blocks=1))
+    c1, _ = run_gemm(ra, M, N, K, An, Bn, occ=dict(cta_group=1, sm_budget=24))
+    assert np.array_equal(c4, c2) and np.array_equal(c4, c1)
 
 
 def test_cta_pairs_integer_exact_and_bit_identical_to_single(ra):
