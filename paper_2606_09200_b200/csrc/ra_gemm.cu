@@ -45,6 +45,10 @@ constexpr int kEpiThreads = 128;
 constexpr int kMaxStages = 8;
 constexpr int kBarrierBytes = 256;
 constexpr int kAlignSlack = 1024;
+// epilogue staging for TMA stores: per epilogue warp two buffers of 32 rows x 64 bf16 (128-byte swizzled rows)
+constexpr int kEpiBoxCols = 64;
+constexpr int kEpiBufBytes = 32 * kEpiBoxCols * 2;          // 4 KiB
+constexpr int kEpiStageBytes = 4 * 2 * kEpiBufBytes;        // 32 KiB
 
 // bytes of one pipeline stage in ONE CTA: 128*xh rows of X + bn/cg rows of Y, 64 bf16 each
 __host__ __device__ constexpr int stage_bytes(int bn, int cg, int xh) { return (kBM * xh + bn / cg) * kBK * 2; }
@@ -63,6 +67,8 @@ struct GemmParams {
     int hintX, hintY;  // L2 policy per operand: 0 normal, 1 evict_first, 2 evict_last
     int group_x;       // rasterisation: X-tiles per group
     int xmn, ymn;      // operand storage: 0 = K-contiguous rows (K-major), 1 = row index contiguous (MN-major)
+    int epi_tma;       // 1: whole tiles leave through shared memory + TMA stores (non-swapped C only)
+    int skew;          // XH == 2: k-blocks by which X block 0 leads block 1 at both ends of a tile (<= stages)
 };
 
 // ---- device helpers ---------------------------------------------------------------------------
@@ -186,6 +192,20 @@ __device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&v)[32]) {
 __device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
 __device__ __forceinline__ void epi_bar_sync() { asm volatile("bar.sync 1, %0;" ::"n"(kEpiThreads) : "memory"); }
 
+// TMA store of one (64 cols x 32 rows) box, shared -> global, clipped at the tensor's bounds
+__device__ __forceinline__ void tma_store_2d(const CUtensorMap* map, uint32_t src_smem, int c0, int c1) {
+    asm volatile("cp.async.bulk.tensor.2d.global.shared::cta.bulk_group [%0, {%2, %3}], [%1];"
+                 ::"l"(map), "r"(src_smem), "r"(c0), "r"(c1) : "memory");
+}
+__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void bulk_wait_read() { asm volatile("cp.async.bulk.wait_group.read %0;" ::"n"(N) : "memory"); }
+__device__ __forceinline__ void bulk_wait_all() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
+__device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+__device__ __forceinline__ void st_shared_v4(uint32_t addr, uint32_t a, uint32_t b, uint32_t c, uint32_t d) {
+    asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(a), "r"(b), "r"(c), "r"(d) : "memory");
+}
+
 __device__ __forceinline__ uint64_t make_policy(int kind) {
     return kind == 1 ? policy_evict_first() : (kind == 2 ? policy_evict_last() : policy_evict_normal());
 }
@@ -298,10 +318,46 @@ __device__ __forceinline__ void store_out(const GemmParams& p, const float (&acc
     }
 }
 
+// 32 accumulator values of row x, columns y0.. -> alpha/beta -> 16 packed bf16x2 (same arithmetic as store_out)
+__device__ __forceinline__ void pack_out(const GemmParams& p, const uint32_t (&v)[32], int x, int y0, uint32_t (&o)[16]) {
+    const float alpha = p.alpha, beta = p.beta;
+    if (beta == 0.f) {
+#pragma unroll
+        for (int j = 0; j < 16; ++j) {
+            const __nv_bfloat162 r = __floats2bfloat162_rn(alpha * __uint_as_float(v[2 * j]), alpha * __uint_as_float(v[2 * j + 1]));
+            o[j] = *reinterpret_cast<const uint32_t*>(&r);
+        }
+        return;
+    }
+    const __nv_bfloat16* row = p.C + (size_t)x * p.ldc + y0;
+    uint32_t cin[16];
+    if (x < p.RX && y0 + 32 <= p.RY) {
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            const uint4 t = *reinterpret_cast<const uint4*>(row + 8 * q);
+            cin[4 * q] = t.x; cin[4 * q + 1] = t.y; cin[4 * q + 2] = t.z; cin[4 * q + 3] = t.w;
+        }
+    } else {
+#pragma unroll
+        for (int j = 0; j < 16; ++j) {
+            const uint32_t lo = (x < p.RX && y0 + 2 * j < p.RY) ? (uint32_t)__bfloat16_as_ushort(row[2 * j]) : 0u;
+            const uint32_t hi = (x < p.RX && y0 + 2 * j + 1 < p.RY) ? (uint32_t)__bfloat16_as_ushort(row[2 * j + 1]) : 0u;
+            cin[j] = lo | (hi << 16);
+        }
+    }
+#pragma unroll
+    for (int j = 0; j < 16; ++j) {
+        const float2 c = __bfloat1622float2(*reinterpret_cast<const __nv_bfloat162*>(&cin[j]));
+        const __nv_bfloat162 r = __floats2bfloat162_rn(fmaf(beta, c.x, alpha * __uint_as_float(v[2 * j])),
+                                                       fmaf(beta, c.y, alpha * __uint_as_float(v[2 * j + 1])));
+        o[j] = *reinterpret_cast<const uint32_t*>(&r);
+    }
+}
+
 template <int BN, int CG, int XH>
-__global__ void __launch_bounds__(kGemmThreads, 1)
-gemm_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constant__ CUtensorMap mapY, const GemmParams p,
-            Trace tr) {
+__global__ void __launch_bounds__(256, 2)
+gemm_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constant__ CUtensorMap mapY,
+            const __grid_constant__ CUtensorMap mapC, const GemmParams p, Trace tr) {
     // CG == 2: the CTA pair of a 2-cluster works on one 256 x BN tile.  Each CTA stages its own 128 rows of X
     // and its own BN/2 rows of Y; the leader (cluster rank 0) issues tcgen05.mma.cta_group::2, which reads both
     // CTAs' stages and writes rows [128*rank, 128*rank+128) of the accumulator into each CTA's TMEM.
@@ -327,7 +383,8 @@ gemm_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constant__ CU
     // 1024-byte alignment for the 128B swizzle; the barrier block sits after the stages.  Both CTAs of a pair
     // compute identical offsets (same kernel, same dynamic-smem base), which cta_group::2 relies on.
     const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
-    const uint32_t bar_base = smem_base + p.stages * kStageBytes;
+    const uint32_t epi_base = smem_base + p.stages * kStageBytes;     // staging for TMA stores (epi_tma only)
+    const uint32_t bar_base = epi_base + (p.epi_tma ? kEpiStageBytes : 0);
     auto full_bar = [&](int s) { return bar_base + 8u * s; };
     auto empty_bar = [&](int s) { return bar_base + 8u * (kMaxStages + s); };
     auto tfull_bar = [&](int b) { return bar_base + 8u * (2 * kMaxStages + b); };
@@ -424,41 +481,72 @@ gemm_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constant__ CU
             int acc_it = 0;
             const uint32_t idesc = kIdesc | ((uint32_t)p.xmn << 15) | ((uint32_t)p.ymn << 16);
             const int kx_step = p.xmn ? (2048 >> 4) : (32 >> 4), ky_step = p.ymn ? (2048 >> 4) : (32 >> 4);
+            // the four UMMA_K steps of X block h against the Y rows of one stage, into accumulator column acc_col
+            auto issue_block = [&](int st, int h, uint32_t acc_col, bool first) {
+                const uint32_t sx = smem_base + st * kStageBytes;
+                const uint32_t sxh = sx + h * kXHalfBytes;
+                const uint64_t dx = p.xmn ? umma_desc_sw128_mn(sxh) : umma_desc_sw128(sxh);
+                const uint64_t dy = p.ymn ? umma_desc_sw128_mn(sx + kXBytes) : umma_desc_sw128(sx + kXBytes);
+#pragma unroll
+                for (int k = 0; k < kBK / kUmmaK; ++k) {
+                    // per UMMA_K step: K-major +32 B inside the swizzle atom, MN-major +2 k-groups of 1024 B
+                    umma_bf16<CG>(tmem_base + acc_col, dx + (uint64_t)(kx_step * k), dy + (uint64_t)(ky_step * k), idesc,
+                                  (!first || k > 0) ? 1u : 0u);
+                }
+            };
+            auto wait_full = [&](int st, uint32_t ph) {
+                mbar_wait(full_bar(st), ph);               // TMA bytes (of both CTAs) have landed
+                tc_fence_after();
+            };
+            auto wait_drained = [&](int b, uint32_t ph) {
+                mbar_wait(tempty_bar(b), ph);              // every epilogue warp (of the pair) drained this accumulator
+                tc_fence_after();
+            };
             while (sched.next(sg)) {
-                // XH == 1: accumulator acc_it & 1 (double buffer).  XH == 2: block h of the tile accumulates in
-                // columns [h*BN, h*BN + BN); each block has its own "drained" barrier so block 0 of this tile can
-                // start while the epilogue is still reading block 1 of the previous one.
-                const int buf = (XH == 1) ? (acc_it & 1) : 0;
-                const uint32_t aphase = (XH == 1) ? ((acc_it >> 1) & 1) : (acc_it & 1);
                 if constexpr (XH == 1) {
-                    mbar_wait(tempty_bar(buf), aphase ^ 1u);   // every epilogue warp (of the pair) drained this accumulator
-                    tc_fence_after();
-                }
-                for (int kb = sg.kb0; kb < sg.kb1; ++kb) {
-                    mbar_wait(full_bar(stage), phase);     // TMA bytes (of both CTAs) have landed
-                    tc_fence_after();
-                    const uint32_t sx = smem_base + stage * kStageBytes;
-                    const uint64_t dy = p.ymn ? umma_desc_sw128_mn(sx + kXBytes) : umma_desc_sw128(sx + kXBytes);
-#pragma unroll
-                    for (int h = 0; h < XH; ++h) {
-                        if (XH == 2 && kb == sg.kb0) {
-                            mbar_wait(tempty_bar(h), aphase ^ 1u);
-                            tc_fence_after();
-                        }
-                        const uint32_t sxh = sx + h * kXHalfBytes;
-                        const uint64_t dx = p.xmn ? umma_desc_sw128_mn(sxh) : umma_desc_sw128(sxh);
-                        const uint32_t tmem_d = tmem_base + (uint32_t)((XH == 1 ? buf : h) * BN);
-#pragma unroll
-                        for (int k = 0; k < kBK / kUmmaK; ++k) {
-                            // per UMMA_K step: K-major +32 B inside the swizzle atom, MN-major +2 k-groups of 1024 B
-                            umma_bf16<CG>(tmem_d, dx + (uint64_t)(kx_step * k), dy + (uint64_t)(ky_step * k), idesc,
-                                          (kb > sg.kb0 || k > 0) ? 1u : 0u);
-                        }
+                    // two accumulators (acc_it & 1): the epilogue of tile i overlaps the whole main loop of tile i+1
+                    const int buf = acc_it & 1;
+                    wait_drained(buf, ((acc_it >> 1) & 1) ^ 1u);
+                    for (int kb = sg.kb0; kb < sg.kb1; ++kb) {
+                        wait_full(stage, phase);
+                        issue_block(stage, 0, (uint32_t)(buf * BN), kb == sg.kb0);
+                        umma_commit<CG>(empty_bar(stage));   // frees the smem stage (in both CTAs) when these MMAs retire
+                        if (++stage == p.stages) { stage = 0; phase ^= 1u; }
                     }
-                    umma_commit<CG>(empty_bar(stage));     // frees the smem stage (in both CTAs) when these MMAs retire
-                    if (++stage == p.stages) { stage = 0; phase ^= 1u; }
+                    umma_commit<CG>(tfull_bar(buf));         // accumulator complete (signals both CTAs' epilogues)
+                } else {
+                    // X block h accumulates in columns [h*BN, h*BN + BN); both belong to this tile, so the TMEM drain
+                    // (64 B/clk: ~2k cycles per block) cannot hide behind a second buffer.  Instead the two blocks are
+                    // skewed by D k-blocks at both ends of the tile: block 0 finishes D k-blocks early and is drained
+                    // while block 1 finishes; in the next tile block 0 starts as soon as it is drained and runs D
+                    // k-blocks ahead while block 1 is drained.  In between they run in lockstep so that a stage is
+                    // held no longer than needed (D <= stages: a stage is released by block 1).
+                    const uint32_t aph = (uint32_t)(acc_it & 1);
+                    const int nkb = sg.kb1 - sg.kb0;
+                    const int D = (p.skew > 0 && nkb >= 2 * p.skew) ? p.skew : 0;
+                    int sb = stage, ia = 0, ib = 0;          // block 1's stage cursor; k-blocks issued per block
+                    auto step_a = [&]() {
+                        wait_full(stage, phase);
+                        if (ia == 0) wait_drained(0, aph ^ 1u);
+                        issue_block(stage, 0, 0u, ia == 0);
+                        if (++stage == p.stages) { stage = 0; phase ^= 1u; }
+                        ++ia;
+                    };
+                    auto step_b = [&]() {
+                        if (ib == 0) wait_drained(1, aph ^ 1u);
+                        issue_block(sb, 1, (uint32_t)BN, ib == 0);
+                        umma_commit<CG>(empty_bar(sb));       // frees the smem stage (in both CTAs) when these MMAs retire
+                        if (++sb == p.stages) sb = 0;
+                        ++ib;
+                    };
+                    while (ia < D) step_a();                 // head: block 0 runs ahead
+                    while (ib < D) step_b();                 //       block 1 catches up
+                    while (ia < nkb - D) { step_a(); step_b(); }
+                    while (ia < nkb) step_a();               // tail: block 0 finishes first ...
+                    umma_commit<CG>(tfull_bar(0));
+                    while (ib < nkb) step_b();               //       ... and is drained while block 1 finishes
+                    umma_commit<CG>(tfull_bar(1));
                 }
-                umma_commit<CG>(tfull_bar(buf));           // accumulator(s) complete (signals both CTAs' epilogues)
                 ++acc_it;
             }
         }
@@ -470,6 +558,7 @@ gemm_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constant__ CU
         Sched sched(p, wid, nw);
         Seg sg;
         int acc_it = 0;
+        uint32_t sbuf_it = 0;                               // staging-buffer rotation (per warp)
         while (sched.next(sg)) {
             const int buf = (XH == 1) ? (acc_it & 1) : 0;
             const uint32_t aphase = (XH == 1) ? ((acc_it >> 1) & 1) : (acc_it & 1);
@@ -482,25 +571,57 @@ gemm_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constant__ CU
                 const int slot = 2 * wid + (sg.start_unit == sched.u0 ? 0 : 1);
                 part = p.partials + (size_t)slot * (kBM * BN);
             }
-            mbar_wait(tfull_bar(buf), aphase);
-            tc_fence_after();
 #pragma unroll 1
             for (int h = 0; h < XH; ++h) {
                 const int acc_idx = (XH == 1) ? buf : h;
+                mbar_wait(tfull_bar(acc_idx), aphase);
+                tc_fence_after();
                 const uint32_t taddr = tmem_base + ((uint32_t)(quarter * 32) << 16) + (uint32_t)(acc_idx * BN);
+                if (whole && p.epi_tma) {
+                    // registers -> swizzled shared memory (this warp's 32 rows x 64 columns) -> one TMA store per box;
+                    // full 128-byte lines leave the SM, the tensor map clips ragged edges.
+                    const int row0 = tx * kTileX + (int)rank * (kBM * XH) + h * kBM + quarter * 32;
 #pragma unroll 1
-                for (int c = 0; c < BN / 32; ++c) {
-                    uint32_t v[32];
-                    tmem_ld32(taddr + c * 32, v);
-                    tmem_ld_wait();
-                    float acc[32];
+                    for (int cc = 0; cc < BN / kEpiBoxCols; ++cc) {
+                        const uint32_t sbuf = epi_base + (uint32_t)((quarter * 2 + (sbuf_it & 1)) * kEpiBufBytes);
+                        ++sbuf_it;
+                        if (lane == 0) bulk_wait_read<1>();       // the store that last read this buffer has drained it
+                        __syncwarp();
+                        const int y0 = ty * BN + cc * kEpiBoxCols;
+                        const uint32_t srow = sbuf + (uint32_t)lane * 128u;
+                        const uint32_t sw = (uint32_t)(lane & 7);
 #pragma unroll
-                    for (int j = 0; j < 32; ++j) acc[j] = __uint_as_float(v[j]);
-                    if (whole) {
-                        store_out(p, acc, x + h * kBM, ty * BN + c * 32);
-                    } else {
+                        for (int hf = 0; hf < 2; ++hf) {
+                            uint32_t v[32], o[16];
+                            tmem_ld32(taddr + cc * kEpiBoxCols + hf * 32, v);
+                            tmem_ld_wait();
+                            pack_out(p, v, row0 + lane, y0 + hf * 32, o);
 #pragma unroll
-                        for (int j = 0; j < 32; ++j) __stcg(part + (size_t)(c * 32 + j) * kBM + xl, acc[j]);
+                            for (int q = 0; q < 4; ++q)
+                                st_shared_v4(srow + (((uint32_t)(q + 4 * hf) ^ sw) << 4), o[4 * q], o[4 * q + 1], o[4 * q + 2], o[4 * q + 3]);
+                        }
+                        fence_async_smem();
+                        __syncwarp();
+                        if (lane == 0) {
+                            if (row0 < p.RX && y0 < p.RY) tma_store_2d(&mapC, sbuf, y0, row0);
+                            bulk_commit();
+                        }
+                    }
+                } else {
+#pragma unroll 1
+                    for (int c = 0; c < BN / 32; ++c) {
+                        uint32_t v[32];
+                        tmem_ld32(taddr + c * 32, v);
+                        tmem_ld_wait();
+                        float acc[32];
+#pragma unroll
+                        for (int j = 0; j < 32; ++j) acc[j] = __uint_as_float(v[j]);
+                        if (whole) {
+                            store_out(p, acc, x + h * kBM, ty * BN + c * 32);
+                        } else {
+#pragma unroll
+                            for (int j = 0; j < 32; ++j) __stcg(part + (size_t)(c * 32 + j) * kBM + xl, acc[j]);
+                        }
                     }
                 }
                 // this warp's quarter of the accumulator is drained: tell the (leader's) MMA issuer
@@ -557,6 +678,8 @@ gemm_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constant__ CU
             }
         }
     }
+
+    if (warp >= 2 && lane == 0 && p.epi_tma) bulk_wait_all();   // this warp's TMA stores have left shared memory
 
     // teardown: nobody may exit (or free TMEM) while the peer can still signal its barriers / read its stages
     tc_fence_before();
@@ -625,6 +748,7 @@ static ra_status make_map(CUtensorMap* map, const void* base, int rows, int K, i
 struct Plan {
     ra_gemm_plan pub;
     int bn;
+    int epi_tma;       // whole tiles leave through the shared-memory staging area + TMA stores
     size_t counters_bytes, ws_bytes;
 };
 
@@ -676,7 +800,11 @@ static ra_status make_plan(int transA, int transB, int M, int N, int K, const ra
     // shared memory the GEMM may allocate on an SM
     long avail = (long)smem_per_sm - occ.smem_reserve_bytes - reserved;
     if (avail > optin) avail = optin;
-    const long room = avail - kAlignSlack - kBarrierBytes;
+    // non-swapped C leaves through a 32 KiB staging area + TMA stores (full-line writes); the skinny path keeps
+    // direct stores (its C is tiny) and spends the space on pipeline depth
+    // (nor does a GEMM squeezed below ~128 KiB by the reserve: there pipeline depth matters more)
+    int epi_bytes = (!swap && avail - kAlignSlack - kBarrierBytes - kEpiStageBytes >= 96 * 1024) ? kEpiStageBytes : 0;
+    long room = avail - kAlignSlack - kBarrierBytes - epi_bytes;
     auto stages_for = [&](int bn_, int cg_, int xh_) {
         int s = room > 0 ? (int)(room / stage_bytes(bn_, cg_, xh_)) : 0;
         return s > kMaxStages ? kMaxStages : s;
@@ -705,6 +833,12 @@ static ra_status make_plan(int transA, int transB, int M, int N, int K, const ra
     // was 85-88 % busy; cuBLAS's 256x256-per-CTA kernel 96 %).  Needs >= 3 stages of 48 KiB and enough tiles that
     // the coarser wave quantisation does not eat the gain.
     int xh = 1;
+    if (cg == 2 && occ.m_blocks != 1 && RX >= 4 * kBM && occ.tiles_per_cta == 0 && stages_for(256, 2, 2) < 3 &&
+        epi_bytes > 0 && room + epi_bytes >= 3 * stage_bytes(256, 2, 2)) {
+        // three 48 KiB stages fit only without the store staging: operand traffic matters more than store width
+        room += epi_bytes;
+        epi_bytes = 0;
+    }
     if (cg == 2 && occ.m_blocks != 1 && RX >= 4 * kBM && stages_for(256, 2, 2) >= 3 && occ.tiles_per_cta == 0) {
         const long long t1 = (long long)((RX + 2 * kBM - 1) / (2 * kBM)) * ((RY + bn - 1) / bn);
         const long long t2 = (long long)((RX + 4 * kBM - 1) / (4 * kBM)) * ((RY + bn - 1) / bn);
@@ -727,7 +861,7 @@ static ra_status make_plan(int transA, int transB, int M, int N, int K, const ra
         stages = 1;
         clamped = 1;
     }
-    int dyn = stages * stage_bytes(bn, cg, xh) + kAlignSlack + kBarrierBytes;
+    int dyn = stages * stage_bytes(bn, cg, xh) + kAlignSlack + kBarrierBytes + epi_bytes;
 
     const int tile_x = kBM * cg * xh;
     const int tiles_x = (RX + tile_x - 1) / tile_x, tiles_y = (RY + bn - 1) / bn;
@@ -779,6 +913,7 @@ static ra_status make_plan(int transA, int transB, int M, int N, int K, const ra
     g.cta_group = cg;
     g.m_blocks = xh;
     pl.bn = bn;
+    pl.epi_tma = epi_bytes > 0;
     if (stream_k) {
         const long long U = n_tiles * kb;
         // max number of CTA ranges one tile can span
@@ -792,11 +927,11 @@ static ra_status make_plan(int transA, int transB, int M, int N, int K, const ra
 }
 
 template <int BN, int CG, int XH>
-static ra_status launch_gemm(const CUtensorMap& mx, const CUtensorMap& my, const GemmParams& p, int grid, int dyn,
+static ra_status launch_gemm(const CUtensorMap& mx, const CUtensorMap& my, const CUtensorMap& mc, const GemmParams& p, int grid, int dyn,
                              cudaStream_t stream) {
     RA_CUDA(cudaFuncSetAttribute(gemm_kernel<BN, CG, XH>, cudaFuncAttributeMaxDynamicSharedMemorySize, dyn));
     if constexpr (CG == 1) {
-        gemm_kernel<BN, 1, XH><<<grid, kGemmThreads, dyn, stream>>>(mx, my, p, g_trace);
+        gemm_kernel<BN, 1, XH><<<grid, kGemmThreads, dyn, stream>>>(mx, my, mc, p, g_trace);
         RA_CUDA(cudaGetLastError());
         return RA_OK;
     }
@@ -812,7 +947,7 @@ static ra_status launch_gemm(const CUtensorMap& mx, const CUtensorMap& my, const
     attr[0].val.clusterDim.z = 1;
     cfg.attrs = attr;
     cfg.numAttrs = 1;
-    RA_CUDA(cudaLaunchKernelEx(&cfg, gemm_kernel<BN, CG, XH>, mx, my, p, g_trace));
+    RA_CUDA(cudaLaunchKernelEx(&cfg, gemm_kernel<BN, CG, XH>, mx, my, mc, p, g_trace));
     return RA_OK;
 }
 
@@ -898,19 +1033,23 @@ ra_status gemm_launch(int transA, int transB, int M, int N, int K, float alpha, 
     const void* X = swap ? B : A;
     const void* Y = swap ? A : B;
     const int ldx = swap ? ldb : lda, ldy = swap ? lda : ldb;
-    CUtensorMap mx, my;
+    CUtensorMap mx, my, mc;
     // op(A)(i,k): K-contiguous iff transA == 0;  op(B)(k,j): K-contiguous iff transB == 1
     const int a_mn = transA ? 1 : 0, b_mn = transB ? 0 : 1;
     p.xmn = swap ? b_mn : a_mn;
     p.ymn = swap ? a_mn : b_mn;
     RA_TRY(make_map(&mx, X, p.RX, K, ldx, kBM * xh, p.xmn));
     RA_TRY(make_map(&my, Y, p.RY, K, ldy, pl.bn / cg, p.ymn));
-    if (cg == 2 && xh == 2) return launch_gemm<256, 2, 2>(mx, my, p, pl.pub.grid, pl.pub.dyn_smem_bytes, stream);
-    if (cg == 2) return launch_gemm<256, 2, 1>(mx, my, p, pl.pub.grid, pl.pub.dyn_smem_bytes, stream);
+    p.epi_tma = pl.epi_tma;
+    p.skew = pl.pub.stages;   // measured on 8192^3 (4 stages): drain wait per tile 5.9k cycles at skew 0, 1.5k at 4
+    if (p.epi_tma) RA_TRY(make_map(&mc, C, M, N, ldc, 32, 0));    // C: box = 64 columns x 32 rows (one epilogue warp)
+    else mc = mx;                                                  // unused
+    if (cg == 2 && xh == 2) return launch_gemm<256, 2, 2>(mx, my, mc, p, pl.pub.grid, pl.pub.dyn_smem_bytes, stream);
+    if (cg == 2) return launch_gemm<256, 2, 1>(mx, my, mc, p, pl.pub.grid, pl.pub.dyn_smem_bytes, stream);
     switch (pl.bn) {
-        case 64: return launch_gemm<64, 1, 1>(mx, my, p, pl.pub.grid, pl.pub.dyn_smem_bytes, stream);
-        case 128: return launch_gemm<128, 1, 1>(mx, my, p, pl.pub.grid, pl.pub.dyn_smem_bytes, stream);
-        case 256: return launch_gemm<256, 1, 1>(mx, my, p, pl.pub.grid, pl.pub.dyn_smem_bytes, stream);
+        case 64: return launch_gemm<64, 1, 1>(mx, my, mc, p, pl.pub.grid, pl.pub.dyn_smem_bytes, stream);
+        case 128: return launch_gemm<128, 1, 1>(mx, my, mc, p, pl.pub.grid, pl.pub.dyn_smem_bytes, stream);
+        case 256: return launch_gemm<256, 1, 1>(mx, my, mc, p, pl.pub.grid, pl.pub.dyn_smem_bytes, stream);
     }
     return RA_ERR_UNSUPPORTED;
 }

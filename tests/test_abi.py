@@ -70,7 +70,7 @@ def test_plan_depth_shrinks_with_reserve(ra):
     p0 = ra.ra_gemm_plan_query(0, 1, 8192, 8192, 8192)
     assert p0["m_blocks"] == 2 and p0["tile_m"] == 512 and p0["cta_group"] == 2 and p0["n_tiles"] == 512
     p1 = ra.ra_gemm_plan_query(0, 1, 8192, 8192, 8192, dict(m_blocks=1))
-    assert p1["m_blocks"] == 1 and p1["tile_m"] == 256 and p1["stages"] == 7     # 7 x 32 KiB
+    assert p1["m_blocks"] == 1 and p1["tile_m"] == 256 and p1["stages"] == 6     # 6 x 32 KiB + 32 KiB store staging
     # too little shared memory for three 48 KiB stages -> back to one block per CTA
     p2 = ra.ra_gemm_plan_query(0, 1, 8192, 8192, 8192, dict(smem_reserve_bytes=112 * KB))
     assert p2["m_blocks"] == 1 and p2["smem_left_per_sm"] >= 112 * KB

@@ -148,7 +148,7 @@ def test_cta_pairs(ra, M, N, K, occ):
 
 
 @pytest.mark.parametrize("M,N,K", [(512, 256, 64), (1000, 520, 200), (2048, 2048, 512), (700, 264, 4096), (4096, 1024, 1024),
-                                   (513, 264, 72)])
+                                   (513, 264, 72), (1024, 512, 448), (520, 256, 8192)])   # K: skew on/off, empty middle
 @pytest.mark.parametrize("occ", [dict(cta_group=2, m_blocks=2), dict(cta_group=2, m_blocks=2, sm_budget=10, smem_reserve_bytes=64 * 1024)])
 def test_big_tiles(ra, M, N, K, occ):
     """m_blocks = 2: two 128-row MMA blocks per CTA share one B stage (512 x 256 tiles per CTA pair, single accumulator set)."""
