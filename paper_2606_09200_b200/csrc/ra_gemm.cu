@@ -103,6 +103,24 @@ __device__ __forceinline__ void mbar_arrive_cluster(uint32_t bar_cluster) {
 template <int CG>
 __device__ __forceinline__ void tma_load_2d(uint32_t dst_smem, const CUtensorMap* map, int c0, int c1, uint32_t bar,
                                             uint64_t policy) {
+    if (policy == 0) {
+        // no cache hint: the default L2 behaviour (a createpolicy evict_normal hint is NOT the same thing -- ncu
+        // shows such lines as "evict_normal_demote" and 2.4x the cross-die L2 fabric traffic)
+        if constexpr (CG == 1) {
+            asm volatile(
+                "cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes"
+                " [%0], [%1, {%3, %4}], [%2];"
+                ::"r"(dst_smem), "l"(map), "r"(bar), "r"(c0), "r"(c1)
+                : "memory");
+        } else {
+            asm volatile(
+                "cp.async.bulk.tensor.2d.cta_group::2.shared::cluster.global.tile.mbarrier::complete_tx::bytes"
+                " [%0], [%1, {%3, %4}], [%2];"
+                ::"r"(dst_smem), "l"(map), "r"(bar), "r"(c0), "r"(c1)
+                : "memory");
+        }
+        return;
+    }
     if constexpr (CG == 1) {
         asm volatile(
             "cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes.L2::cache_hint"
@@ -207,7 +225,7 @@ __device__ __forceinline__ void st_shared_v4(uint32_t addr, uint32_t a, uint32_t
 }
 
 __device__ __forceinline__ uint64_t make_policy(int kind) {
-    return kind == 1 ? policy_evict_first() : (kind == 2 ? policy_evict_last() : policy_evict_normal());
+    return kind == 1 ? policy_evict_first() : (kind == 2 ? policy_evict_last() : 0ull);   // 0 = no hint
 }
 
 // ---- static schedule: every role walks the same sequence of (tile, kb0, kb1) segments ----------
