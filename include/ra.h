@@ -216,6 +216,39 @@ typedef struct {
 /* Runs n_iters iterations under `cfg`, synchronises, fills `res` (host pointers all). */
 ra_status ra_overlap_run(const ra_workload* w, const ra_overlap_cfg* cfg, ra_overlap_result* res);
 
+/* ---------------------------------------------------------------------------------------------
+ * The same step from HOST buffers (the end-to-end entry point).  One step = copy this step's inputs
+ * host -> device, run the n_iters iterations of ra_overlap_run under `cfg`, copy the results device ->
+ * host.  The library software-pipelines consecutive steps on its own copy streams:
+ *     H2D(step s+1)  ||  compute(step s)  ||  D2H(step s-1)
+ * over the device buffer sets dev0 / dev1 (dev1 may be NULL: one set, copies and compute of
+ * consecutive steps then serialise).  Every step reads the same host inputs and overwrites the same
+ * host outputs (a serving loop would rotate them).
+ *
+ * ra_host_io   HOST pointers; pinned memory is needed for the copies to overlap (pageable memory is
+ *              legal but makes cudaMemcpyAsync synchronous).  Sizes follow dev0:
+ *   A, B       the GEMM operands exactly as ra_gemm takes them: rows x ld bf16 (rows = M or K by transA, ...)
+ *   C          out, M x ldc bf16 (may be NULL: not copied back)
+ *   ar_in      P host pointers of ar_count floats (the rank buffers before the step)
+ *   ar_out     ar_count floats: rank 0's buffer after the step's n_iters allreduces (may be NULL)
+ *   a2a_in     P*P*chunk_bytes, goes to a2a_a;  a2a_out: the buffer the last iteration wrote (may be NULL)
+ * dev0, dev1   workloads of identical shape with disjoint DEVICE buffers (caller-owned, as in ra_overlap_run).
+ * res          total_ms = GPU time from the first copy to the last, over all n_steps (events on the copy streams).
+ * Synchronous.  RA_ERR_INVALID_ARG for a NULL required pointer, n_steps < 1 or mismatched sets.
+ * --------------------------------------------------------------------------------------------- */
+typedef struct {
+    const void* A;
+    const void* B;
+    void* C;
+    const float* const* ar_in;
+    float* ar_out;
+    const void* a2a_in;
+    void* a2a_out;
+} ra_host_io;
+
+ra_status ra_overlap_run_host(const ra_workload* dev0, const ra_workload* dev1, const ra_host_io* io,
+                              const ra_overlap_cfg* cfg, int n_steps, ra_overlap_result* res);
+
 /* Runs cfgs[0..n) `runs` times each, interleaved round-robin so that clock drift hits all settings
  * alike; the first runs/3 passes are warm-up and the mean of the rest is stored in results[i].total_ms
  * ("the first one-third of runs are considered warm-up").  *best = argmin over

@@ -28,7 +28,7 @@ EXPORTS = (
     "ra_status_str", "ra_last_cuda_error", "ra_shutdown", "ra_device_info", "ra_gemm_plan_query",
     "ra_gemm_workspace_bytes", "ra_gemm", "ra_allreduce_emul", "ra_allreduce_emul_ex", "ra_alltoall_emul",
     "ra_alltoall_emul_ex",
-    "ra_overlap_run", "ra_overlap_sweep", "ra_set_trace",
+    "ra_overlap_run", "ra_overlap_run_host", "ra_overlap_sweep", "ra_set_trace",
 )
 
 
@@ -67,6 +67,11 @@ class OverlapCfg(Structure):
                 ("prio_comm", c_int32), ("dependent", c_int32), ("record_kernel_times", c_int32)]
 
 
+class HostIO(Structure):
+    _fields_ = [("A", c_void_p), ("B", c_void_p), ("C", c_void_p), ("ar_in", POINTER(c_void_p)), ("ar_out", c_void_p),
+                ("a2a_in", c_void_p), ("a2a_out", c_void_p)]
+
+
 class OverlapResult(Structure):
     _fields_ = [("total_ms", c_float), ("median_ms", c_float), ("min_ms", c_float), ("gemm_ms_sum", c_float),
                 ("coll_ms_sum", c_float), ("overlap_rate", c_float), ("plan", GemmPlan),
@@ -101,6 +106,8 @@ def _L():
     lib.ra_alltoall_emul.argtypes = [c_void_p, c_void_p, c_int, c_size_t, c_int, c_void_p]
     lib.ra_alltoall_emul_ex.argtypes = [c_void_p, c_void_p, c_int, c_size_t, c_int, c_int, c_int, c_int, c_void_p]
     lib.ra_overlap_run.argtypes = [POINTER(Workload), POINTER(OverlapCfg), POINTER(OverlapResult)]
+    lib.ra_overlap_run_host.argtypes = [POINTER(Workload), POINTER(Workload), POINTER(HostIO), POINTER(OverlapCfg), c_int,
+                                        POINTER(OverlapResult)]
     lib.ra_overlap_sweep.argtypes = [POINTER(Workload), POINTER(OverlapCfg), c_int, c_int, POINTER(OverlapResult),
                                      POINTER(c_int)]
     lib.ra_set_trace.argtypes = [c_void_p, c_size_t]
@@ -132,7 +139,9 @@ def _ptr(x) -> int | None:
         return None
     if isinstance(x, int):
         return x
-    return int(x.data_ptr())
+    if hasattr(x, "data_ptr"):
+        return int(x.data_ptr())
+    return int(x.ctypes.data)          # numpy array (host buffers of ra_overlap_run_host)
 
 
 def _stream(stream) -> int | None:
@@ -289,6 +298,27 @@ def ra_overlap_run(workload: Workload, cfg: OverlapCfg) -> dict:
         res.kernel_times = ctypes.cast(times, POINTER(c_float))
     _check(_L().ra_overlap_run(byref(workload), byref(cfg), byref(res)), "ra_overlap_run")
     return _result_dict(res, workload.n_iters, times)
+
+
+def make_host_io(*, A=None, B=None, C=None, ar_in=None, ar_out=None, a2a_in=None, a2a_out=None):
+    """Marshal the HOST buffers of one step (pinned torch CPU tensors or numpy arrays).  Returns (HostIO, keepalive)."""
+    io = HostIO()
+    keep = [A, B, C, ar_in, ar_out, a2a_in, a2a_out]
+    io.A, io.B, io.C = _ptr(A), _ptr(B), _ptr(C)
+    if ar_in is not None:
+        arr = _ptr_array(ar_in)
+        keep.append(arr)
+        io.ar_in = ctypes.cast(arr, POINTER(c_void_p))
+    io.ar_out, io.a2a_in, io.a2a_out = _ptr(ar_out), _ptr(a2a_in), _ptr(a2a_out)
+    return io, keep
+
+
+def ra_overlap_run_host(dev0: Workload, dev1, io: HostIO, cfg: OverlapCfg, n_steps: int = 1) -> dict:
+    """n_steps steps from host buffers, copies pipelined against compute over the device sets dev0 / dev1 (or None)."""
+    res = OverlapResult()
+    _check(_L().ra_overlap_run_host(byref(dev0), byref(dev1) if dev1 is not None else None, byref(io), byref(cfg),
+                                    int(n_steps), byref(res)), "ra_overlap_run_host")
+    return _result_dict(res, dev0.n_iters, None)
 
 
 def ra_overlap_sweep(workload: Workload, cfgs, runs: int = 30):

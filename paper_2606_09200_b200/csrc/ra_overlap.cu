@@ -72,40 +72,20 @@ static ra_status launch_coll(const ra_workload* w, const ra_overlap_cfg* cfg, in
     return RA_OK;
 }
 
-static ra_status run_once(const ra_workload* w, const ra_overlap_cfg* cfg, ra_overlap_result* res) {
-    std::lock_guard<std::mutex> lk(g_cache.mu);
+// Enqueues the n_iters iterations of one step on (s_comp, s_comm); on return s_comp is ordered after everything.
+// Caller holds g_cache.mu.  rec_base: first timed-event slot for per-kernel events (rec only).
+static ra_status enqueue_step(const ra_workload* w, const ra_overlap_cfg* cfg, cudaStream_t s_comp, cudaStream_t s_comm,
+                              bool rec, ra_gemm_plan* plan) {
     const int n = w->n_iters;
     const bool has_gemm = w->M > 0 && w->N > 0;
     const bool has_coll = w->kind != RA_COLL_NONE;
     const bool overlap = cfg->mode == RA_MODE_OVERLAP;
-    const bool rec = cfg->record_kernel_times != 0;
-
-    DeviceInfo di;
-    RA_TRY(device_info(&di));
-    RA_TRY(require_sm100(di));
-    if (cfg->prio_compute > di.prio_least || cfg->prio_compute < di.prio_greatest || cfg->prio_comm > di.prio_least ||
-        cfg->prio_comm < di.prio_greatest)
-        return RA_ERR_INVALID_ARG;
-
-    cudaStream_t s_comp, s_comm;
-    RA_TRY(get_stream(0, cfg->prio_compute, &s_comp));
-    if (overlap) RA_TRY(get_stream(1, cfg->prio_comm, &s_comm));
-    else s_comm = s_comp;
-
-    RA_TRY(ensure_events(g_cache.dep_events, (size_t)n + 2, cudaEventDisableTiming));
-    RA_TRY(ensure_events(g_cache.timed_events, 2 + (rec ? 4 * (size_t)n : 0), cudaEventDefault));
-    cudaEvent_t ev_start = g_cache.timed_events[0], ev_end = g_cache.timed_events[1];
     auto kev = [&](int i, int which) { return g_cache.timed_events[2 + 4 * (size_t)i + which]; };
-    cudaEvent_t ev_comm_done = g_cache.dep_events[n];
-
-    ra_gemm_plan plan{};
-    RA_CUDA(cudaEventRecord(ev_start, s_comp));
-    if (overlap) RA_CUDA(cudaStreamWaitEvent(s_comm, ev_start, 0));
     for (int i = 0; i < n; ++i) {
         if (has_gemm) {
             if (rec) RA_CUDA(cudaEventRecord(kev(i, 0), s_comp));
             RA_TRY(gemm_launch(w->transA, w->transB, w->M, w->N, w->K, w->alpha, w->A, w->lda, w->B, w->ldb, w->beta,
-                               w->C, w->ldc, &cfg->occ, w->workspace, w->workspace_bytes, s_comp, &plan));
+                               w->C, w->ldc, &cfg->occ, w->workspace, w->workspace_bytes, s_comp, plan));
             if (rec) RA_CUDA(cudaEventRecord(kev(i, 1), s_comp));
         }
         if (has_coll) {
@@ -119,9 +99,46 @@ static ra_status run_once(const ra_workload* w, const ra_overlap_cfg* cfg, ra_ov
         }
     }
     if (overlap) {
-        RA_CUDA(cudaEventRecord(ev_comm_done, s_comm));
-        RA_CUDA(cudaStreamWaitEvent(s_comp, ev_comm_done, 0));
+        RA_CUDA(cudaEventRecord(g_cache.dep_events[n], s_comm));
+        RA_CUDA(cudaStreamWaitEvent(s_comp, g_cache.dep_events[n], 0));
     }
+    return RA_OK;
+}
+
+static ra_status check_priorities(const ra_overlap_cfg* cfg) {
+    DeviceInfo di;
+    RA_TRY(device_info(&di));
+    RA_TRY(require_sm100(di));
+    if (cfg->prio_compute > di.prio_least || cfg->prio_compute < di.prio_greatest || cfg->prio_comm > di.prio_least ||
+        cfg->prio_comm < di.prio_greatest)
+        return RA_ERR_INVALID_ARG;
+    return RA_OK;
+}
+
+static ra_status run_once(const ra_workload* w, const ra_overlap_cfg* cfg, ra_overlap_result* res) {
+    std::lock_guard<std::mutex> lk(g_cache.mu);
+    const int n = w->n_iters;
+    const bool has_gemm = w->M > 0 && w->N > 0;
+    const bool has_coll = w->kind != RA_COLL_NONE;
+    const bool overlap = cfg->mode == RA_MODE_OVERLAP;
+    const bool rec = cfg->record_kernel_times != 0;
+
+    RA_TRY(check_priorities(cfg));
+
+    cudaStream_t s_comp, s_comm;
+    RA_TRY(get_stream(0, cfg->prio_compute, &s_comp));
+    if (overlap) RA_TRY(get_stream(1, cfg->prio_comm, &s_comm));
+    else s_comm = s_comp;
+
+    RA_TRY(ensure_events(g_cache.dep_events, (size_t)n + 2, cudaEventDisableTiming));
+    RA_TRY(ensure_events(g_cache.timed_events, 2 + (rec ? 4 * (size_t)n : 0), cudaEventDefault));
+    cudaEvent_t ev_start = g_cache.timed_events[0], ev_end = g_cache.timed_events[1];
+    auto kev = [&](int i, int which) { return g_cache.timed_events[2 + 4 * (size_t)i + which]; };
+
+    ra_gemm_plan plan{};
+    RA_CUDA(cudaEventRecord(ev_start, s_comp));
+    if (overlap) RA_CUDA(cudaStreamWaitEvent(s_comm, ev_start, 0));
+    RA_TRY(enqueue_step(w, cfg, s_comp, s_comm, rec, &plan));
     RA_CUDA(cudaEventRecord(ev_end, s_comp));
     RA_CUDA(cudaEventSynchronize(ev_end));
     RA_CUDA(cudaGetLastError());
@@ -164,9 +181,105 @@ static ra_status run_once(const ra_workload* w, const ra_overlap_cfg* cfg, ra_ov
     return RA_OK;
 }
 
+// ---- host-buffer pipeline: H2D(step s+1)  ||  compute(step s)  ||  D2H(step s-1) ---------------------------
+static size_t a_bytes(const ra_workload* w) { return (size_t)(w->transA ? w->K : w->M) * (size_t)w->lda * 2; }
+static size_t b_bytes(const ra_workload* w) { return (size_t)(w->transB ? w->N : w->K) * (size_t)w->ldb * 2; }
+static size_t c_bytes(const ra_workload* w) { return (size_t)w->M * (size_t)w->ldc * 2; }
+
+static bool same_shape(const ra_workload* a, const ra_workload* b) {
+    return a->transA == b->transA && a->transB == b->transB && a->M == b->M && a->N == b->N && a->K == b->K &&
+           a->lda == b->lda && a->ldb == b->ldb && a->ldc == b->ldc && a->kind == b->kind && a->P == b->P &&
+           a->ar_count == b->ar_count && a->chunk_bytes == b->chunk_bytes && a->n_iters == b->n_iters;
+}
+
+static ra_status run_host(const ra_workload* const* dev, int n_sets, const ra_host_io* io, const ra_overlap_cfg* cfg,
+                          int n_steps, ra_overlap_result* res) {
+    std::lock_guard<std::mutex> lk(g_cache.mu);
+    const ra_workload* w0 = dev[0];
+    const int n = w0->n_iters;
+    const bool has_gemm = w0->M > 0 && w0->N > 0;
+    const bool overlap = cfg->mode == RA_MODE_OVERLAP;
+    RA_TRY(check_priorities(cfg));
+
+    cudaStream_t s_comp, s_comm, s_h2d, s_d2h;
+    RA_TRY(get_stream(0, cfg->prio_compute, &s_comp));
+    if (overlap) RA_TRY(get_stream(1, cfg->prio_comm, &s_comm));
+    else s_comm = s_comp;
+    RA_TRY(get_stream(2, 0, &s_h2d));
+    RA_TRY(get_stream(3, 0, &s_d2h));
+    // dep events: [0, n] per-iteration + join (enqueue_step), then 3 per buffer set
+    RA_TRY(ensure_events(g_cache.dep_events, (size_t)n + 2 + 3 * (size_t)n_sets, cudaEventDisableTiming));
+    RA_TRY(ensure_events(g_cache.timed_events, 2, cudaEventDefault));
+    cudaEvent_t ev_start = g_cache.timed_events[0], ev_end = g_cache.timed_events[1];
+    auto set_ev = [&](int k, int which) { return g_cache.dep_events[(size_t)n + 2 + 3 * (size_t)k + which]; };   // 0 h2d, 1 compute, 2 d2h
+
+    ra_gemm_plan plan{};
+    RA_CUDA(cudaEventRecord(ev_start, s_h2d));
+    for (int s = 0; s < n_steps; ++s) {
+        const int k = s % n_sets;
+        const ra_workload* w = dev[k];
+        // the set is free once the D2H of the step that last used it has finished
+        if (s >= n_sets) RA_CUDA(cudaStreamWaitEvent(s_h2d, set_ev(k, 2), 0));
+        if (has_gemm) {
+            RA_CUDA(cudaMemcpyAsync(const_cast<void*>(w->A), io->A, a_bytes(w), cudaMemcpyHostToDevice, s_h2d));
+            RA_CUDA(cudaMemcpyAsync(const_cast<void*>(w->B), io->B, b_bytes(w), cudaMemcpyHostToDevice, s_h2d));
+        }
+        if (w->kind == RA_COLL_ALLREDUCE) {
+            for (int r = 0; r < w->P; ++r)
+                RA_CUDA(cudaMemcpyAsync(w->ar_bufs[r], io->ar_in[r], w->ar_count * sizeof(float), cudaMemcpyHostToDevice, s_h2d));
+        } else if (w->kind == RA_COLL_ALLTOALL) {
+            RA_CUDA(cudaMemcpyAsync(w->a2a_a, io->a2a_in, (size_t)w->P * w->P * w->chunk_bytes, cudaMemcpyHostToDevice, s_h2d));
+        }
+        RA_CUDA(cudaEventRecord(set_ev(k, 0), s_h2d));
+        RA_CUDA(cudaStreamWaitEvent(s_comp, set_ev(k, 0), 0));
+        if (overlap) RA_CUDA(cudaStreamWaitEvent(s_comm, set_ev(k, 0), 0));
+        RA_TRY(enqueue_step(w, cfg, s_comp, s_comm, false, &plan));
+        RA_CUDA(cudaEventRecord(set_ev(k, 1), s_comp));
+        RA_CUDA(cudaStreamWaitEvent(s_d2h, set_ev(k, 1), 0));
+        if (has_gemm && io->C) RA_CUDA(cudaMemcpyAsync(io->C, w->C, c_bytes(w), cudaMemcpyDeviceToHost, s_d2h));
+        if (w->kind == RA_COLL_ALLREDUCE && io->ar_out) {
+            RA_CUDA(cudaMemcpyAsync(io->ar_out, w->ar_bufs[0], w->ar_count * sizeof(float), cudaMemcpyDeviceToHost, s_d2h));
+        } else if (w->kind == RA_COLL_ALLTOALL && io->a2a_out) {
+            const void* last = (n & 1) ? w->a2a_b : w->a2a_a;     // iteration n-1 wrote here
+            RA_CUDA(cudaMemcpyAsync(io->a2a_out, last, (size_t)w->P * w->P * w->chunk_bytes, cudaMemcpyDeviceToHost, s_d2h));
+        }
+        RA_CUDA(cudaEventRecord(set_ev(k, 2), s_d2h));
+    }
+    RA_CUDA(cudaEventRecord(ev_end, s_d2h));
+    RA_CUDA(cudaEventSynchronize(ev_end));
+    RA_CUDA(cudaGetLastError());
+    float total = 0.f;
+    RA_CUDA(cudaEventElapsedTime(&total, ev_start, ev_end));
+    res->total_ms = res->median_ms = res->min_ms = total;
+    res->plan = plan;
+    res->gemm_ms_sum = res->coll_ms_sum = 0.f;
+    res->overlap_rate = 0.f;
+    return RA_OK;
+}
+
 }  // namespace ra
 
 extern "C" {
+
+ra_status ra_overlap_run_host(const ra_workload* dev0, const ra_workload* dev1, const ra_host_io* io,
+                              const ra_overlap_cfg* cfg, int n_steps, ra_overlap_result* res) {
+    RA_TRY(ra::validate(dev0, cfg, res));
+    if (io == nullptr || n_steps < 1) return RA_ERR_INVALID_ARG;
+    if (dev1 != nullptr) {
+        RA_TRY(ra::validate(dev1, cfg, res));
+        if (!ra::same_shape(dev0, dev1)) return RA_ERR_INVALID_ARG;
+    }
+    const bool has_gemm = dev0->M > 0 && dev0->N > 0;
+    if (has_gemm && (io->A == nullptr || io->B == nullptr)) return RA_ERR_INVALID_ARG;
+    if (dev0->kind == RA_COLL_ALLREDUCE) {
+        if (io->ar_in == nullptr) return RA_ERR_INVALID_ARG;
+        for (int r = 0; r < dev0->P; ++r)
+            if (io->ar_in[r] == nullptr) return RA_ERR_INVALID_ARG;
+    }
+    if (dev0->kind == RA_COLL_ALLTOALL && io->a2a_in == nullptr) return RA_ERR_INVALID_ARG;
+    const ra_workload* sets[2] = {dev0, dev1};
+    return ra::run_host(sets, dev1 ? 2 : 1, io, cfg, n_steps, res);
+}
 
 ra_status ra_overlap_run(const ra_workload* w, const ra_overlap_cfg* cfg, ra_overlap_result* res) {
     RA_TRY(ra::validate(w, cfg, res));

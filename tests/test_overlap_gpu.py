@@ -156,3 +156,84 @@ def test_trace_records_residency(ra):
     assert len(gemm_sms) == 64 and len(set(gemm_sms)) == 64          # one persistent GEMM CTA per SM
     assert smid.max() < ra.ra_device_info()["sm_count"]
     assert np.all(rec[:, 3] >= rec[:, 2])
+
+
+# ---- ra_overlap_run_host: the same step from HOST buffers, copies pipelined against compute -------------------------
+def _pinned(a):
+    import torch
+    return torch.from_numpy(a.view(np.int16) if a.dtype == np.uint16 else a).pin_memory()
+
+
+@pytest.mark.parametrize("two_sets", [False, True])
+@pytest.mark.parametrize("n_steps", [1, 3])
+def test_host_pipeline_allreduce(ra, two_sets, n_steps):
+    import torch
+    cfg0 = ra_inputs.CONFIGS[0]
+    M, N, K = cfg0.M, cfg0.N, cfg0.K
+    A = ra_inputs.normal_bf16((M, K), cfg0.seed, ra_inputs.STREAM_A)
+    B = ra_inputs.normal_bf16((N, K), cfg0.seed, ra_inputs.STREAM_B)
+    bufs = ra_inputs.allreduce_buffers(cfg0)
+    ref, _ = oracle.gemm(0, 1, M, N, K, 1.0, A, B)
+    rowA, colB = oracle.gemm_norms(0, 1, M, N, K, A, B)
+    ref_bufs = [b.copy() for b in bufs]
+    oracle.overlap_replay(cfg0.n_iters, ar_bufs=ref_bufs)           # every step starts from the same host inputs
+
+    def dev_set():
+        g = dict(M=M, N=N, K=K, A=torch.zeros((M, K), dtype=torch.int16, device="cuda"),
+                 B=torch.zeros((N, K), dtype=torch.int16, device="cuda"),
+                 C=torch.full((M, N), 0x7FC0, dtype=torch.int16, device="cuda"),
+                 workspace=torch.empty(max(ra.ra_gemm_workspace_bytes(0, 1, M, N, K), 16), dtype=torch.uint8, device="cuda"))
+        ar = [torch.zeros(cfg0.ar_count, dtype=torch.float32, device="cuda") for _ in range(cfg0.P)]
+        return ra.make_workload(gemm=g, allreduce=ar, n_iters=cfg0.n_iters), (g, ar)
+
+    (w0, k0), t0 = dev_set()
+    (w1, k1), t1 = dev_set() if two_sets else ((None, None), None)
+    hA, hB = _pinned(A), _pinned(B)
+    hC = torch.full((M, N), 0x7FC0, dtype=torch.int16).pin_memory()
+    h_in = [_pinned(b) for b in bufs]
+    h_out = torch.zeros(cfg0.ar_count, dtype=torch.float32).pin_memory()
+    io, keep = ra.make_host_io(A=hA, B=hB, C=hC, ar_in=h_in, ar_out=h_out)
+    res = ra.ra_overlap_run_host(w0, w1, io, ra.make_cfg(mode=1, prio_comm=ra.ra_device_info()["prio_greatest"]), n_steps)
+    assert res["total_ms"] > 0
+    err = gemm_norm_err(hC.numpy().view(np.uint16), ref, rowA, colB)
+    assert err <= GEMM_TOL, err
+    assert h_out.numpy().tobytes() == ref_bufs[0].tobytes()
+    assert all(np.array_equal(t.numpy(), b) for t, b in zip(h_in, bufs)), "host inputs were modified"
+
+
+@pytest.mark.parametrize("n_iters", [1, 2])
+def test_host_pipeline_alltoall(ra, n_iters):
+    import torch
+    P, chunk = 4, 48 * 1024 + 16
+    send = ra_inputs.tagged_chunks(P, chunk)
+    want = send if n_iters % 2 == 0 else oracle.alltoall(send, P, chunk)      # applied twice = identity
+
+    def dev_set():
+        a = torch.zeros(send.size, dtype=torch.int64, device="cuda")
+        b = torch.zeros_like(a)
+        return ra.make_workload(alltoall=dict(a=a, b=b, P=P, chunk_bytes=chunk), n_iters=n_iters), (a, b)
+
+    (w0, k0), t0 = dev_set()
+    (w1, k1), t1 = dev_set()
+    h_in = torch.from_numpy(send.view(np.int64)).pin_memory()
+    h_out = torch.zeros_like(h_in).pin_memory()
+    io, keep = ra.make_host_io(a2a_in=h_in, a2a_out=h_out)
+    ra.ra_overlap_run_host(w0, w1, io, ra.make_cfg(mode=1), 3)
+    assert h_out.numpy().tobytes() == want.tobytes()
+
+
+def test_host_pipeline_errors(ra):
+    import torch
+    a = torch.zeros(64, dtype=torch.int64, device="cuda")
+    w, keep = ra.make_workload(alltoall=dict(a=a, b=torch.zeros_like(a), P=2, chunk_bytes=128), n_iters=1)
+    io, k = ra.make_host_io()                                                  # a2a_in missing
+    with pytest.raises(ra.RaError) as e:
+        ra.ra_overlap_run_host(w, None, io, ra.make_cfg(mode=1), 1)
+    assert e.value.status == ra.RA_ERR_INVALID_ARG
+    h = torch.zeros(64, dtype=torch.int64).pin_memory()
+    io, k = ra.make_host_io(a2a_in=h)
+    with pytest.raises(ra.RaError):
+        ra.ra_overlap_run_host(w, None, io, ra.make_cfg(mode=1), 0)            # n_steps < 1
+    w2, keep2 = ra.make_workload(alltoall=dict(a=a, b=torch.zeros_like(a), P=2, chunk_bytes=64), n_iters=1)
+    with pytest.raises(ra.RaError):
+        ra.ra_overlap_run_host(w, w2, io, ra.make_cfg(mode=1), 1)              # mismatched sets
