@@ -1,0 +1,115 @@
+"""GPU parity at BASELINE.json's FULL sizes (configs 1-4), in the launch configuration bench.py times.
+
+The step runs through ra_overlap_run (overlap mode, priority pair, the planner's default occupancy = what the sweep
+picks on cb-*, plus the mb-* winner) exactly as the bench does.  Collectives are compared in full, bit for bit
+(the oracle does 1 GiB in milliseconds); the 8192^3 GEMM on sampled outputs the oracle computes one by one
+(every tile of the 512 x 256 / 256 x 256 grids contributes: tile corners, tile-edge rows/columns and random
+interior points); the 64 x 16384 x 16384 GEMM in full.  Also checks that NaN is gone from every C entry
+(the buffer starts NaN-filled), i.e. every tile was written.
+"""
+import numpy as np
+import pytest
+
+import oracle
+import ra_inputs
+from helpers import GEMM_TOL, bf16_bits_to_f64, gemm_norm_err, to_dev, to_host
+
+pytestmark = pytest.mark.gpu
+
+N_ITERS = 2          # even: the alltoall ping-pong returns to `a`; the in-place allreduce is replayed twice
+
+
+@pytest.fixture(scope="module")
+def ra():
+    import paper_2606_09200_b200 as m
+    return m
+
+
+def _sample_points(M, N, rng, n_random=6000):
+    """Tile corners / edges of every 128-row x 64-column block boundary family plus random interior points."""
+    ii, jj = [], []
+    rows = sorted({r for b in range(0, M, 128) for r in (b, b + 127) if r < M} | {0, M - 1})
+    cols = sorted({c for b in range(0, N, 64) for c in (b, b + 63) if c < N} | {0, N - 1})
+    # every boundary row against a few random columns, every boundary column against a few random rows
+    for r in rows:
+        for c in rng.integers(0, N, 4):
+            ii.append(r), jj.append(int(c))
+    for c in cols:
+        for r in rng.integers(0, M, 4):
+            ii.append(int(r)), jj.append(c)
+    ii += list(rng.integers(0, M, n_random))
+    jj += list(rng.integers(0, N, n_random))
+    return np.asarray(ii, dtype=np.int64), np.asarray(jj, dtype=np.int64)
+
+
+def _settings(ra, cfg):
+    hi = ra.ra_device_info()["prio_greatest"]
+    out = [dict(mode=1, prio_compute=0, prio_comm=hi)]                                   # planner default + priority on
+    if cfg.M <= 64:
+        out.append(dict(mode=1, prio_comm=hi, occ=dict(smem_reserve_bytes=64 * 1024, sm_budget=148)))   # mb-ar winner
+        out.append(dict(mode=1, occ=dict(sm_budget=128)))                                # mb-a2a winner
+    else:
+        out.append(dict(mode=1, occ=dict(smem_reserve_bytes=64 * 1024, sm_budget=128), coll_sm_budget=20))
+    return out
+
+
+@pytest.mark.parametrize("index", [1, 2, 3, 4])
+def test_full_size_config(ra, index):
+    import torch
+    cfg = ra_inputs.CONFIGS[index]
+    M, N, K = cfg.M, cfg.N, cfg.K
+    A, B = ra_inputs.gemm_operands(cfg)
+    rowA, colB = oracle.gemm_norms(0, 1, M, N, K, A, B)
+    rng = np.random.default_rng(cfg.seed)
+    if M * N <= 1 << 21:
+        ref_full, _ = oracle.gemm(0, 1, M, N, K, 1.0, A, B)
+        ii = jj = None
+    else:
+        ii, jj = _sample_points(M, N, rng)
+        ref_s = oracle.gemm_samples(0, 1, M, N, K, 1.0, A, B, ii, jj)
+    dA, dB = to_dev(A), to_dev(B)
+    if cfg.coll == "allreduce":
+        bufs = ra_inputs.allreduce_buffers(cfg)
+        ref_bufs = [b.copy() for b in bufs]
+        oracle.overlap_replay(N_ITERS, ar_bufs=ref_bufs)
+    else:
+        send = ra_inputs.alltoall_payload(cfg)
+        ref_b = oracle.alltoall(send, cfg.P, cfg.chunk_bytes)          # after iteration 0: b = transpose(a)
+        assert oracle.alltoall(ref_b, cfg.P, cfg.chunk_bytes).tobytes() == send.tobytes()   # iteration 1 restores a
+
+    for kw in _settings(ra, cfg):
+        dC = torch.full((M, N), 0x7FC0, dtype=torch.int16, device="cuda")                # NaN-filled
+        occ = kw.get("occ")
+        ws = torch.empty(max(ra.ra_gemm_workspace_bytes(0, 1, M, N, K, occ), 16), dtype=torch.uint8, device="cuda")
+        g = dict(M=M, N=N, K=K, A=dA, B=dB, C=dC, workspace=ws)
+        if cfg.coll == "allreduce":
+            dev = [to_dev(b) for b in bufs]
+            w, keep = ra.make_workload(gemm=g, allreduce=dev, n_iters=N_ITERS)
+        else:
+            da = to_dev(send)
+            db = torch.zeros_like(da)
+            w, keep = ra.make_workload(gemm=g, alltoall=dict(a=da, b=db, P=cfg.P, chunk_bytes=cfg.chunk_bytes),
+                                       n_iters=N_ITERS)
+        res = ra.ra_overlap_run(w, ra.make_cfg(**kw))
+        torch.cuda.synchronize()
+        plan = res["plan"]
+
+        got = to_host(dC, np.uint16).reshape(M, N)
+        assert np.all(np.isfinite(bf16_bits_to_f64(got))), f"unwritten / non-finite C entries, plan {plan}"
+        if ii is None:
+            err = gemm_norm_err(got, ref_full, rowA, colB)
+        else:
+            gs = bf16_bits_to_f64(got[ii, jj])
+            err = float(np.max(np.abs(gs - ref_s) / (rowA[ii] * colB[jj] + 1e-30)))
+        assert err <= GEMM_TOL, (err, plan)
+
+        if cfg.coll == "allreduce":
+            for r, (dd, rr) in enumerate(zip(dev, ref_bufs)):
+                assert to_host(dd, np.float32).tobytes() == rr.tobytes(), f"allreduce rank {r} not bit-exact ({kw})"
+            del dev
+        else:
+            assert to_host(db, np.uint64).tobytes() == ref_b.tobytes(), f"alltoall b not bit-exact ({kw})"
+            assert to_host(da, np.uint64).tobytes() == send.tobytes(), f"alltoall a not restored ({kw})"
+            del da, db
+        del dC, w
+        torch.cuda.empty_cache()
