@@ -154,6 +154,13 @@ CONFIGS = (
     Config(2, "mb-ar", 64, 16384, 16384, "allreduce", 8, ar_count=16 * MiB),
     Config(3, "cb-a2a", 8192, 8192, 8192, "alltoall", 8, chunk_bytes=8 * MiB),
     Config(4, "mb-a2a", 64, 16384, 16384, "alltoall", 8, chunk_bytes=8 * MiB),
+    # The paper's literal Table 1 workloads: 4 GPUs, 896 MB collectives.  896 MiB is
+    # exactly the bf16 output of the 8192 x 57344 GEMM, read here as the PER-RANK message: allreduce over P = 4 rank
+    # buffers of 896 MiB (fp32 elements), alltoall with 4 chunks of 224 MiB per rank.
+    Config(5, "paper-cb-ar", 8192, 8192, 8192, "allreduce", 4, ar_count=224 * MiB, n_iters=10),
+    Config(6, "paper-mb-ar", 8192, 57344, 8192, "allreduce", 4, ar_count=224 * MiB, n_iters=10),
+    Config(7, "paper-cb-a2a", 8192, 8192, 8192, "alltoall", 4, chunk_bytes=224 * MiB, n_iters=10),
+    Config(8, "paper-mb-a2a", 8192, 57344, 8192, "alltoall", 4, chunk_bytes=224 * MiB, n_iters=10),
 )
 
 

@@ -81,3 +81,14 @@ def test_config_table_matches_baseline_json():
     assert c[4].coll == "alltoall" and (c[4].M, c[4].N, c[4].K) == (64, 16384, 16384)
     assert c[1].coll_bytes == 1 << 30 and c[3].coll_bytes == 1 << 30
     assert c[2].gemm_bytes == 2 * (64 * 16384 + 16384 * 16384 + 64 * 16384)
+
+
+def test_paper_literal_configs():
+    """PAPER.md:84-92 (Table 1): GEMM 8192^3 / 8192 x 57344 x 8192, collectives of 896 MB on 4 GPUs."""
+    c = {x.name: x for x in gen.CONFIGS}
+    for name in ("paper-cb-ar", "paper-mb-ar", "paper-cb-a2a", "paper-mb-a2a"):
+        assert c[name].P == 4
+    assert (c["paper-mb-ar"].M, c["paper-mb-ar"].N, c["paper-mb-ar"].K) == (8192, 57344, 8192)
+    assert c["paper-mb-ar"].ar_count * 4 == 896 << 20 == 8192 * 57344 * 2        # the GEMM's bf16 output
+    assert c["paper-mb-a2a"].chunk_bytes * 4 == 896 << 20
+    assert c["paper-cb-ar"].coll_bytes == 2 * 4 * (896 << 20)
