@@ -201,6 +201,10 @@ typedef struct {
     int32_t prio_compute, prio_comm; /* cudaStreamCreateWithPriority values; equal = "priority off" */
     int32_t dependent;          /* 1: K_c^i waits for K_g^i (the paper's schedule); 0: free-running streams */
     int32_t record_kernel_times;/* 1: per-kernel event pairs (perturbs the schedule slightly) */
+    int32_t use_graph;          /* 1: capture the n_iters schedule (both streams, all dependencies) into a CUDA graph
+                                   once per (workload, setting) and replay it with one launch -- for launch-bound
+                                   steps.  Ignored when record_kernel_times = 1.  Graphs are cached until ra_shutdown;
+                                   the caller's buffers must stay valid while they are cached. */
 } ra_overlap_cfg;
 
 typedef struct {

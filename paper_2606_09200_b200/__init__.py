@@ -64,7 +64,7 @@ class Workload(Structure):
 class OverlapCfg(Structure):
     _fields_ = [("mode", c_int32), ("occ", Occupancy), ("coll_sm_budget", c_int32), ("coll_smem_bytes", c_int32),
                 ("coll_ctas_per_sm", c_int32), ("coll_variant", c_int32), ("prio_compute", c_int32),
-                ("prio_comm", c_int32), ("dependent", c_int32), ("record_kernel_times", c_int32)]
+                ("prio_comm", c_int32), ("dependent", c_int32), ("record_kernel_times", c_int32), ("use_graph", c_int32)]
 
 
 class HostIO(Structure):
@@ -271,7 +271,7 @@ def make_workload(*, gemm=None, allreduce=None, alltoall=None, n_iters=1):
 
 
 def make_cfg(mode=RA_MODE_OVERLAP, occ=None, coll_sm_budget=0, coll_smem_bytes=0, coll_ctas_per_sm=0, coll_variant=0,
-             prio_compute=0, prio_comm=0, dependent=1, record_kernel_times=0) -> OverlapCfg:
+             prio_compute=0, prio_comm=0, dependent=1, record_kernel_times=0, use_graph=0) -> OverlapCfg:
     c = OverlapCfg()
     c.mode = int(mode)
     c.occ = _occ(occ) or Occupancy(0, 0, 0, 1, 0)
@@ -279,6 +279,7 @@ def make_cfg(mode=RA_MODE_OVERLAP, occ=None, coll_sm_budget=0, coll_smem_bytes=0
     c.coll_ctas_per_sm, c.coll_variant = int(coll_ctas_per_sm), int(coll_variant)
     c.prio_compute, c.prio_comm = int(prio_compute), int(prio_comm)
     c.dependent, c.record_kernel_times = int(dependent), int(record_kernel_times)
+    c.use_graph = int(use_graph)
     return c
 
 

@@ -6,7 +6,9 @@
 // section 3.3): the communication stream is created with the higher priority.  Serial baseline
 // (Fig. 1a): everything on one stream.  Metrics.
 #include <algorithm>
+#include <cstring>
 #include <map>
+#include <string>
 #include <mutex>
 #include <vector>
 
@@ -27,6 +29,7 @@ struct Cache {
     std::map<std::pair<int, int>, cudaStream_t> streams;   // (role, priority) -> stream
     std::vector<cudaEvent_t> dep_events;                   // no timing
     std::vector<cudaEvent_t> timed_events;                 // timing
+    std::map<std::string, cudaGraphExec_t> graphs;         // (workload, cfg, trace) bytes -> instantiated step graph
 };
 static Cache g_cache;
 
@@ -136,9 +139,56 @@ static ra_status run_once(const ra_workload* w, const ra_overlap_cfg* cfg, ra_ov
     auto kev = [&](int i, int which) { return g_cache.timed_events[2 + 4 * (size_t)i + which]; };
 
     ra_gemm_plan plan{};
+    cudaGraphExec_t gexec = nullptr;
+    if (cfg->use_graph && !rec) {
+        // One CUDA graph per (workload, setting): the whole n_iters schedule -- both streams, the K_g^i -> K_c^i
+        // dependencies, stream-K memsets, copy-engine nodes -- is captured once and replayed with a single launch,
+        // which takes the host out of launch-bound steps (Tiny: ~8 kernels of a few microseconds each).
+        ra_overlap_cfg kc = *cfg;
+        kc.record_kernel_times = 0;
+        std::string key(reinterpret_cast<const char*>(w), sizeof(*w));
+        key.append(reinterpret_cast<const char*>(&kc), sizeof(kc));
+        key.append(reinterpret_cast<const char*>(&g_trace), sizeof(g_trace));
+        if (w->kind == RA_COLL_ALLREDUCE) key.append(reinterpret_cast<const char*>(w->ar_bufs), sizeof(float*) * (size_t)w->P);
+        auto it = g_cache.graphs.find(key);
+        if (it != g_cache.graphs.end()) {
+            gexec = it->second;
+            // the plan is a pure function of (shape, knobs): recompute it for the result
+            if (has_gemm) RA_TRY(ra_gemm_plan_query(w->transA, w->transB, w->M, w->N, w->K, &cfg->occ, &plan));
+        } else {
+            cudaGraph_t graph = nullptr;
+            RA_CUDA(cudaStreamBeginCapture(s_comp, cudaStreamCaptureModeRelaxed));
+            ra_status st = RA_OK;
+            if (overlap) {
+                cudaError_t e = cudaEventRecord(g_cache.dep_events[n + 1], s_comp);      // fork: s_comm joins the capture
+                if (e == cudaSuccess) e = cudaStreamWaitEvent(s_comm, g_cache.dep_events[n + 1], 0);
+                if (e != cudaSuccess) st = cuda_fail(e);
+            }
+            if (st == RA_OK) st = enqueue_step(w, cfg, s_comp, s_comm, false, &plan);
+            const cudaError_t ec = cudaStreamEndCapture(s_comp, &graph);                 // always end the capture
+            if (st != RA_OK) {
+                if (graph) cudaGraphDestroy(graph);
+                (void)cudaGetLastError();
+                return st;
+            }
+            RA_CUDA(ec);
+            const cudaError_t ei = cudaGraphInstantiate(&gexec, graph, 0);
+            cudaGraphDestroy(graph);
+            RA_CUDA(ei);
+            if (g_cache.graphs.size() >= 64) {                                           // bounded cache
+                for (auto& kv : g_cache.graphs) cudaGraphExecDestroy(kv.second);
+                g_cache.graphs.clear();
+            }
+            g_cache.graphs[key] = gexec;
+        }
+    }
     RA_CUDA(cudaEventRecord(ev_start, s_comp));
-    if (overlap) RA_CUDA(cudaStreamWaitEvent(s_comm, ev_start, 0));
-    RA_TRY(enqueue_step(w, cfg, s_comp, s_comm, rec, &plan));
+    if (gexec) {
+        RA_CUDA(cudaGraphLaunch(gexec, s_comp));
+    } else {
+        if (overlap) RA_CUDA(cudaStreamWaitEvent(s_comm, ev_start, 0));
+        RA_TRY(enqueue_step(w, cfg, s_comp, s_comm, rec, &plan));
+    }
     RA_CUDA(cudaEventRecord(ev_end, s_comp));
     RA_CUDA(cudaEventSynchronize(ev_end));
     RA_CUDA(cudaGetLastError());
@@ -329,6 +379,8 @@ void ra_shutdown(void) {
     std::lock_guard<std::mutex> lk(ra::g_cache.mu);
     for (auto& kv : ra::g_cache.streams) cudaStreamDestroy(kv.second);
     ra::g_cache.streams.clear();
+    for (auto& kv : ra::g_cache.graphs) cudaGraphExecDestroy(kv.second);
+    ra::g_cache.graphs.clear();
     for (cudaEvent_t e : ra::g_cache.dep_events) cudaEventDestroy(e);
     for (cudaEvent_t e : ra::g_cache.timed_events) cudaEventDestroy(e);
     ra::g_cache.dep_events.clear();

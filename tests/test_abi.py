@@ -41,7 +41,7 @@ def test_struct_layouts_match_header(ra):
     assert ctypes.sizeof(ra.Occupancy) == 24
     assert ctypes.sizeof(ra.GemmPlan) == 56
     assert ctypes.sizeof(ra.Workload) == 152
-    assert ctypes.sizeof(ra.OverlapCfg) == 4 + 24 + 8 * 4
+    assert ctypes.sizeof(ra.OverlapCfg) == 4 + 24 + 9 * 4
     assert ctypes.sizeof(ra.OverlapResult) == 24 + 56 + 8
     assert ctypes.sizeof(ra.HostIO) == 7 * 8
 

@@ -40,6 +40,11 @@ MODES = [
     dict(mode=1, prio_compute=0, prio_comm=-5, occ=dict(sm_budget=74, smem_reserve_bytes=96 * 1024), coll_sm_budget=74),
     dict(mode=1, prio_compute=0, prio_comm=-5, occ=dict(tiles_per_cta=1), record_kernel_times=1),
     dict(mode=1, dependent=0, occ=dict(sm_budget=37)),
+    # the same schedules captured into a CUDA graph (one launch per step)
+    dict(mode=0, use_graph=1),
+    dict(mode=1, prio_compute=0, prio_comm=-5, use_graph=1),
+    dict(mode=1, dependent=0, occ=dict(sm_budget=37), use_graph=1),
+    dict(mode=1, coll_variant=2, use_graph=1),                               # copy-engine alltoall = memcpy nodes
 ]
 
 
@@ -237,3 +242,34 @@ def test_host_pipeline_errors(ra):
     w2, keep2 = ra.make_workload(alltoall=dict(a=a, b=torch.zeros_like(a), P=2, chunk_bytes=64), n_iters=1)
     with pytest.raises(ra.RaError):
         ra.ra_overlap_run_host(w, w2, io, ra.make_cfg(mode=1), 1)              # mismatched sets
+
+
+def test_graph_replay_matches_oracle_and_streams(ra):
+    """use_graph: first call captures + runs, later calls replay the cached graph; the in-place allreduce and the
+    stream-K GEMM (memset node + workspace) must behave exactly as the stream schedule does."""
+    import torch
+    M, N, K = 300, 200, 8192                       # stream-K plan (workspace, counter memset)
+    A, B, g, dC = _gemm_side(ra, M, N, K, 123)
+    assert ra.ra_gemm_plan_query(0, 1, M, N, K)["split_k"] > 1
+    bufs = [ra_inputs.uniform_f32(100003, 123, ra_inputs.STREAM_AR + r) for r in range(3)]
+    n_iters, calls = 3, 3
+    ref_bufs = [b.copy() for b in bufs]
+    oracle.overlap_replay(n_iters * calls, ar_bufs=ref_bufs)
+    dev = [to_dev(b) for b in bufs]
+    w, keep = ra.make_workload(gemm=g, allreduce=dev, n_iters=n_iters)
+    cfg = ra.make_cfg(mode=1, prio_comm=ra.ra_device_info()["prio_greatest"], use_graph=1)
+    outs = []
+    for _ in range(calls):
+        dC.fill_(0x7FC0)
+        res = ra.ra_overlap_run(w, cfg)
+        assert res["plan"]["split_k"] > 1 and res["total_ms"] > 0
+        outs.append(to_host(dC, np.uint16).copy())
+    for d, r in zip(dev, ref_bufs):
+        assert to_host(d, np.float32).tobytes() == r.tobytes()
+    dC.fill_(0x7FC0)
+    ra.ra_overlap_run(w, ra.make_cfg(mode=1))      # plain streams
+    plain = to_host(dC, np.uint16)
+    assert all(np.array_equal(o, plain) for o in outs)
+    ref, _ = oracle.gemm(0, 1, M, N, K, 1.0, A, B)
+    rowA, colB = oracle.gemm_norms(0, 1, M, N, K, A, B)
+    assert gemm_norm_err(plain.reshape(M, N), ref, rowA, colB) <= GEMM_TOL
