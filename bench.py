@@ -392,7 +392,9 @@ def run_ours(args, cfg):
         ra.ra_overlap_run(w, ra.make_cfg(mode=1))
     reset_collective(cfg, d, h)
     cands = [] if args.sweep == "none" else sweep_candidates(ra, cfg, quick=(args.sweep == "quick"))
-    cand_kws = [dict(mode=0)] + [dict(mode=1)] + cands
+    # S7': the model-based policy's pick runs inside the same sweep so that its regret is measured, not assumed
+    sug = ra.ra_overlap_suggest(w, peaks["bf16_tflops_sustained"], peaks["hbm_gbs"])
+    cand_kws = [dict(mode=0)] + [dict(mode=1)] + [sug["kw"]] + cands
     results, best = ra.ra_overlap_sweep(w, [ra.make_cfg(**kw) for kw in cand_kws], runs=args.sweep_runs)
     reset_collective(cfg, d, h)
     best_kw = cand_kws[best]
@@ -409,6 +411,10 @@ def run_ours(args, cfg):
             on, off = (results[best]["total_ms"], r["total_ms"]) if lab["priority"] == "on" else (r["total_ms"], results[best]["total_ms"])
             norm_time = on / off
 
+    policy = {"setting": cfg_label(sug["kw"]), "predicted_ms_per_iter": sug["t_overlap_ms"], "measured_ms_per_iter": results[2]["total_ms"] / n_iters,
+              "sweep_best_ms_per_iter": results[best]["total_ms"] / n_iters,
+              "regret": results[2]["total_ms"] / results[best]["total_ms"] - 1.0, "gemm_bound": sug["gemm_bound"],
+              "model_roofline_ms": sug["t_roofline_ms"], "settings_in_sweep": len(cand_kws) - 1}
     alone = kernels_alone(ra, cfg, d, h, peaks, n_iters)
     residency = residency_map(ra, w, best_kw, ra.ra_device_info()["sm_count"])
     reset_collective(cfg, d, h)
@@ -504,7 +510,7 @@ def run_ours(args, cfg):
         "gemm_in_step_ms": gemm_in_step_ms, "coll_in_step_ms": statistics.mean(c_ms),
         "alone": alone, "combined_roofline_ms": {"burst": comb["bf16_tflops"], "sustained": comb["bf16_tflops_sustained"]},
         "overlap_vs_roofline": {"burst": over_ms / comb["bf16_tflops"], "sustained": over_ms / comb["bf16_tflops_sustained"]},
-        "peaks": peaks, "roofline": roof, "cpu_baseline": cpu,
+        "peaks": peaks, "roofline": roof, "cpu_baseline": cpu, "policy": policy,
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                 "api": "ra_overlap_run_host (pinned host buffers; H2D, compute and D2H of consecutive steps pipelined over two device sets)",
                 "gpu_ms_per_step": e2e_res["total_ms"] / args.steps},

@@ -253,6 +253,30 @@ typedef struct {
 ra_status ra_overlap_run_host(const ra_workload* dev0, const ra_workload* dev1, const ra_host_io* io,
                               const ra_overlap_cfg* cfg, int n_steps, ra_overlap_result* res);
 
+/* ---------------------------------------------------------------------------------------------
+ * S7'  Knob policy from a roofline model (automating the knob selection is the
+ * paper's future work).  Host only, runs nothing: predicts the setting the exhaustive sweep would pick
+ * from the two kernels' flops / bytes and the chip's tensor and HBM peaks (csrc/ra_policy.cu states the
+ * model).  `peaks` NULL or zero fields = built-in B200 figures (1400 TFLOP/s sustained bf16, 6450 GB/s).
+ * Times are per pipelined iteration, in ms.  bench.py runs the suggestion inside the sweep and reports
+ * its regret against the sweep's best.
+ * --------------------------------------------------------------------------------------------- */
+typedef struct {
+    double tensor_tflops;       /* dense bf16 peak to model against (sustained) */
+    double hbm_gbs;             /* HBM bandwidth to model against */
+} ra_peaks;
+
+typedef struct {
+    ra_overlap_cfg cfg;         /* the suggested setting (mode = RA_MODE_OVERLAP) */
+    int32_t gemm_bound;         /* 0: the GEMM alone is tensor-bound, 1: HBM-bound */
+    double t_gemm_ms, t_coll_ms;/* each kernel alone at its roofline */
+    double t_overlap_ms;        /* predicted per-iteration time of the n_iters pipeline (head and tail included) */
+    double t_serial_ms;         /* t_gemm_ms + t_coll_ms */
+    double t_roofline_ms;       /* max(flops / tensor peak, (gemm + collective bytes) / HBM peak) */
+} ra_suggestion;
+
+ra_status ra_overlap_suggest(const ra_workload* w, const ra_peaks* peaks, ra_suggestion* out);
+
 /* Runs cfgs[0..n) `runs` times each, interleaved round-robin so that clock drift hits all settings
  * alike; the first runs/3 passes are warm-up and the mean of the rest is stored in results[i].total_ms
  * ("the first one-third of runs are considered warm-up").  *best = argmin over

@@ -12,7 +12,7 @@ from __future__ import annotations
 
 import ctypes
 import os
-from ctypes import POINTER, Structure, byref, c_char_p, c_float, c_int, c_int32, c_size_t, c_uint64, c_void_p
+from ctypes import POINTER, Structure, byref, c_char_p, c_double, c_float, c_int, c_int32, c_size_t, c_uint64, c_void_p
 
 from . import build as _build
 
@@ -28,7 +28,7 @@ EXPORTS = (
     "ra_status_str", "ra_last_cuda_error", "ra_shutdown", "ra_device_info", "ra_gemm_plan_query",
     "ra_gemm_workspace_bytes", "ra_gemm", "ra_allreduce_emul", "ra_allreduce_emul_ex", "ra_alltoall_emul",
     "ra_alltoall_emul_ex",
-    "ra_overlap_run", "ra_overlap_run_host", "ra_overlap_sweep", "ra_set_trace",
+    "ra_overlap_run", "ra_overlap_run_host", "ra_overlap_suggest", "ra_overlap_sweep", "ra_set_trace",
 )
 
 
@@ -72,6 +72,15 @@ class HostIO(Structure):
                 ("a2a_in", c_void_p), ("a2a_out", c_void_p)]
 
 
+class Peaks(Structure):
+    _fields_ = [("tensor_tflops", c_double), ("hbm_gbs", c_double)]
+
+
+class Suggestion(Structure):
+    _fields_ = [("cfg", OverlapCfg), ("gemm_bound", c_int32), ("t_gemm_ms", c_double), ("t_coll_ms", c_double),
+                ("t_overlap_ms", c_double), ("t_serial_ms", c_double), ("t_roofline_ms", c_double)]
+
+
 class OverlapResult(Structure):
     _fields_ = [("total_ms", c_float), ("median_ms", c_float), ("min_ms", c_float), ("gemm_ms_sum", c_float),
                 ("coll_ms_sum", c_float), ("overlap_rate", c_float), ("plan", GemmPlan),
@@ -108,6 +117,7 @@ def _L():
     lib.ra_overlap_run.argtypes = [POINTER(Workload), POINTER(OverlapCfg), POINTER(OverlapResult)]
     lib.ra_overlap_run_host.argtypes = [POINTER(Workload), POINTER(Workload), POINTER(HostIO), POINTER(OverlapCfg), c_int,
                                         POINTER(OverlapResult)]
+    lib.ra_overlap_suggest.argtypes = [POINTER(Workload), POINTER(Peaks), POINTER(Suggestion)]
     lib.ra_overlap_sweep.argtypes = [POINTER(Workload), POINTER(OverlapCfg), c_int, c_int, POINTER(OverlapResult),
                                      POINTER(c_int)]
     lib.ra_set_trace.argtypes = [c_void_p, c_size_t]
@@ -320,6 +330,20 @@ def ra_overlap_run_host(dev0: Workload, dev1, io: HostIO, cfg: OverlapCfg, n_ste
     _check(_L().ra_overlap_run_host(byref(dev0), byref(dev1) if dev1 is not None else None, byref(io), byref(cfg),
                                     int(n_steps), byref(res)), "ra_overlap_run_host")
     return _result_dict(res, dev0.n_iters, None)
+
+
+def ra_overlap_suggest(workload: Workload, tensor_tflops: float = 0.0, hbm_gbs: float = 0.0) -> dict:
+    """Model-based knob policy (host only).  Returns {"cfg": OverlapCfg, "kw": make_cfg keywords, predictions...}."""
+    s = Suggestion()
+    pk = Peaks(float(tensor_tflops), float(hbm_gbs))
+    _check(_L().ra_overlap_suggest(byref(workload), byref(pk), byref(s)), "ra_overlap_suggest")
+    c = s.cfg
+    kw = dict(mode=c.mode, occ=dict(smem_reserve_bytes=c.occ.smem_reserve_bytes, sm_budget=c.occ.sm_budget,
+                                    tiles_per_cta=c.occ.tiles_per_cta, cta_group=c.occ.cta_group, m_blocks=c.occ.m_blocks),
+              coll_sm_budget=c.coll_sm_budget, coll_smem_bytes=c.coll_smem_bytes, coll_ctas_per_sm=c.coll_ctas_per_sm,
+              coll_variant=c.coll_variant, prio_compute=c.prio_compute, prio_comm=c.prio_comm, dependent=c.dependent)
+    return {"kw": kw, "gemm_bound": "hbm" if s.gemm_bound else "tensor", "t_gemm_ms": s.t_gemm_ms, "t_coll_ms": s.t_coll_ms,
+            "t_overlap_ms": s.t_overlap_ms, "t_serial_ms": s.t_serial_ms, "t_roofline_ms": s.t_roofline_ms}
 
 
 def ra_overlap_sweep(workload: Workload, cfgs, runs: int = 30):

@@ -150,3 +150,76 @@ def test_product_never_imports_oracle():
         if f.endswith((".py", ".c")):
             txt = open(os.path.join(ROOT, "oracle", f)).read()
             assert "import paper_2606_09200_b200" not in txt and "ra.h" not in txt
+
+
+# ---- S7': the model-based knob policy is host-only, so its logic is tested here ---------------------------------------
+class _FakeBuf:
+    def __init__(self, n):
+        self.n = n
+
+    def numel(self):
+        return self.n
+
+    def data_ptr(self):
+        return 16
+
+
+def _workload(ra, M, N, K, coll, P, count=0, chunk=0, n_iters=20):
+    g = dict(M=M, N=N, K=K, A=16, B=16, C=16)
+    if coll == "allreduce":
+        return ra.make_workload(gemm=g, allreduce=[_FakeBuf(count) for _ in range(P)], n_iters=n_iters)
+    return ra.make_workload(gemm=g, alltoall=dict(a=16, b=32, P=P, chunk_bytes=chunk), n_iters=n_iters)
+
+
+def test_policy_rooflines_and_choices(ra):
+    T, H = 1400.0, 6450.0
+    # compute-bound GEMM + allreduce: tensor roofline, all SMs, no reserve, priority off
+    w, keep = _workload(ra, 8192, 8192, 8192, "allreduce", 8, count=16 << 20)
+    s = ra.ra_overlap_suggest(w, T, H)
+    flops, gb, cb = 2.0 * 8192 ** 3, 2.0 * 3 * 8192 ** 2, 2.0 * 4 * 8 * (16 << 20)
+    eff = 512 / (7 * 74)                                      # 512 big tiles on 74 CTA pairs: 7 waves
+    assert s["gemm_bound"] == "tensor"
+    assert abs(s["t_gemm_ms"] - flops / (T * 1e9 * eff)) < 1e-9
+    assert abs(s["t_coll_ms"] - cb / (H * 1e6)) < 1e-9
+    assert abs(s["t_roofline_ms"] - max(s["t_gemm_ms"], (gb + cb) / (H * 1e6))) < 1e-9
+    assert abs(s["t_serial_ms"] - (s["t_gemm_ms"] + s["t_coll_ms"])) < 1e-12
+    assert s["t_gemm_ms"] <= s["t_overlap_ms"] <= s["t_serial_ms"]
+    kw = s["kw"]
+    assert kw["occ"]["sm_budget"] == 0 and kw["occ"]["smem_reserve_bytes"] == 0 and kw["prio_comm"] == kw["prio_compute"]
+    # the same GEMM fills shared memory, so the alltoall must be the shared-memory-free variant
+    w, keep = _workload(ra, 8192, 8192, 8192, "alltoall", 8, chunk=8 << 20)
+    assert ra.ra_overlap_suggest(w, T, H)["kw"]["coll_variant"] == 1
+    # skinny GEMM: HBM-bound, leaves 20 SMs free -> TMA-ring alltoall; overlap cannot beat total bytes / bandwidth
+    w, keep = _workload(ra, 64, 16384, 16384, "alltoall", 8, chunk=8 << 20)
+    s = ra.ra_overlap_suggest(w, T, H)
+    gb = 2.0 * (64 * 16384 + 16384 * 16384 + 64 * 16384)
+    assert s["gemm_bound"] == "hbm" and s["kw"]["coll_variant"] == 0
+    assert abs(s["t_roofline_ms"] - (gb + float(1 << 30)) / (H * 1e6)) < 1e-9
+    assert abs(s["t_overlap_ms"] - s["t_serial_ms"]) < 1e-9     # bytes-bound on both sides: nothing to hide
+    # one pipelined iteration has no partner for either kernel: the prediction is the serial time
+    w, keep = _workload(ra, 8192, 8192, 8192, "allreduce", 8, count=16 << 20, n_iters=1)
+    s = ra.ra_overlap_suggest(w, T, H)
+    assert abs(s["t_overlap_ms"] - s["t_serial_ms"]) < 1e-9
+
+
+def test_policy_budget_follows_wave_quantisation(ra):
+    # 4096 x 4608: 8 x 18 = 144 big tiles -> 72 pairs run them in 2 full waves (eff 1.0), 74 pairs need 2 waves at 97 %:
+    # the model must not pick a budget that quantises worse than all SMs, and must pick an even count
+    w, keep = _workload(ra, 4096, 4608, 8192, "allreduce", 8, count=1 << 20)
+    s = ra.ra_overlap_suggest(w)
+    b = s["kw"]["occ"]["sm_budget"]
+    assert b % 2 == 0 and (b == 0 or 74 <= b <= 148)
+    p_all = ra.ra_gemm_plan_query(0, 1, 4096, 4608, 8192)
+    p_pick = ra.ra_gemm_plan_query(0, 1, 4096, 4608, 8192, dict(sm_budget=b))
+
+    def t(p):
+        workers = p["grid"] // p["cta_group"]
+        waves = -(-p["n_tiles"] // workers)
+        return 1.0 / ((p["grid"] / 148) * (p["n_tiles"] / (waves * workers)))
+    assert t(p_pick) <= t(p_all) * 1.0001
+
+
+def test_policy_errors(ra):
+    import ctypes
+    lib = ctypes.CDLL(ra.lib_path())
+    assert lib.ra_overlap_suggest(None, None, None) == ra.RA_ERR_INVALID_ARG
