@@ -603,9 +603,26 @@ gemm_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constant__ CU
                     for (int cc = 0; cc < BN / kEpiBoxCols; ++cc) {
                         const uint32_t sbuf = epi_base + (uint32_t)((quarter * 2 + (sbuf_it & 1)) * kEpiBufBytes);
                         ++sbuf_it;
+                        const int y0 = ty * BN + cc * kEpiBoxCols;
+                        if (y0 + kEpiBoxCols > p.RY && (p.RY & 7)) {
+                            // TMA stores clip at 16-byte granularity: with N % 8 != 0 the box holding the ragged edge
+                            // would overwrite up to 7 pad elements after column N-1 (found by the guard-band test), so
+                            // that one box per row of tiles goes out through predicated element stores instead.
+#pragma unroll 1
+                            for (int hf = 0; hf < 2; ++hf) {
+                                uint32_t v[32];
+                                tmem_ld32(taddr + cc * kEpiBoxCols + hf * 32, v);
+                                tmem_ld_wait();
+                                float acc[32];
+#pragma unroll
+                                for (int j = 0; j < 32; ++j) acc[j] = __uint_as_float(v[j]);
+                                store_out(p, acc, row0 + lane, y0 + hf * 32);
+                            }
+                            --sbuf_it;      // no staging buffer was used: keep the two-deep rotation intact
+                            continue;
+                        }
                         if (lane == 0) bulk_wait_read<1>();       // the store that last read this buffer has drained it
                         __syncwarp();
-                        const int y0 = ty * BN + cc * kEpiBoxCols;
                         const uint32_t srow = sbuf + (uint32_t)lane * 128u;
                         const uint32_t sw = (uint32_t)(lane & 7);
 #pragma unroll
