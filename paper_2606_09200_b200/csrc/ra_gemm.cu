@@ -825,7 +825,9 @@ static ra_status make_plan(int transA, int transB, int M, int N, int K, const ra
         clamped = 1;
     }
 
-    const int swap = (M <= 64 && N >= 128) ? 1 : 0;
+    // skinny M (weight streaming): the long weight dimension becomes the 128-row X side, the M tokens the Y side
+    // (BN = 64 or 128), so N/128 independent tiles stream the weights without any K split.
+    const int swap = ((M <= 64 && N >= 128) || (M <= 128 && N >= 1024)) ? 1 : 0;
     const int RX = swap ? N : M, RY = swap ? M : N;
     int bn = RY > 128 ? 256 : (RY > 64 ? 128 : 64);
     const int kb = (K + kBK - 1) / kBK;
@@ -853,10 +855,10 @@ static ra_status make_plan(int transA, int transB, int M, int N, int K, const ra
     // 128 + 256, i.e. 1/3 less L2->SM traffic per flop.  Used for the data-parallel schedule on large problems.
     int cg = 1;
     if (occ.cta_group != 1 && !swap && bn == 256 && RX >= 256 && budget >= 2 && stages_for(256, 2, 1) >= 2) {
-        const long long t2 = (long long)((RX + 2 * kBM - 1) / (2 * kBM)) * ((RY + bn - 1) / bn);
-        // measured on B200: pairs at 86 % wave efficiency (4096^3) still beat single-CTA stream-K by 28 %
-        const bool sk_wanted = occ.tiles_per_cta == 0 && kb >= 8 && wave_eff(t2, budget / 2) < 0.7;
-        if (!sk_wanted || occ.cta_group == 2) cg = 2;
+        // measured on B200: pair tiles beat single-CTA stream-K even at low wave efficiency (1024^3: 13 vs 27 us at
+        // 22 %, 3000x1000x2048: 19 vs 37 us at 65 %, 256x8192x8192: 54 vs 73 us at 43 %) -- half the L2->SM traffic
+        // per flop and no partial-tile round trip -- so pairs are taken whenever the shape allows them.
+        cg = 2;
     }
     if (occ.cta_group == 2 && cg != 2) {
         if (!occ.allow_clamp) return RA_ERR_INFEASIBLE_KNOB;

@@ -42,18 +42,15 @@ ra_status ra_overlap_suggest(const ra_workload* w, const ra_peaks* peaks, ra_sug
     const double hbm = (peaks && peaks->hbm_gbs > 0) ? peaks->hbm_gbs : ra::kDefaultHbmGbs;
 
     int sm_count = ra::kDefaultSmCount;
-    int prio_greatest = 0;
     {
         ra::DeviceInfo di;
         if (ra::device_info(&di) == RA_OK) {
             sm_count = di.sm_count;
-            prio_greatest = di.prio_greatest;
         } else {
             ra::g_last_cuda_error = 0;
             (void)cudaGetLastError();
         }
     }
-    (void)prio_greatest;
 
     const bool has_gemm = w->M > 0 && w->N > 0;
     const double M = w->M, N = w->N, K = w->K;
