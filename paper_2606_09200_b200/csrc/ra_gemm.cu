@@ -870,13 +870,13 @@ static ra_status make_plan(int transA, int transB, int M, int N, int K, const ra
     // was 85-88 % busy; cuBLAS's 256x256-per-CTA kernel 96 %).  Needs >= 3 stages of 48 KiB and enough tiles that
     // the coarser wave quantisation does not eat the gain.
     int xh = 1;
-    if (cg == 2 && occ.m_blocks != 1 && RX >= 4 * kBM && occ.tiles_per_cta == 0 && stages_for(256, 2, 2) < 3 &&
+    if (cg == 2 && occ.m_blocks != 1 && RX >= 4 * kBM && stages_for(256, 2, 2) < 3 &&
         epi_bytes > 0 && room + epi_bytes >= 3 * stage_bytes(256, 2, 2)) {
         // three 48 KiB stages fit only without the store staging: operand traffic matters more than store width
         room += epi_bytes;
         epi_bytes = 0;
     }
-    if (cg == 2 && occ.m_blocks != 1 && RX >= 4 * kBM && stages_for(256, 2, 2) >= 3 && occ.tiles_per_cta == 0) {
+    if (cg == 2 && occ.m_blocks != 1 && RX >= 4 * kBM && stages_for(256, 2, 2) >= 3) {
         const long long t1 = (long long)((RX + 2 * kBM - 1) / (2 * kBM)) * ((RY + bn - 1) / bn);
         const long long t2 = (long long)((RX + 4 * kBM - 1) / (4 * kBM)) * ((RY + bn - 1) / bn);
         const double e1 = wave_eff(t1, budget / 2) * 0.88, e2 = wave_eff(t2, budget / 2) * 0.96;

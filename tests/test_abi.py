@@ -97,7 +97,8 @@ def test_plan_infeasible_knob(ra):
 
 def test_bounded_work_mode_grid(ra):
     p = ra.ra_gemm_plan_query(0, 1, 8192, 8192, 8192, dict(tiles_per_cta=4))
-    assert p["grid"] == 2048 // 4 and p["split_k"] == 1
+    assert p["n_tiles"] == 512 and p["cta_group"] == 2                # 512 x 256 tiles on CTA pairs
+    assert p["grid"] == 2 * 512 // 4 and p["split_k"] == 1            # 2 CTAs per tile, 4 tiles per pair
     assert 2 * (p["dyn_smem_bytes"] + 1024) > 228 * KB               # a second GEMM CTA cannot fit on the SM
 
 
