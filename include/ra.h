@@ -80,6 +80,9 @@ typedef struct {
     int32_t m_blocks;         /* 0 = planner decides; 1 = one 128-row MMA block per CTA (two TMEM accumulators, the
                                  epilogue fully overlaps the next tile); 2 = two blocks sharing one B stage (CTA
                                  pairs only: 512 x 256 tiles, 25 % less operand traffic per flop, one accumulator set) */
+    int32_t cluster_k;        /* 0 = planner decides; 1 = never; 2 = cluster split-K where the shape allows: a 2-CTA
+                                 cluster splits one tile's K range and reduces through distributed shared memory
+                                 (single-CTA tiles with at most #SMs/2 of them, e.g. skinny-N or few-token GEMMs) */
 } ra_occupancy;
 
 /* What S3 decided -- for tests, logs and the sweep tables. */
@@ -96,9 +99,10 @@ typedef struct {
     int32_t clamped;          /* 1 if a knob was clamped */
     int32_t cta_group;        /* 1, or 2 = CTA pairs: `grid` counts CTAs (2 per tile), sm_budget rounded down to even */
     int32_t m_blocks;         /* 128-row MMA blocks per CTA (1 or 2); tile_m = 128 * cta_group * m_blocks */
+    int32_t cluster_k;        /* 1, or 2 = cluster split-K: `grid` = 2 CTAs per tile, no workspace */
 } ra_gemm_plan;
 
-/* Host-only: computes the plan ra_gemm would use.  `occ` NULL = defaults {0,0,0,1,0,0}. */
+/* Host-only: computes the plan ra_gemm would use.  `occ` NULL = defaults {0,0,0,1,0,0,0}. */
 ra_status ra_gemm_plan_query(int transA, int transB, int M, int N, int K, const ra_occupancy* occ, ra_gemm_plan* out);
 
 /* Bytes of device workspace ra_gemm needs for this problem and knob setting (0 if none).

@@ -40,13 +40,13 @@ class RaError(RuntimeError):
 
 class Occupancy(Structure):
     _fields_ = [("smem_reserve_bytes", c_int32), ("sm_budget", c_int32), ("tiles_per_cta", c_int32),
-                ("allow_clamp", c_int32), ("cta_group", c_int32), ("m_blocks", c_int32)]
+                ("allow_clamp", c_int32), ("cta_group", c_int32), ("m_blocks", c_int32), ("cluster_k", c_int32)]
 
 
 class GemmPlan(Structure):
     _fields_ = [(n, c_int32) for n in ("ctas_per_sm", "grid", "stages", "tile_m", "tile_n", "tile_k", "split_k",
                                        "swap_ab", "dyn_smem_bytes", "smem_left_per_sm", "n_tiles", "clamped", "cta_group",
-                                       "m_blocks")]
+                                       "m_blocks", "cluster_k")]
 
     def as_dict(self):
         return {n: getattr(self, n) for n, _ in self._fields_}
@@ -171,7 +171,7 @@ def _occ(occ) -> Occupancy | None:
         return occ
     return Occupancy(int(occ.get("smem_reserve_bytes", 0)), int(occ.get("sm_budget", 0)),
                      int(occ.get("tiles_per_cta", 0)), int(occ.get("allow_clamp", 1)), int(occ.get("cta_group", 0)),
-                     int(occ.get("m_blocks", 0)))
+                     int(occ.get("m_blocks", 0)), int(occ.get("cluster_k", 0)))
 
 
 def _occ_ref(occ):
@@ -339,7 +339,8 @@ def ra_overlap_suggest(workload: Workload, tensor_tflops: float = 0.0, hbm_gbs: 
     _check(_L().ra_overlap_suggest(byref(workload), byref(pk), byref(s)), "ra_overlap_suggest")
     c = s.cfg
     kw = dict(mode=c.mode, occ=dict(smem_reserve_bytes=c.occ.smem_reserve_bytes, sm_budget=c.occ.sm_budget,
-                                    tiles_per_cta=c.occ.tiles_per_cta, cta_group=c.occ.cta_group, m_blocks=c.occ.m_blocks),
+                                    tiles_per_cta=c.occ.tiles_per_cta, cta_group=c.occ.cta_group, m_blocks=c.occ.m_blocks,
+                                    cluster_k=c.occ.cluster_k),
               coll_sm_budget=c.coll_sm_budget, coll_smem_bytes=c.coll_smem_bytes, coll_ctas_per_sm=c.coll_ctas_per_sm,
               coll_variant=c.coll_variant, prio_compute=c.prio_compute, prio_comm=c.prio_comm, dependent=c.dependent)
     return {"kw": kw, "gemm_bound": "hbm" if s.gemm_bound else "tensor", "t_gemm_ms": s.t_gemm_ms, "t_coll_ms": s.t_coll_ms,

@@ -69,6 +69,8 @@ struct GemmParams {
     int xmn, ymn;      // operand storage: 0 = K-contiguous rows (K-major), 1 = row index contiguous (MN-major)
     int epi_tma;       // 1: whole tiles leave through shared memory + TMA stores (non-swapped C only)
     int skew;          // XH == 2: k-blocks by which X block 0 leads block 1 at both ends of a tile (<= stages)
+    int ks;            // 2: cluster split-K -- the two CTAs of a cluster take one tile's k-blocks half each and CTA 1
+                       //    hands its accumulator to CTA 0 through distributed shared memory (CG == 1, XH == 1 only)
 };
 
 // ---- device helpers ---------------------------------------------------------------------------
@@ -224,6 +226,40 @@ __device__ __forceinline__ void st_shared_v4(uint32_t addr, uint32_t a, uint32_t
     asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(a), "r"(b), "r"(c), "r"(d) : "memory");
 }
 
+// ---- cluster split-K: accumulator hand-over through distributed shared memory ---------------------------------
+__device__ __forceinline__ void st_cluster_v4(uint32_t addr_cluster, uint32_t a, uint32_t b, uint32_t c, uint32_t d) {
+    asm volatile("st.shared::cluster.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(addr_cluster), "r"(a), "r"(b), "r"(c), "r"(d) : "memory");
+}
+__device__ __forceinline__ void ld_shared_v4(uint32_t addr, uint32_t& a, uint32_t& b, uint32_t& c, uint32_t& d) {
+    asm volatile("ld.shared.v4.b32 {%0, %1, %2, %3}, [%4];" : "=r"(a), "=r"(b), "=r"(c), "=r"(d) : "r"(addr) : "memory");
+}
+// arrive on a barrier of another CTA of the cluster, releasing this thread's prior (distributed) shared-memory writes
+__device__ __forceinline__ void mbar_arrive_release_cluster(uint32_t bar_cluster) {
+    asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(bar_cluster) : "memory");
+}
+__device__ __forceinline__ bool mbar_try_wait_acquire_cluster(uint32_t bar, uint32_t parity) {
+    uint32_t ok;
+    asm volatile(
+        "{\n\t.reg .pred P;\n\t"
+        "mbarrier.try_wait.parity.acquire.cluster.shared::cta.b64 P, [%1], %2;\n\t"
+        "selp.u32 %0, 1, 0, P;\n\t}"
+        : "=r"(ok)
+        : "r"(bar), "r"(parity)
+        : "memory");
+    return ok != 0;
+}
+__device__ __forceinline__ void mbar_wait_acquire_cluster(uint32_t bar, uint32_t parity) {
+    uint64_t t0 = 0;
+    uint32_t spins = 0;
+    while (!mbar_try_wait_acquire_cluster(bar, parity)) {
+        if ((++spins & 4095u) == 0) {
+            const uint64_t now = globaltimer();
+            if (t0 == 0) t0 = now;
+            else if (now - t0 > 5000000000ull) __trap();   // 5 s: a protocol bug is a failed launch, not a hang
+        }
+    }
+}
+
 __device__ __forceinline__ uint64_t make_policy(int kind) {
     return kind == 1 ? policy_evict_first() : (kind == 2 ? policy_evict_last() : 0ull);   // 0 = no hint
 }
@@ -237,8 +273,9 @@ struct Sched {
     const GemmParams& p;
     long long u0, u1, cur;  // stream-K unit range of this worker
     int it;
-    int wid, nw;            // worker (CTA, or CTA pair) index and count
-    __device__ Sched(const GemmParams& p_, int wid_, int nw_) : p(p_), it(0), wid(wid_), nw(nw_) {
+    int wid, nw;            // worker (CTA, CTA pair, or split-K cluster) index and count
+    int krank;              // cluster split-K: which half of a tile's k-blocks this CTA takes (else 0)
+    __device__ Sched(const GemmParams& p_, int wid_, int nw_, int krank_ = 0) : p(p_), it(0), wid(wid_), nw(nw_), krank(krank_) {
         if (p.stream_k) {
             const long long U = (long long)p.n_tiles * p.kb_per_tile;
             u0 = (long long)wid * U / nw;
@@ -266,6 +303,11 @@ struct Sched {
         s.tile = (int)t;
         s.kb0 = 0;
         s.kb1 = p.kb_per_tile;
+        if (p.ks == 2) {                       // CTA 0: k-blocks [0, h), CTA 1: [h, KB)
+            const int h = p.kb_per_tile >> 1;
+            if (krank == 0) s.kb1 = h;
+            else s.kb0 = h;
+        }
         s.start_unit = 0;
         return true;
     }
@@ -409,12 +451,16 @@ gemm_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constant__ CU
     auto tempty_bar = [&](int b) { return bar_base + 8u * (2 * kMaxStages + 2 + b); };
     const uint32_t tmem_slot = bar_base + 8u * (2 * kMaxStages + 4);
     const uint32_t flag_slot = tmem_slot + 8;
+    const uint32_t ks_ready_bar = tmem_slot + 16;   // in CTA 1: CTA 0's stages are free to receive the accumulator
+    const uint32_t ks_data_bar = tmem_slot + 24;    // in CTA 0: CTA 1's accumulator has landed
     uint8_t* smem_gen = smem_raw + (smem_base - smem_u32(smem_raw));   // generic view of smem_base
 
     const int warp = threadIdx.x >> 5;
     const int lane = threadIdx.x & 31;
     const uint32_t rank = (CG == 2) ? cluster_ctarank() : 0u;          // 0 = leader
-    const int wid = (int)(blockIdx.x / CG), nw = (int)(gridDim.x / CG);
+    const int kdiv = (CG == 2) ? 2 : p.ks;                             // CTAs per worker
+    const int wid = (int)(blockIdx.x / kdiv), nw = (int)(gridDim.x / kdiv);
+    const int krank = (CG == 1 && p.ks == 2) ? (int)cluster_ctarank() : 0;
     uint64_t* rec = (threadIdx.x == 0) ? trace_begin(tr, KID_GEMM) : nullptr;
 
     if (warp == 0 && lane == 0) {
@@ -428,6 +474,8 @@ gemm_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constant__ CU
             mbar_init(tfull_bar(b), 1);
             mbar_init(tempty_bar(b), 4 * CG);     // one arrive per epilogue warp of the pair
         }
+        mbar_init(ks_ready_bar, 4);               // one arrive per epilogue warp of CTA 0
+        mbar_init(ks_data_bar, kEpiThreads);      // every epilogue thread of CTA 1 releases its own writes
         mbar_fence_init();
     }
     if (warp == 1) {
@@ -442,7 +490,7 @@ gemm_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constant__ CU
         }
     }
     tc_fence_before();
-    if constexpr (CG == 2) cluster_sync_all();    // the peer's barriers exist before anything remote touches them
+    if (CG == 2 || p.ks == 2) cluster_sync_all(); // the peer's barriers exist before anything remote touches them
     else __syncthreads();
     tc_fence_after();
     const uint32_t tmem_base = *reinterpret_cast<volatile uint32_t*>(smem_gen + (tmem_slot - smem_base));
@@ -451,7 +499,7 @@ gemm_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constant__ CU
         // ================= TMA producer (one per CTA) =================
         if (lane == 0) {
             const uint64_t polX = make_policy(p.hintX), polY = make_policy(p.hintY);
-            Sched sched(p, wid, nw);
+            Sched sched(p, wid, nw, krank);
             Seg sg;
             int stage = 0;
             uint32_t phase = 0;
@@ -492,7 +540,7 @@ gemm_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constant__ CU
     } else if (warp == 1) {
         // ================= MMA issuer (leader CTA only) =================
         if (lane == 0 && rank == 0) {
-            Sched sched(p, wid, nw);
+            Sched sched(p, wid, nw, krank);
             Seg sg;
             int stage = 0;
             uint32_t phase = 0;
@@ -573,7 +621,7 @@ gemm_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constant__ CU
         const int quarter = warp & 3;                       // TMEM lane quarter this warp may read
         const int xl = quarter * 32 + lane;                 // row inside this CTA's 128-row slab
         const int et = threadIdx.x - 64;                    // 0..127
-        Sched sched(p, wid, nw);
+        Sched sched(p, wid, nw, krank);
         Seg sg;
         int acc_it = 0;
         uint32_t sbuf_it = 0;                               // staging-buffer rotation (per warp)
@@ -584,6 +632,59 @@ gemm_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constant__ CU
             tile_xy(p, sg.tile, tx, ty);
             const bool whole = (sg.kb0 == 0 && sg.kb1 == p.kb_per_tile);
             const int x = tx * kTileX + (int)rank * (kBM * XH) + xl;   // row of X block 0
+            if (CG == 1 && XH == 1 && p.ks == 2) {
+                // ---- cluster split-K: each CTA of the pair holds the sum over half of the k-blocks.  CTA 1 writes its
+                // accumulator into CTA 0's (now idle) stage ring through distributed shared memory -- layout
+                // [32-column chunk][row][32 floats], the eight 16-byte pieces of a row XOR-swizzled by (row & 7) so that
+                // neither side has bank conflicts -- and CTA 0 adds its own half FIRST (k ascending), applies alpha/beta
+                // and stores.  One hand-over per tile, no global-memory round trip, bit-reproducible.
+                mbar_wait(tfull_bar(buf), aphase);
+                tc_fence_after();
+                const uint32_t taddr = tmem_base + ((uint32_t)(quarter * 32) << 16) + (uint32_t)(buf * BN);
+                const uint32_t sw = (uint32_t)(xl & 7);
+                if (krank == 1) {
+                    mbar_wait_acquire_cluster(ks_ready_bar, 0);                // CTA 0's MMAs no longer read its stages
+                    const uint32_t dst0 = mapa(smem_base, 0);
+#pragma unroll 1
+                    for (int c = 0; c < BN / 32; ++c) {
+                        uint32_t v[32];
+                        tmem_ld32(taddr + c * 32, v);
+                        tmem_ld_wait();
+                        const uint32_t drow = dst0 + (uint32_t)((c * kBM + xl) * 128);
+#pragma unroll
+                        for (int q = 0; q < 8; ++q)
+                            st_cluster_v4(drow + (((uint32_t)q ^ sw) << 4), v[4 * q], v[4 * q + 1], v[4 * q + 2], v[4 * q + 3]);
+                    }
+                    mbar_arrive_release_cluster(mapa(ks_data_bar, 0));
+                } else {
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive_release_cluster(mapa(ks_ready_bar, 1));
+                    mbar_wait_acquire_cluster(ks_data_bar, 0);
+#pragma unroll 1
+                    for (int c = 0; c < BN / 32; ++c) {
+                        uint32_t v[32];
+                        tmem_ld32(taddr + c * 32, v);
+                        tmem_ld_wait();
+                        const uint32_t srow = smem_base + (uint32_t)((c * kBM + xl) * 128);
+                        float acc[32];
+#pragma unroll
+                        for (int q = 0; q < 8; ++q) {
+                            uint32_t a, b, cc, d;
+                            ld_shared_v4(srow + (((uint32_t)q ^ sw) << 4), a, b, cc, d);
+                            acc[4 * q + 0] = __fadd_rn(__uint_as_float(v[4 * q + 0]), __uint_as_float(a));
+                            acc[4 * q + 1] = __fadd_rn(__uint_as_float(v[4 * q + 1]), __uint_as_float(b));
+                            acc[4 * q + 2] = __fadd_rn(__uint_as_float(v[4 * q + 2]), __uint_as_float(cc));
+                            acc[4 * q + 3] = __fadd_rn(__uint_as_float(v[4 * q + 3]), __uint_as_float(d));
+                        }
+                        store_out(p, acc, x, ty * BN + c * 32);
+                    }
+                }
+                tc_fence_before();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(tempty_bar(buf));
+                ++acc_it;
+                continue;
+            }
             float* part = nullptr;
             if (!whole) {
                 const int slot = 2 * wid + (sg.start_unit == sched.u0 ? 0 : 1);
@@ -718,7 +819,7 @@ gemm_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constant__ CU
 
     // teardown: nobody may exit (or free TMEM) while the peer can still signal its barriers / read its stages
     tc_fence_before();
-    if constexpr (CG == 2) cluster_sync_all();
+    if (CG == 2 || p.ks == 2) cluster_sync_all();
     else __syncthreads();
     if (warp == 1) {
         tc_fence_after();
@@ -795,7 +896,7 @@ static ra_status validate_shape(int transA, int transB, int M, int N, int K) {
 
 static ra_status make_plan(int transA, int transB, int M, int N, int K, const ra_occupancy* occ_in, Plan* out) {
     RA_TRY(validate_shape(transA, transB, M, N, K));
-    ra_occupancy occ = {0, 0, 0, 1, 0, 0};
+    ra_occupancy occ = {0, 0, 0, 1, 0, 0, 0};
     if (occ_in) occ = *occ_in;
     if (occ.smem_reserve_bytes < 0 || occ.sm_budget < 0 || occ.tiles_per_cta < 0) return RA_ERR_INVALID_ARG;
 
@@ -833,6 +934,7 @@ static ra_status make_plan(int transA, int transB, int M, int N, int K, const ra
     const int kb = (K + kBK - 1) / kBK;
     if (occ.cta_group < 0 || occ.cta_group > 2) return RA_ERR_INVALID_ARG;
     if (occ.m_blocks < 0 || occ.m_blocks > 2) return RA_ERR_INVALID_ARG;
+    if (occ.cluster_k < 0 || occ.cluster_k > 2) return RA_ERR_INVALID_ARG;
 
     // shared memory the GEMM may allocate on an SM
     long avail = (long)smem_per_sm - occ.smem_reserve_bytes - reserved;
@@ -905,7 +1007,7 @@ static ra_status make_plan(int transA, int transB, int M, int N, int K, const ra
     const long long n_tiles = (long long)tiles_x * tiles_y;
     if (n_tiles > 0x3fffffffLL) return RA_ERR_UNSUPPORTED;
 
-    int grid, stream_k = 0, ctas_per_sm = 1;
+    int grid, stream_k = 0, ctas_per_sm = 1, ks = 1;
     if (occ.tiles_per_cta > 0) {
         // bounded work: more CTAs than SMs.  Residency must stay at one GEMM CTA per SM (TMEM holds
         // two accumulators), so pad the request past half of what an SM can give.
@@ -928,7 +1030,20 @@ static ra_status make_plan(int transA, int transB, int M, int N, int K, const ra
         // partials measured 4 % faster than stream-K on all 148 SMs, since 128 SMs already saturate HBM.
         const long long U = n_tiles * kb;
         const double eff = wave_eff(n_tiles, workers);
-        if (cg == 1 && n_tiles > 0 && kb >= 8 && eff < (n_tiles <= workers ? 0.8 : 0.9)) {
+        // Cluster split-K: when two CTAs per tile still fit in one wave, a 2-CTA cluster splits the tile's k-blocks
+        // and hands one accumulator over through distributed shared memory -- twice the CTAs streaming operands and
+        // no global-memory partials, counters or memset.  Taken when it fills at least half of the budgeted SMs (below
+        // that stream-K's finer split wins) and the receiving stage ring can hold a 128 x BN fp32 accumulator.
+        const bool ks_fits = cg == 1 && xh == 1 && n_tiles > 0 && 2 * n_tiles <= workers && kb >= 2 &&
+                             (long)stages * stage_bytes(bn, 1, 1) >= (long)kBM * bn * 4;
+        if (ks_fits && occ.cluster_k != 1 && ((kb >= 16 && 4 * n_tiles >= workers) || occ.cluster_k == 2)) {
+            ks = 2;
+            w = (int)(2 * n_tiles);
+        } else if (occ.cluster_k == 2) {
+            if (!occ.allow_clamp) return RA_ERR_INFEASIBLE_KNOB;
+            clamped = 1;
+        }
+        if (ks == 1 && cg == 1 && n_tiles > 0 && kb >= 8 && eff < (n_tiles <= workers ? 0.8 : 0.9)) {
             stream_k = 1;
             w = workers;
             if ((long long)w * 4 > U) w = (int)(U / 4);   // at least 4 k-blocks per CTA
@@ -949,6 +1064,7 @@ static ra_status make_plan(int transA, int transB, int M, int N, int K, const ra
     g.split_k = 1;
     g.cta_group = cg;
     g.m_blocks = xh;
+    g.cluster_k = ks;
     pl.bn = bn;
     pl.epi_tma = epi_bytes > 0;
     if (stream_k) {
@@ -966,9 +1082,10 @@ static ra_status make_plan(int transA, int transB, int M, int N, int K, const ra
 template <int BN, int CG, int XH>
 static ra_status launch_gemm(const CUtensorMap& mx, const CUtensorMap& my, const CUtensorMap& mc, const GemmParams& p, int grid, int dyn,
                              cudaStream_t stream) {
+    const int cluster = (CG == 2) ? 2 : p.ks;           // CTA pair (tcgen05 cta_group::2) or split-K cluster
     RA_CUDA(cudaFuncSetAttribute(gemm_kernel<BN, CG, XH>, cudaFuncAttributeMaxDynamicSharedMemorySize, dyn));
-    if constexpr (CG == 1) {
-        gemm_kernel<BN, 1, XH><<<grid, kGemmThreads, dyn, stream>>>(mx, my, mc, p, g_trace);
+    if (cluster == 1) {
+        gemm_kernel<BN, CG, XH><<<grid, kGemmThreads, dyn, stream>>>(mx, my, mc, p, g_trace);
         RA_CUDA(cudaGetLastError());
         return RA_OK;
     }
@@ -979,7 +1096,7 @@ static ra_status launch_gemm(const CUtensorMap& mx, const CUtensorMap& my, const
     cfg.stream = stream;
     cudaLaunchAttribute attr[1];
     attr[0].id = cudaLaunchAttributeClusterDimension;
-    attr[0].val.clusterDim.x = CG;
+    attr[0].val.clusterDim.x = (unsigned)cluster;
     attr[0].val.clusterDim.y = 1;
     attr[0].val.clusterDim.z = 1;
     cfg.attrs = attr;
@@ -1078,6 +1195,7 @@ ra_status gemm_launch(int transA, int transB, int M, int N, int K, float alpha, 
     RA_TRY(make_map(&mx, X, p.RX, K, ldx, kBM * xh, p.xmn));
     RA_TRY(make_map(&my, Y, p.RY, K, ldy, pl.bn / cg, p.ymn));
     p.epi_tma = pl.epi_tma;
+    p.ks = pl.pub.cluster_k;
     p.skew = pl.pub.stages;   // measured on 8192^3 (4 stages): drain wait per tile 5.9k cycles at skew 0, 1.5k at 4
     if (p.epi_tma) RA_TRY(make_map(&mc, C, M, N, ldc, 32, 0));    // C: box = 64 columns x 32 rows (one epilogue warp)
     else mc = mx;                                                  // unused

@@ -62,7 +62,7 @@ ra_status ra_overlap_suggest(const ra_workload* w, const ra_peaks* peaks, ra_sug
 
     ra_suggestion s{};
     s.cfg.mode = RA_MODE_OVERLAP;
-    s.cfg.occ = {0, 0, 0, 1, 0, 0};
+    s.cfg.occ = {0, 0, 0, 1, 0, 0, 0};
     s.cfg.dependent = 1;
     s.cfg.prio_compute = 0;
     s.cfg.prio_comm = 0;                                  // priority off (persistent GEMM, see header)
@@ -76,7 +76,7 @@ ra_status ra_overlap_suggest(const ra_workload* w, const ra_peaks* peaks, ra_sug
     if (has_gemm) {
         // candidate budgets: all SMs and every smaller even count down to half the chip (the sweep's range)
         for (int b = sm_count; b >= sm_count / 2; b -= 2) {
-            ra_occupancy occ = {0, b == sm_count ? 0 : b, 0, 1, 0, 0};
+            ra_occupancy occ = {0, b == sm_count ? 0 : b, 0, 1, 0, 0, 0};
             ra_gemm_plan pl{};
             RA_TRY(ra_gemm_plan_query(w->transA, w->transB, w->M, w->N, w->K, &occ, &pl));
             const int workers = pl.grid / (pl.cta_group > 0 ? pl.cta_group : 1);

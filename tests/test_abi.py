@@ -38,11 +38,11 @@ def test_status_strings(ra):
 
 def test_struct_layouts_match_header(ra):
     # sizes computed by hand from include/ra.h (LP64)
-    assert ctypes.sizeof(ra.Occupancy) == 24
-    assert ctypes.sizeof(ra.GemmPlan) == 56
+    assert ctypes.sizeof(ra.Occupancy) == 28
+    assert ctypes.sizeof(ra.GemmPlan) == 60
     assert ctypes.sizeof(ra.Workload) == 152
-    assert ctypes.sizeof(ra.OverlapCfg) == 4 + 24 + 9 * 4
-    assert ctypes.sizeof(ra.OverlapResult) == 24 + 56 + 8
+    assert ctypes.sizeof(ra.OverlapCfg) == 4 + 28 + 9 * 4
+    assert ctypes.sizeof(ra.OverlapResult) == 24 + 60 + 4 + 8
     assert ctypes.sizeof(ra.HostIO) == 7 * 8
 
 

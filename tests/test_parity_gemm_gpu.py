@@ -287,3 +287,41 @@ def test_errors(ra):
     torch.cuda.synchronize()
     out = to_host(c, np.uint16).reshape(64, 64)
     assert np.all(out[:32, :32] == 0x4000) and np.all(out[:32, 32:] == 0x3F80)
+
+
+# ---- cluster split-K: 2-CTA clusters split one tile's K range, reduction through distributed shared memory ---------
+@pytest.mark.parametrize("M,N,K", [(200, 200, 8192), (130, 100, 1000), (128, 64, 128), (64, 1024, 2048), (17, 640, 1536),
+                                   (300, 128, 4096), (257, 131, 333), (1000, 64, 320), (8192, 128, 1024)])
+def test_cluster_split_k(ra, M, N, K):
+    occ = dict(cluster_k=2, cta_group=1)
+    plan = ra.ra_gemm_plan_query(0, 1, M, N, K, occ)
+    assert plan["cluster_k"] == 2 and plan["split_k"] == 1 and plan["grid"] == 2 * plan["n_tiles"], plan
+    assert ra.ra_gemm_workspace_bytes(0, 1, M, N, K, occ) == 0
+    check(ra, M, N, K, seed=8000 + M + N + K, occ=occ)
+    check(ra, M, N, K, seed=8100 + M + N + K, alpha=-0.5, beta=2.0, occ=occ)
+
+
+@pytest.mark.parametrize("transA,transB", [(0, 0), (1, 0), (1, 1)])
+def test_cluster_split_k_trans(ra, transA, transB):
+    check(ra, 264, 200, 1032, seed=8200 + 2 * transA + transB, occ=dict(cluster_k=2, cta_group=1), transA=transA, transB=transB)
+    check(ra, 40, 648, 520, seed=8210 + 2 * transA + transB, occ=dict(cluster_k=2), transA=transA, transB=transB)   # swapped
+
+
+def test_cluster_split_k_auto_exact_and_reproducible(ra):
+    M, N, K = 8192, 128, 2048                                  # 64 tiles x 32 k-blocks: the planner picks it on its own
+    plan = ra.ra_gemm_plan_query(0, 1, M, N, K)
+    assert plan["cluster_k"] == 2 and plan["grid"] == 128, plan
+    A = ra_inputs.smallint_bf16((M, K), 51, ra_inputs.STREAM_A)
+    B = ra_inputs.smallint_bf16((N, K), 51, ra_inputs.STREAM_B)
+    _, ref16 = oracle.gemm(0, 1, M, N, K, 1.0, A, B)
+    got, _ = run_gemm(ra, M, N, K, A, B)
+    assert np.array_equal(got, ref16)                          # integer inputs: exact in any summation order
+    An = ra_inputs.normal_bf16((M, K), 52, ra_inputs.STREAM_A)
+    Bn = ra_inputs.normal_bf16((N, K), 52, ra_inputs.STREAM_B)
+    first, _ = run_gemm(ra, M, N, K, An, Bn)
+    for _ in range(3):
+        again, _ = run_gemm(ra, M, N, K, An, Bn)
+        assert np.array_equal(first, again)                    # fixed order (low half + high half): run-to-run identical
+    ref, _ = oracle.gemm(0, 1, M, N, K, 1.0, An, Bn)
+    rowA, colB = oracle.gemm_norms(0, 1, M, N, K, An, Bn)
+    assert gemm_norm_err(first, ref, rowA, colB) <= GEMM_TOL
