@@ -174,7 +174,9 @@ def sweep_candidates(ra, cfg, quick: bool):
     for r in reserves:
         for b in budgets:
             for prio in (0, hi):
-                for csb in sorted({0, info["sm_count"] - b} if b < info["sm_count"] else {0}):
+                # collective SM budget: the SMs the GEMM leaves free, or -- with the GEMM on every SM -- a throttled
+                # collective on 24-48 SMs that still finishes inside the GEMM's time but disturbs fewer SMs
+                for csb in sorted({0, info["sm_count"] - b} if b < info["sm_count"] else ({0, 24, 32, 48} if r == 0 else {0})):
                     base = dict(mode=1, occ=dict(smem_reserve_bytes=r, sm_budget=b), prio_compute=0, prio_comm=prio, coll_sm_budget=csb)
                     if cfg.coll == "alltoall":
                         # TMA ring sized to fit INSIDE the reserve (ring + 1 KiB system + barriers), and the
