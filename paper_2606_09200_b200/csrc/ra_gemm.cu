@@ -944,6 +944,20 @@ static ra_status make_plan(int transA, int transB, int M, int N, int K, const ra
     const int RX = swap ? N : M, RY = swap ? M : N;
     int bn = RY > 128 ? 256 : (RY > 64 ? 128 : 64);
     const int kb = (K + kBK - 1) / kBK;
+    // Small problems: when narrower tiles still fit in ONE wave, take them -- more CTAs share the work and each CTA's
+    // serial tail (TMEM drain + stores, ~0.45 us per 64-column box per warp) shrinks with the tile; operand re-use per
+    // byte is worse but nothing is bandwidth-bound at this size (1024^3: 13 us with 256 x 256 pair tiles on 32 CTAs).
+    bool one_wave = false;
+    if (!swap && occ.cta_group != 2 && occ.m_blocks != 2 && occ.tiles_per_cta == 0 && occ.cluster_k != 2) {
+        const long long tx1 = (RX + kBM - 1) / kBM;
+        for (int cand = 64; cand < bn; cand <<= 1) {
+            if (tx1 * ((RY + cand - 1) / cand) <= budget) {
+                bn = cand;
+                one_wave = true;
+                break;
+            }
+        }
+    }
     if (occ.cta_group < 0 || occ.cta_group > 2) return RA_ERR_INVALID_ARG;
     if (occ.m_blocks < 0 || occ.m_blocks > 2) return RA_ERR_INVALID_ARG;
     if (occ.cluster_k < 0 || occ.cluster_k > 2) return RA_ERR_INVALID_ARG;
@@ -1055,7 +1069,7 @@ static ra_status make_plan(int transA, int transB, int M, int N, int K, const ra
             if (!occ.allow_clamp) return RA_ERR_INFEASIBLE_KNOB;
             clamped = 1;
         }
-        if (ks == 1 && cg == 1 && n_tiles > 0 && kb >= 8 && eff < (n_tiles <= workers ? 0.8 : 0.9)) {
+        if (ks == 1 && cg == 1 && !one_wave && n_tiles > 0 && kb >= 8 && eff < (n_tiles <= workers ? 0.8 : 0.9)) {
             stream_k = 1;
             w = workers;
             if ((long long)w * 4 > U) w = (int)(U / 4);   // at least 4 k-blocks per CTA

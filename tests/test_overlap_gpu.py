@@ -248,7 +248,7 @@ def test_graph_replay_matches_oracle_and_streams(ra):
     """use_graph: first call captures + runs, later calls replay the cached graph; the in-place allreduce and the
     stream-K GEMM (memset node + workspace) must behave exactly as the stream schedule does."""
     import torch
-    M, N, K = 200, 200, 8192                       # stream-K plan (workspace, counter memset)
+    M, N, K = 64, 4096, 8192                       # stream-K plan (workspace, counter memset)
     A, B, g, dC = _gemm_side(ra, M, N, K, 123)
     assert ra.ra_gemm_plan_query(0, 1, M, N, K)["split_k"] > 1
     bufs = [ra_inputs.uniform_f32(100003, 123, ra_inputs.STREAM_AR + r) for r in range(3)]

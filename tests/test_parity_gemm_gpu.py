@@ -71,7 +71,7 @@ def check(ra, M, N, K, seed, alpha=1.0, beta=0.0, occ=None, transA=0, transB=1):
     (128, 256, 64, None), (200, 136, 72, None), (130, 260, 200, None), (384, 768, 2048, None),     # single-CTA tiles
     (64, 1024, 2048, None), (17, 640, 1536, None),                                                  # operand swap (+ stream-K)
     (512, 512, 256, dict(cta_group=2)), (1000, 520, 200, dict(cta_group=2)), (2048, 2048, 512, dict(cta_group=2)),  # CTA pairs
-    (200, 200, 4096, None), (300, 200, 4096, dict(cta_group=1)),                                    # stream-K
+    (200, 200, 4096, None), (200, 10000, 1024, None),                                               # one narrow wave / stream-K
     (257, 131, 75, None), (1030, 259, 333, dict(cta_group=2)), (61, 643, 1027, None),               # odd M, N, K (padded ld)
 ])
 def test_all_trans_combinations(ra, transA, transB, M, N, K, occ):
@@ -103,7 +103,7 @@ def test_tiny_config(ra):
     (200, 136, 72), (1, 8, 8), (130, 260, 200), (77, 40, 1000),  # ragged M, N, K tails
     (384, 768, 4096),                                          # several tiles per CTA? (6 tiles)
     (64, 1024, 2048), (17, 640, 1536), (64, 128, 512),         # skinny-M: operand swap (+ stream-K)
-    (200, 200, 8192), (300, 200, 8192),                        # stream-K on the non-swapped path (M < 256) / pair tiles
+    (200, 200, 8192), (300, 200, 8192), (200, 10000, 1024),   # one narrow wave; stream-K on the non-swapped path
     (129, 67, 75), (5, 3, 1), (257, 1001, 333), (1030, 259, 1027),   # nothing a multiple of 8 (ld padded): OOB fill in K,
                                                                # element-granular edges in M and N
 ])
@@ -308,7 +308,7 @@ def test_cluster_split_k_trans(ra, transA, transB):
 
 
 def test_cluster_split_k_auto_exact_and_reproducible(ra):
-    M, N, K = 8192, 128, 2048                                  # 64 tiles x 32 k-blocks: the planner picks it on its own
+    M, N, K = 8192, 64, 2048                                   # 64 tiles x 32 k-blocks: the planner picks it on its own
     plan = ra.ra_gemm_plan_query(0, 1, M, N, K)
     assert plan["cluster_k"] == 2 and plan["grid"] == 128, plan
     A = ra_inputs.smallint_bf16((M, K), 51, ra_inputs.STREAM_A)

@@ -57,7 +57,7 @@ def _gemm_with_guards(ra, M, N, K, ldc, occ, transA=0, transB=1, alpha=1.0, beta
     (1000, 520, 200, dict(cta_group=2, m_blocks=2)),                      # big tiles, ragged both ways (TMA store clips)
     (1000, 520, 200, dict(cta_group=2, m_blocks=1)),                      # pair tiles
     (200, 136, 72, None),                                                 # single-CTA tile, one ragged tile
-    (300, 200, 4096, dict(cta_group=1)),                                  # stream-K: partial tiles + fix-up stores
+    (200, 10000, 1024, None),                                             # stream-K: partial tiles + fix-up stores
     (64, 1000, 512, None),                                                # skinny / swapped: transposed direct stores
     (1000, 520, 200, dict(cta_group=2, smem_reserve_bytes=128 * 1024)),   # squeezed: no store staging, direct stores
     (513, 257 + 7, 64, dict(cta_group=2, m_blocks=2)),                    # one row / a few columns into the next tile
