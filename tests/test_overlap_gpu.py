@@ -273,3 +273,37 @@ def test_graph_replay_matches_oracle_and_streams(ra):
     ref, _ = oracle.gemm(0, 1, M, N, K, 1.0, A, B)
     rowA, colB = oracle.gemm_norms(0, 1, M, N, K, A, B)
     assert gemm_norm_err(plain.reshape(M, N), ref, rowA, colB) <= GEMM_TOL
+
+
+@pytest.mark.parametrize("mode", [0, 1])
+def test_host_pipeline_gemm_only_and_collective_only(ra, mode):
+    """ra_overlap_run_host with only one of the two kernels, serial and overlap mode, outputs optional."""
+    import torch
+    M, N, K = 130, 264, 200
+    A = ra_inputs.normal_bf16((M, K), 31, ra_inputs.STREAM_A)
+    B = ra_inputs.normal_bf16((N, K), 31, ra_inputs.STREAM_B)
+    ref, _ = oracle.gemm(0, 1, M, N, K, 1.0, A, B)
+    rowA, colB = oracle.gemm_norms(0, 1, M, N, K, A, B)
+    g = dict(M=M, N=N, K=K, A=torch.zeros((M, K), dtype=torch.int16, device="cuda"),
+             B=torch.zeros((N, K), dtype=torch.int16, device="cuda"), C=torch.zeros((M, N), dtype=torch.int16, device="cuda"),
+             workspace=torch.empty(max(ra.ra_gemm_workspace_bytes(0, 1, M, N, K), 16), dtype=torch.uint8, device="cuda"))
+    w, keep = ra.make_workload(gemm=g, n_iters=2)
+    hC = torch.zeros((M, N), dtype=torch.int16).pin_memory()
+    io, k2 = ra.make_host_io(A=_pinned(A), B=_pinned(B), C=hC)
+    ra.ra_overlap_run_host(w, None, io, ra.make_cfg(mode=mode), 2)
+    assert gemm_norm_err(hC.numpy().view(np.uint16), ref, rowA, colB) <= GEMM_TOL
+    # C = NULL: nothing is copied back, the device result is still there
+    g["C"].zero_()
+    io2, k3 = ra.make_host_io(A=_pinned(A), B=_pinned(B))
+    ra.ra_overlap_run_host(w, None, io2, ra.make_cfg(mode=mode), 1)
+    assert gemm_norm_err(to_host(g["C"], np.uint16).reshape(M, N), ref, rowA, colB) <= GEMM_TOL
+
+    bufs = [ra_inputs.uniform_f32(5003, 32, ra_inputs.STREAM_AR + r) for r in range(5)]
+    ref_bufs = [b.copy() for b in bufs]
+    oracle.overlap_replay(3, ar_bufs=ref_bufs)
+    dev = [torch.zeros(5003, dtype=torch.float32, device="cuda") for _ in range(5)]
+    wc, kc = ra.make_workload(allreduce=dev, n_iters=3)
+    h_out = torch.zeros(5003, dtype=torch.float32).pin_memory()
+    io3, k4 = ra.make_host_io(ar_in=[_pinned(b) for b in bufs], ar_out=h_out)
+    ra.ra_overlap_run_host(wc, None, io3, ra.make_cfg(mode=mode), 2)
+    assert h_out.numpy().tobytes() == ref_bufs[0].tobytes()
