@@ -1038,6 +1038,10 @@ static ra_status make_plan(int transA, int transB, int M, int N, int K, const ra
         // bounded work: more CTAs than SMs.  Residency must stay at one GEMM CTA per SM (TMEM holds
         // two accumulators), so pad the request past half of what an SM can give.
         grid = cg * (int)((n_tiles + occ.tiles_per_cta - 1) / occ.tiles_per_cta);
+        if (occ.cluster_k == 2) {                 // cluster split-K is a one-tile-per-cluster schedule
+            if (!occ.allow_clamp) return RA_ERR_INFEASIBLE_KNOB;
+            clamped = 1;
+        }
         const int half = (smem_per_sm - 2 * reserved) / 2 + 16;
         if (dyn < half) {
             if (half > avail) {

@@ -84,6 +84,28 @@ def test_plan_depth_shrinks_with_reserve(ra):
         assert p["split_k"] > 1 and p["grid"] == b
 
 
+def test_cluster_split_k_plans(ra):
+    p = ra.ra_gemm_plan_query(0, 1, 8192, 64, 8192)                   # 64 single-CTA tiles, long K: picked automatically
+    assert p["cluster_k"] == 2 and p["grid"] == 128 and p["split_k"] == 1
+    assert ra.ra_gemm_workspace_bytes(0, 1, 8192, 64, 8192) == 0
+    assert ra.ra_gemm_plan_query(0, 1, 8192, 64, 8192, dict(cluster_k=1))["cluster_k"] == 1
+    # not available for CTA-pair tiles or in bounded-work mode: clamped, or refused without allow_clamp
+    for occ in (dict(cluster_k=2, cta_group=2), dict(cluster_k=2, tiles_per_cta=1)):
+        q = ra.ra_gemm_plan_query(0, 1, 2048, 2048, 2048, occ)
+        assert q["cluster_k"] == 1 and q["clamped"] == 1, q
+        with pytest.raises(ra.RaError) as e:
+            ra.ra_gemm_plan_query(0, 1, 2048, 2048, 2048, dict(occ, allow_clamp=0))
+        assert e.value.status == ra.RA_ERR_INFEASIBLE_KNOB
+
+
+def test_small_problem_takes_one_narrow_wave(ra):
+    p = ra.ra_gemm_plan_query(0, 1, 1024, 1024, 1024)
+    assert (p["tile_m"], p["tile_n"], p["grid"], p["split_k"], p["cta_group"]) == (128, 64, 128, 1, 1), p
+    p = ra.ra_gemm_plan_query(0, 1, 256, 256, 256)
+    assert (p["tile_n"], p["grid"]) == (64, 8), p
+    assert ra.ra_gemm_plan_query(0, 1, 2048, 2048, 2048)["cta_group"] == 2      # too big for one wave: pair tiles
+
+
 def test_plan_infeasible_knob(ra):
     with pytest.raises(ra.RaError) as e:
         ra.ra_gemm_plan_query(0, 1, 512, 512, 512, dict(smem_reserve_bytes=226 * KB, allow_clamp=0))
