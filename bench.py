@@ -538,7 +538,7 @@ def main():
     ap.add_argument("--config", default="cb-ar")
     ap.add_argument("--n-iters", type=int, default=0, help="iterations per step (default: the config's, 20)")
     ap.add_argument("--sweep", default="quick", choices=["none", "quick", "full"])
-    ap.add_argument("--sweep-runs", type=int, default=6)
+    ap.add_argument("--sweep-runs", type=int, default=9)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--table", default="", help="write the sweep table (JSON) here")
     args = ap.parse_args()
