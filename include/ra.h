@@ -132,6 +132,15 @@ ra_status ra_gemm(int transA, int transB, int M, int N, int K, float alpha, cons
                   int ldb, float beta, void* C, int ldc, const ra_occupancy* occ, void* workspace,
                   size_t workspace_bytes, void* stream);
 
+/* The same GEMM with a choice of output type ("fp32 output").  c_dtype = RA_DTYPE_BF16 is ra_gemm.
+ * RA_DTYPE_F32: C is M x N fp32, ldc in floats (ldc % 4 == 0, 16-byte aligned base); C = alpha*acc + beta*C_in is
+ * stored as computed in fp32 (no bf16 rounding), and beta != 0 reads C_in as fp32.  Rounding that C to bf16 (RNE)
+ * gives exactly ra_gemm's result.  RA_ERR_INVALID_ARG for any other c_dtype. */
+typedef enum { RA_DTYPE_BF16 = 0, RA_DTYPE_F32 = 1 } ra_dtype;
+ra_status ra_gemm_ex(int transA, int transB, int M, int N, int K, float alpha, const void* A, int lda, const void* B,
+                     int ldb, float beta, void* C, int ldc, int c_dtype, const ra_occupancy* occ, void* workspace,
+                     size_t workspace_bytes, void* stream);
+
 /* ---------------------------------------------------------------------------------------------
  * S4  Allreduce stand-in   (section 2.2: "GEMM kernels compute local gradients, which
  * are then aggregated across all GPUs using allreduce"; BASELINE.json north_star: one device,

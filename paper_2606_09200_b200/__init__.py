@@ -22,11 +22,12 @@ RA_OK, RA_ERR_INVALID_ARG, RA_ERR_UNSUPPORTED, RA_ERR_INFEASIBLE_KNOB, RA_ERR_CU
 RA_COLL_ALLREDUCE, RA_COLL_ALLTOALL, RA_COLL_NONE = 0, 1, 2
 RA_MODE_SERIAL, RA_MODE_OVERLAP = 0, 1
 RA_MAX_RANKS = 16
+RA_DTYPE_BF16, RA_DTYPE_F32 = 0, 1
 
 # every symbol include/ra.h declares (tests/test_abi.py checks the header against this and the .so)
 EXPORTS = (
     "ra_status_str", "ra_last_cuda_error", "ra_shutdown", "ra_device_info", "ra_gemm_plan_query",
-    "ra_gemm_workspace_bytes", "ra_gemm", "ra_allreduce_emul", "ra_allreduce_emul_ex", "ra_alltoall_emul",
+    "ra_gemm_workspace_bytes", "ra_gemm", "ra_gemm_ex", "ra_allreduce_emul", "ra_allreduce_emul_ex", "ra_alltoall_emul",
     "ra_alltoall_emul_ex",
     "ra_overlap_run", "ra_overlap_run_host", "ra_overlap_suggest", "ra_overlap_sweep", "ra_set_trace",
 )
@@ -110,6 +111,8 @@ def _L():
     lib.ra_gemm_workspace_bytes.argtypes = [c_int] * 5 + [POINTER(Occupancy)]
     lib.ra_gemm.argtypes = [c_int, c_int, c_int, c_int, c_int, c_float, c_void_p, c_int, c_void_p, c_int, c_float,
                             c_void_p, c_int, POINTER(Occupancy), c_void_p, c_size_t, c_void_p]
+    lib.ra_gemm_ex.argtypes = [c_int, c_int, c_int, c_int, c_int, c_float, c_void_p, c_int, c_void_p, c_int, c_float,
+                               c_void_p, c_int, c_int, POINTER(Occupancy), c_void_p, c_size_t, c_void_p]
     lib.ra_allreduce_emul.argtypes = [POINTER(c_void_p), c_int, c_size_t, c_int, c_void_p]
     lib.ra_allreduce_emul_ex.argtypes = [POINTER(c_void_p), c_int, c_size_t, c_int, c_int, c_void_p]
     lib.ra_alltoall_emul.argtypes = [c_void_p, c_void_p, c_int, c_size_t, c_int, c_void_p]
@@ -207,6 +210,14 @@ def ra_gemm(transA, transB, M, N, K, alpha, A, lda, B, ldb, beta, C, ldc, occ=No
         workspace_bytes = workspace.numel() * workspace.element_size()
     _check(_L().ra_gemm(transA, transB, M, N, K, float(alpha), _ptr(A), lda, _ptr(B), ldb, float(beta), _ptr(C), ldc,
                         _occ_ref(occ), _ptr(workspace), int(workspace_bytes or 0), _stream(stream)), "ra_gemm")
+
+
+def ra_gemm_ex(transA, transB, M, N, K, alpha, A, lda, B, ldb, beta, C, ldc, c_dtype=RA_DTYPE_BF16, occ=None, workspace=None,
+               workspace_bytes=None, stream=None) -> None:
+    if workspace is not None and workspace_bytes is None:
+        workspace_bytes = workspace.numel() * workspace.element_size()
+    _check(_L().ra_gemm_ex(transA, transB, M, N, K, float(alpha), _ptr(A), lda, _ptr(B), ldb, float(beta), _ptr(C), ldc,
+                           int(c_dtype), _occ_ref(occ), _ptr(workspace), int(workspace_bytes or 0), _stream(stream)), "ra_gemm_ex")
 
 
 def _ptr_array(bufs):

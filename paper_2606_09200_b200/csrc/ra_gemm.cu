@@ -69,6 +69,7 @@ struct GemmParams {
     int xmn, ymn;      // operand storage: 0 = K-contiguous rows (K-major), 1 = row index contiguous (MN-major)
     int epi_tma;       // 1: whole tiles leave through shared memory + TMA stores (non-swapped C only)
     int skew;          // XH == 2: k-blocks by which X block 0 leads block 1 at both ends of a tile (<= stages)
+    int c_f32;         // 1: C is fp32 (ldc in floats): alpha*acc + beta*C without the bf16 rounding, direct stores only
     int ks;            // 2: cluster split-K -- the two CTAs of a cluster take one tile's k-blocks half each and CTA 1
                        //    hands its accumulator to CTA 0 through distributed shared memory (CG == 1, XH == 1 only)
 };
@@ -325,8 +326,52 @@ __device__ __forceinline__ void tile_xy(const GemmParams& p, int tile, int& tx, 
 
 // ---- epilogue pieces ---------------------------------------------------------------------------
 // 32 accumulator values acc[x][y0 .. y0+31] of row x -> C.
+// fp32 C (ra_gemm_ex, c_dtype = RA_DTYPE_F32): same addressing, 4-byte elements, no rounding step
+__device__ __forceinline__ void store_out_f32(const GemmParams& p, const float (&acc)[32], int x, int y0) {
+    const float alpha = p.alpha, beta = p.beta;
+    float* C = reinterpret_cast<float*>(p.C);
+    if (!p.swap) {
+        float* row = C + (size_t)x * p.ldc + y0;
+        if (y0 + 32 <= p.RY) {
+#pragma unroll
+            for (int v = 0; v < 8; ++v) {
+                float4 o = make_float4(alpha * acc[4 * v], alpha * acc[4 * v + 1], alpha * acc[4 * v + 2], alpha * acc[4 * v + 3]);
+                if (beta != 0.f) {
+                    const float4 c = *reinterpret_cast<const float4*>(row + 4 * v);
+                    o.x = fmaf(beta, c.x, o.x); o.y = fmaf(beta, c.y, o.y); o.z = fmaf(beta, c.z, o.z); o.w = fmaf(beta, c.w, o.w);
+                }
+                *reinterpret_cast<float4*>(row + 4 * v) = o;
+            }
+        } else {
+#pragma unroll
+            for (int j = 0; j < 32; ++j) {
+                if (y0 + j < p.RY) {
+                    float r = alpha * acc[j];
+                    if (beta != 0.f) r = fmaf(beta, row[j], r);
+                    row[j] = r;
+                }
+            }
+        }
+    } else {
+        float* ptr = C + (size_t)y0 * p.ldc + x;
+        const size_t ld = (size_t)p.ldc;
+#pragma unroll
+        for (int j = 0; j < 32; ++j) {
+            if (y0 + j < p.RY) {
+                float r = alpha * acc[j];
+                if (beta != 0.f) r = fmaf(beta, ptr[j * ld], r);
+                ptr[j * ld] = r;
+            }
+        }
+    }
+}
+
 __device__ __forceinline__ void store_out(const GemmParams& p, const float (&acc)[32], int x, int y0) {
     if (x >= p.RX || y0 >= p.RY) return;
+    if (p.c_f32) {
+        store_out_f32(p, acc, x, y0);
+        return;
+    }
     const float alpha = p.alpha, beta = p.beta;
     if (!p.swap) {
         __nv_bfloat16* row = p.C + (size_t)x * p.ldc + y0;
@@ -844,12 +889,17 @@ gemm_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constant__ CU
 }
 
 // C = beta * C  (K == 0 or alpha == 0: op(A), op(B) are not referenced, as in BLAS)
-__global__ void scale_c_kernel(__nv_bfloat16* C, int M, int N, int ldc, float beta) {
+__global__ void scale_c_kernel(void* Cv, int M, int N, int ldc, float beta, int c_f32) {
     const size_t total = (size_t)M * N;
     for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (size_t)gridDim.x * blockDim.x) {
         const size_t r = i / N, c = i - r * N;
-        __nv_bfloat16* ptr = C + r * ldc + c;
-        *ptr = (beta == 0.f) ? __float2bfloat16_rn(0.f) : __float2bfloat16_rn(beta * __bfloat162float(*ptr));
+        if (c_f32) {
+            float* ptr = static_cast<float*>(Cv) + r * ldc + c;
+            *ptr = (beta == 0.f) ? 0.f : beta * *ptr;
+        } else {
+            __nv_bfloat16* ptr = static_cast<__nv_bfloat16*>(Cv) + r * ldc + c;
+            *ptr = (beta == 0.f) ? __float2bfloat16_rn(0.f) : __float2bfloat16_rn(beta * __bfloat162float(*ptr));
+        }
     }
 }
 
@@ -1137,8 +1187,9 @@ static ra_status launch_gemm(const CUtensorMap& mx, const CUtensorMap& my, const
 
 ra_status gemm_launch(int transA, int transB, int M, int N, int K, float alpha, const void* A, int lda, const void* B,
                       int ldb, float beta, void* C, int ldc, const ra_occupancy* occ, void* workspace,
-                      size_t workspace_bytes, cudaStream_t stream, ra_gemm_plan* plan_out) {
+                      size_t workspace_bytes, cudaStream_t stream, ra_gemm_plan* plan_out, int c_f32) {
     RA_TRY(validate_shape(transA, transB, M, N, K));
+    if (c_f32 != 0 && c_f32 != 1) return RA_ERR_INVALID_ARG;
     if (M == 0 || N == 0) return RA_OK;
     if (A == nullptr || B == nullptr || C == nullptr) return RA_ERR_INVALID_ARG;
     const int min_lda = transA ? M : K, min_ldb = transB ? K : N;
@@ -1146,10 +1197,10 @@ ra_status gemm_launch(int transA, int transB, int M, int N, int K, float alpha, 
     if ((reinterpret_cast<uintptr_t>(A) & 15u) || (reinterpret_cast<uintptr_t>(B) & 15u) ||
         (reinterpret_cast<uintptr_t>(C) & 15u))
         return RA_ERR_INVALID_ARG;
-    if ((lda % 8) || (ldb % 8) || (ldc % 8)) return RA_ERR_UNSUPPORTED;
+    if ((lda % 8) || (ldb % 8) || (ldc % (c_f32 ? 4 : 8))) return RA_ERR_UNSUPPORTED;   // 16-byte row pitches
     {
         // C must not overlap A or B
-        const uintptr_t c0 = reinterpret_cast<uintptr_t>(C), c1 = c0 + ((size_t)(M - 1) * ldc + N) * 2;
+        const uintptr_t c0 = reinterpret_cast<uintptr_t>(C), c1 = c0 + ((size_t)(M - 1) * ldc + N) * (c_f32 ? 4 : 2);
         const size_t a_elems = transA ? ((size_t)(K > 0 ? K - 1 : 0) * lda + M) : ((size_t)(M - 1) * lda + K);
         const size_t b_elems = transB ? ((size_t)(N - 1) * ldb + K) : ((size_t)(K > 0 ? K - 1 : 0) * ldb + N);
         const uintptr_t a0 = reinterpret_cast<uintptr_t>(A), a1 = a0 + a_elems * 2;
@@ -1170,7 +1221,7 @@ ra_status gemm_launch(int transA, int transB, int M, int N, int K, float alpha, 
     if (K == 0 || alpha == 0.f) {
         const size_t total = (size_t)M * N;
         const int blocks = (int)((total + 255) / 256 < (size_t)di.sm_count * 8 ? (total + 255) / 256 : (size_t)di.sm_count * 8);
-        scale_c_kernel<<<blocks, 256, 0, stream>>>(static_cast<__nv_bfloat16*>(C), M, N, ldc, beta);
+        scale_c_kernel<<<blocks, 256, 0, stream>>>(C, M, N, ldc, beta, c_f32);
         RA_CUDA(cudaGetLastError());
         return RA_OK;
     }
@@ -1224,7 +1275,8 @@ ra_status gemm_launch(int transA, int transB, int M, int N, int K, float alpha, 
     p.ymn = swap ? a_mn : b_mn;
     RA_TRY(make_map(&mx, X, p.RX, K, ldx, kBM * xh, p.xmn));
     RA_TRY(make_map(&my, Y, p.RY, K, ldy, pl.bn / cg, p.ymn));
-    p.epi_tma = pl.epi_tma;
+    p.c_f32 = c_f32;
+    p.epi_tma = c_f32 ? 0 : pl.epi_tma;        // fp32 rows are written directly: 128 contiguous bytes per thread and chunk
     p.ks = pl.pub.cluster_k;
     p.skew = pl.pub.stages;   // measured on 8192^3 (4 stages): drain wait per tile 5.9k cycles at skew 0, 1.5k at 4
     if (p.epi_tma) RA_TRY(make_map(&mc, C, M, N, ldc, 32, 0));    // C: box = 64 columns x 32 rows (one epilogue warp)
@@ -1261,7 +1313,15 @@ ra_status ra_gemm(int transA, int transB, int M, int N, int K, float alpha, cons
                   int ldb, float beta, void* C, int ldc, const ra_occupancy* occ, void* workspace,
                   size_t workspace_bytes, void* stream) {
     return ra::gemm_launch(transA, transB, M, N, K, alpha, A, lda, B, ldb, beta, C, ldc, occ, workspace,
-                           workspace_bytes, static_cast<cudaStream_t>(stream), nullptr);
+                           workspace_bytes, static_cast<cudaStream_t>(stream), nullptr, 0);
+}
+
+ra_status ra_gemm_ex(int transA, int transB, int M, int N, int K, float alpha, const void* A, int lda, const void* B,
+                     int ldb, float beta, void* C, int ldc, int c_dtype, const ra_occupancy* occ, void* workspace,
+                     size_t workspace_bytes, void* stream) {
+    if (c_dtype != RA_DTYPE_BF16 && c_dtype != RA_DTYPE_F32) return RA_ERR_INVALID_ARG;
+    return ra::gemm_launch(transA, transB, M, N, K, alpha, A, lda, B, ldb, beta, C, ldc, occ, workspace,
+                           workspace_bytes, static_cast<cudaStream_t>(stream), nullptr, c_dtype == RA_DTYPE_F32 ? 1 : 0);
 }
 
 }  // extern "C"

@@ -18,7 +18,7 @@ namespace ra {
 
 ra_status gemm_launch(int transA, int transB, int M, int N, int K, float alpha, const void* A, int lda, const void* B,
                       int ldb, float beta, void* C, int ldc, const ra_occupancy* occ, void* workspace,
-                      size_t workspace_bytes, cudaStream_t stream, ra_gemm_plan* plan_out);
+                      size_t workspace_bytes, cudaStream_t stream, ra_gemm_plan* plan_out, int c_f32);
 ra_status allreduce_launch(float* const* bufs, int P, size_t count, int sm_budget, int ctas_per_sm, cudaStream_t stream);
 ra_status alltoall_launch(const void* send, void* recv, int P, size_t chunk_bytes, int sm_budget,
                           int smem_bytes_per_cta, int ctas_per_sm, int variant, cudaStream_t stream);
@@ -88,7 +88,7 @@ static ra_status enqueue_step(const ra_workload* w, const ra_overlap_cfg* cfg, c
         if (has_gemm) {
             if (rec) RA_CUDA(cudaEventRecord(kev(i, 0), s_comp));
             RA_TRY(gemm_launch(w->transA, w->transB, w->M, w->N, w->K, w->alpha, w->A, w->lda, w->B, w->ldb, w->beta,
-                               w->C, w->ldc, &cfg->occ, w->workspace, w->workspace_bytes, s_comp, plan));
+                               w->C, w->ldc, &cfg->occ, w->workspace, w->workspace_bytes, s_comp, plan, 0));
             if (rec) RA_CUDA(cudaEventRecord(kev(i, 1), s_comp));
         }
         if (has_coll) {

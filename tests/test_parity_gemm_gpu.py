@@ -325,3 +325,66 @@ def test_cluster_split_k_auto_exact_and_reproducible(ra):
     ref, _ = oracle.gemm(0, 1, M, N, K, 1.0, An, Bn)
     rowA, colB = oracle.gemm_norms(0, 1, M, N, K, An, Bn)
     assert gemm_norm_err(first, ref, rowA, colB) <= GEMM_TOL
+
+
+# ---- fp32 output (ra_gemm_ex, RA_DTYPE_F32) -------------------------------------------------------------------------
+def run_gemm_f32(ra, M, N, K, A, B, alpha=1.0, beta=0.0, Cin=None, occ=None, ldc=None, transA=0, transB=1):
+    import torch
+    lda = M if transA else K
+    ldb = K if transB else N
+    ldc = ldc or (N + 3) // 4 * 4
+    dC = torch.full((M, ldc), float("nan"), dtype=torch.float32, device="cuda")
+    if Cin is not None:
+        dC.copy_(torch.from_numpy(Cin))
+    ws = torch.empty(max(ra.ra_gemm_workspace_bytes(transA, transB, M, N, K, occ), 16), dtype=torch.uint8, device="cuda")
+    ra.ra_gemm_ex(transA, transB, M, N, K, alpha, to_dev(A), lda, to_dev(B), ldb, beta, dC, ldc, ra.RA_DTYPE_F32, occ=occ, workspace=ws)
+    torch.cuda.synchronize()
+    return dC.cpu().numpy()
+
+
+@pytest.mark.parametrize("M,N,K,occ", [
+    (1024, 512, 512, None), (700, 264, 1024, dict(cta_group=2, m_blocks=2)), (200, 136, 72, None), (64, 1024, 2048, None),
+    (200, 10000, 1024, None), (8192, 64, 2048, None), (129, 67, 72, None), (40, 648, 520, None)])
+def test_f32_output(ra, M, N, K, occ):
+    """C in fp32: same accumulator, no bf16 rounding.  Error bound: fp32 accumulation only (<= K * 2^-24 of the norm
+    bound, far below it in practice); rounding the fp32 result to bf16 reproduces ra_gemm bit for bit."""
+    A = ra_inputs.normal_bf16((M, K), 61, ra_inputs.STREAM_A)
+    B = ra_inputs.normal_bf16((N, K), 61, ra_inputs.STREAM_B)
+    ref, _ = oracle.gemm(0, 1, M, N, K, 1.0, A, B)
+    rowA, colB = oracle.gemm_norms(0, 1, M, N, K, A, B)
+    ldc = (N + 3) // 4 * 4 + 4
+    full = run_gemm_f32(ra, M, N, K, A, B, occ=occ, ldc=ldc)
+    got = full[:, :N]
+    assert np.all(np.isfinite(got)) and np.all(np.isnan(full[:, N:])), "unwritten C or pad columns touched"
+    err = float(np.max(np.abs(got.astype(np.float64) - ref) / (np.outer(rowA, colB) + 1e-30)))
+    assert err <= 2e-5, err
+    bf, _ = run_gemm(ra, M, N, K, A, B, occ=occ, ldc=(N + 7) // 8 * 8)
+    assert np.array_equal(oracle.f32_to_bf16(np.ascontiguousarray(got)), bf)
+    # alpha / beta with an fp32 C_in
+    rng = np.random.default_rng(M + N + K)
+    Cin = rng.standard_normal((M, ldc)).astype(np.float32)
+    out = run_gemm_f32(ra, M, N, K, A, B, alpha=-0.5, beta=2.0, Cin=Cin, occ=occ, ldc=ldc)
+    want = -0.5 * ref + 2.0 * Cin[:, :N].astype(np.float64)
+    den = 0.5 * np.outer(rowA, colB) + 2.0 * np.abs(Cin[:, :N]) + 1e-30
+    assert float(np.max(np.abs(out[:, :N] - want) / den)) <= 2e-5
+    assert np.array_equal(out[:, N:], Cin[:, N:])
+
+
+def test_f32_output_integer_exact_and_errors(ra):
+    import torch
+    M, N, K = 512, 384, 4096
+    A = ra_inputs.smallint_bf16((M, K), 62, ra_inputs.STREAM_A)
+    B = ra_inputs.smallint_bf16((N, K), 62, ra_inputs.STREAM_B)
+    ref, _ = oracle.gemm(0, 1, M, N, K, 1.0, A, B)
+    got = run_gemm_f32(ra, M, N, K, A, B)
+    assert np.array_equal(got.astype(np.float64), ref)          # integers below 2^24: exact in fp32
+    dC = torch.full((M, N), 3.0, dtype=torch.float32, device="cuda")
+    ra.ra_gemm_ex(0, 1, M, N, K, 0.0, to_dev(A), K, to_dev(B), K, 0.5, dC, N, ra.RA_DTYPE_F32)   # alpha = 0: C = beta*C
+    torch.cuda.synchronize()
+    assert torch.all(dC == 1.5)
+    with pytest.raises(ra.RaError) as e:
+        ra.ra_gemm_ex(0, 1, M, N, K, 1.0, to_dev(A), K, to_dev(B), K, 0.0, dC, N, 7)
+    assert e.value.status == ra.RA_ERR_INVALID_ARG
+    with pytest.raises(ra.RaError) as e:
+        ra.ra_gemm_ex(0, 1, M, N, K, 1.0, to_dev(A), K, to_dev(B), K, 0.0, dC, N + 2, ra.RA_DTYPE_F32)   # ldc % 4 != 0
+    assert e.value.status == ra.RA_ERR_UNSUPPORTED
