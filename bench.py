@@ -265,6 +265,10 @@ def kernels_alone(ra, cfg, d, h, peaks, n_iters):
     out["gemm_plan"] = res[0]["plan"]
     reset_collective(cfg, d, h)
     w, keep = make_workload(ra, cfg, d, n_iters, gemm=False)
+    # the collective alone is a bandwidth measurement: let the clocks recover from the power-capped GEMM runs first
+    import torch
+    torch.cuda.synchronize()
+    time.sleep(0.5)
     res, _ = ra.ra_overlap_sweep(w, [ra.make_cfg(mode=0)], runs=6)
     c_ms = res[0]["total_ms"] / n_iters
     out["coll_ms"] = c_ms
