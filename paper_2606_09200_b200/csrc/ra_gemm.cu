@@ -16,13 +16,24 @@
 //                              kind::f16, bf16 in / fp32 accumulate in TMEM), tcgen05.commit frees
 //                              the smem stage / publishes the accumulator
 //   warps 2-5 epilogue         tcgen05.ld (32 lanes x 32 columns per instruction) -> alpha/beta ->
-//                              cvt.rn.bf16x2.f32 -> global stores.  Two TMEM accumulators (2 x BN
-//                              columns) so the epilogue of tile i overlaps the main loop of tile i+1.
+//                              cvt.rn.bf16x2.f32 -> swizzled shared-memory staging -> TMA stores (direct
+//                              stores on the swapped path, for fp32 C, stream-K fix-ups and ragged-N boxes).
+//                              Two TMEM accumulators (2 x BN columns) so the epilogue of tile i overlaps
+//                              the main loop of tile i+1.
+//
+// Tile forms (template <BN, CG, XH>, picked by make_plan):
+//   <BN,1,1>   single-CTA tiles 128 x BN, BN in {64,128,256}: small / skinny problems, stream-K, split-K
+//   <256,2,1>  CTA pairs (2-CTA cluster, tcgen05 cta_group::2): 256 x 256 per pair, half the Y traffic per CTA
+//   <256,2,2>  big tiles: two 128-row X blocks per CTA share one Y stage, 512 x 256 per pair, all 512 TMEM
+//              columns hold ONE tile; the two blocks are issued skewed so the drain of one hides behind the
+//              MMAs of the other at both ends of a tile (large problems; the tile cuBLAS uses too)
 //
 // Scheduling (S3: occupancy shaping).  grid = sm_budget persistent CTAs, one
-// per SM; pipeline depth (and, when squeezed, the tile) follows from smem_reserve_bytes.  Two
-// work decompositions, both static (no atomics in the schedule):
-//   data-parallel   CTA c owns tiles c, c+G, c+2G, ... (grouped rasterisation for L2 reuse)
+// per SM; pipeline depth (and, when squeezed, the tile) follows from smem_reserve_bytes.  Work
+// decompositions, all static (no atomics in the schedule):
+//   data-parallel   worker c owns tiles c, c+G, c+2G, ... (grouped rasterisation for L2 reuse)
+//   cluster split-K a 2-CTA cluster takes one tile's k-blocks half each; CTA 1 hands its accumulator to CTA 0
+//                   through distributed shared memory (no workspace; low + high half, fixed order)
 //   stream-K        the n_tiles*KB k-block units are cut into G equal contiguous ranges; a tile
 //                   whose units span several CTAs is finished by the LAST of them to arrive
 //                   (threadfence + one integer atomic per part): it sums the fp32 partials of all
