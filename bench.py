@@ -397,7 +397,11 @@ def run_ours(args, cfg):
     for _ in range(max(args.warmup, 3)):
         ra.ra_overlap_run(w, ra.make_cfg(mode=1))
     reset_collective(cfg, d, h)
-    cands = [] if args.sweep == "none" else sweep_candidates(ra, cfg, quick=(args.sweep == "quick"))
+    cands = [] if args.sweep in ("none", "auto") else sweep_candidates(ra, cfg, quick=(args.sweep == "quick"))
+    if args.sweep == "auto":       # the library's own short list: model pick + neighbours (ra_overlap_autotune)
+        auto_cfg, _, _ = ra.ra_overlap_autotune(w, peaks["bf16_tflops_sustained"], peaks["hbm_gbs"], runs=args.sweep_runs)
+        reset_collective(cfg, d, h)
+        cands = [ra.cfg_to_kw(auto_cfg)]
     # S7': the model-based policy's pick runs inside the same sweep so that its regret is measured, not assumed
     sug = ra.ra_overlap_suggest(w, peaks["bf16_tflops_sustained"], peaks["hbm_gbs"])
     cand_kws = [dict(mode=0)] + [dict(mode=1)] + [sug["kw"]] + cands
@@ -541,7 +545,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default="cb-ar")
     ap.add_argument("--n-iters", type=int, default=0, help="iterations per step (default: the config's, 20)")
-    ap.add_argument("--sweep", default="quick", choices=["none", "quick", "full"])
+    ap.add_argument("--sweep", default="quick", choices=["none", "auto", "quick", "full"])
     ap.add_argument("--sweep-runs", type=int, default=9)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--table", default="", help="write the sweep table (JSON) here")

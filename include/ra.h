@@ -290,6 +290,14 @@ typedef struct {
 
 ra_status ra_overlap_suggest(const ra_workload* w, const ra_peaks* peaks, ra_suggestion* out);
 
+/* Model + measurement: times the model's pick and its neighbours (collective variant, throttled collective
+ * coll_sm_budget 24 / 32 / 48 for tensor-bound GEMMs, priority on) with ra_overlap_sweep(runs) -- at most ~14 settings
+ * instead of the exhaustive grid -- and returns the fastest.  Runs the workload (an in-place allreduce keeps summing
+ * its buffers, as in ra_overlap_sweep).  best_res (optional) receives that setting's result, n_tried (optional) the
+ * number of settings timed.  Synchronous; host pointers all. */
+ra_status ra_overlap_autotune(const ra_workload* w, const ra_peaks* peaks, int runs, ra_overlap_cfg* best_cfg,
+                              ra_overlap_result* best_res, int* n_tried);
+
 /* Runs cfgs[0..n) `runs` times each, interleaved round-robin so that clock drift hits all settings
  * alike; the first runs/3 passes are warm-up and the mean of the rest is stored in results[i].total_ms
  * ("the first one-third of runs are considered warm-up").  *best = argmin over

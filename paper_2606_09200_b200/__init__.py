@@ -29,7 +29,7 @@ EXPORTS = (
     "ra_status_str", "ra_last_cuda_error", "ra_shutdown", "ra_device_info", "ra_gemm_plan_query",
     "ra_gemm_workspace_bytes", "ra_gemm", "ra_gemm_ex", "ra_allreduce_emul", "ra_allreduce_emul_ex", "ra_alltoall_emul",
     "ra_alltoall_emul_ex",
-    "ra_overlap_run", "ra_overlap_run_host", "ra_overlap_suggest", "ra_overlap_sweep", "ra_set_trace",
+    "ra_overlap_run", "ra_overlap_run_host", "ra_overlap_suggest", "ra_overlap_autotune", "ra_overlap_sweep", "ra_set_trace",
 )
 
 
@@ -121,6 +121,8 @@ def _L():
     lib.ra_overlap_run_host.argtypes = [POINTER(Workload), POINTER(Workload), POINTER(HostIO), POINTER(OverlapCfg), c_int,
                                         POINTER(OverlapResult)]
     lib.ra_overlap_suggest.argtypes = [POINTER(Workload), POINTER(Peaks), POINTER(Suggestion)]
+    lib.ra_overlap_autotune.argtypes = [POINTER(Workload), POINTER(Peaks), c_int, POINTER(OverlapCfg), POINTER(OverlapResult),
+                                        POINTER(c_int)]
     lib.ra_overlap_sweep.argtypes = [POINTER(Workload), POINTER(OverlapCfg), c_int, c_int, POINTER(OverlapResult),
                                      POINTER(c_int)]
     lib.ra_set_trace.argtypes = [c_void_p, c_size_t]
@@ -343,19 +345,32 @@ def ra_overlap_run_host(dev0: Workload, dev1, io: HostIO, cfg: OverlapCfg, n_ste
     return _result_dict(res, dev0.n_iters, None)
 
 
+def cfg_to_kw(c: OverlapCfg) -> dict:
+    """OverlapCfg -> the keyword form make_cfg takes (for logging / re-creating a setting)."""
+    return dict(mode=c.mode, occ=dict(smem_reserve_bytes=c.occ.smem_reserve_bytes, sm_budget=c.occ.sm_budget,
+                                      tiles_per_cta=c.occ.tiles_per_cta, cta_group=c.occ.cta_group, m_blocks=c.occ.m_blocks,
+                                      cluster_k=c.occ.cluster_k),
+                coll_sm_budget=c.coll_sm_budget, coll_smem_bytes=c.coll_smem_bytes, coll_ctas_per_sm=c.coll_ctas_per_sm,
+                coll_variant=c.coll_variant, prio_compute=c.prio_compute, prio_comm=c.prio_comm, dependent=c.dependent)
+
+
 def ra_overlap_suggest(workload: Workload, tensor_tflops: float = 0.0, hbm_gbs: float = 0.0) -> dict:
     """Model-based knob policy (host only).  Returns {"cfg": OverlapCfg, "kw": make_cfg keywords, predictions...}."""
     s = Suggestion()
     pk = Peaks(float(tensor_tflops), float(hbm_gbs))
     _check(_L().ra_overlap_suggest(byref(workload), byref(pk), byref(s)), "ra_overlap_suggest")
-    c = s.cfg
-    kw = dict(mode=c.mode, occ=dict(smem_reserve_bytes=c.occ.smem_reserve_bytes, sm_budget=c.occ.sm_budget,
-                                    tiles_per_cta=c.occ.tiles_per_cta, cta_group=c.occ.cta_group, m_blocks=c.occ.m_blocks,
-                                    cluster_k=c.occ.cluster_k),
-              coll_sm_budget=c.coll_sm_budget, coll_smem_bytes=c.coll_smem_bytes, coll_ctas_per_sm=c.coll_ctas_per_sm,
-              coll_variant=c.coll_variant, prio_compute=c.prio_compute, prio_comm=c.prio_comm, dependent=c.dependent)
+    kw = cfg_to_kw(s.cfg)
     return {"kw": kw, "gemm_bound": "hbm" if s.gemm_bound else "tensor", "t_gemm_ms": s.t_gemm_ms, "t_coll_ms": s.t_coll_ms,
             "t_overlap_ms": s.t_overlap_ms, "t_serial_ms": s.t_serial_ms, "t_roofline_ms": s.t_roofline_ms}
+
+
+def ra_overlap_autotune(workload: Workload, tensor_tflops: float = 0.0, hbm_gbs: float = 0.0, runs: int = 9):
+    """Model pick + neighbours, measured.  Returns (best OverlapCfg, its result dict, number of settings timed)."""
+    pk = Peaks(float(tensor_tflops), float(hbm_gbs))
+    cfg, res, n = OverlapCfg(), OverlapResult(), c_int(0)
+    _check(_L().ra_overlap_autotune(byref(workload), byref(pk), int(runs), byref(cfg), byref(res), byref(n)),
+           "ra_overlap_autotune")
+    return cfg, _result_dict(res, workload.n_iters, None), n.value
 
 
 def ra_overlap_sweep(workload: Workload, cfgs, runs: int = 30):

@@ -16,6 +16,8 @@
 //   * the TMA-ring alltoall needs its ring somewhere: it is chosen when the GEMM leaves SMs free (skinny GEMM:
 //     128 tiles on 148 SMs) or >= ring + 1 KiB per SM unallocated; otherwise the shared-memory-free LDG/STG variant.
 //   * priority: a persistent GEMM never yields an SM, so priority only orders pending grids; "off".
+#include <cstring>
+
 #include "ra_common.cuh"
 
 namespace ra {
@@ -112,6 +114,60 @@ ra_status ra_overlap_suggest(const ra_workload* w, const ra_peaks* peaks, ra_sug
     s.t_serial_ms = t_gemm_alone + t_coll;
     s.t_roofline_ms = (has_gemm && t_tensor_all > t_bytes) ? t_tensor_all : t_bytes;
     *out = s;
+    return RA_OK;
+}
+
+/* Model pick + its neighbours, measured: the short list the sweeps showed to contain the winner -- the collective's
+ * variant (alltoall), a throttled collective (coll_sm_budget 24 / 32 / 48 when the GEMM is tensor-bound), priority on
+ * for the model's pick -- is timed with ra_overlap_sweep and the best setting returned. */
+ra_status ra_overlap_autotune(const ra_workload* w, const ra_peaks* peaks, int runs, ra_overlap_cfg* best_cfg,
+                              ra_overlap_result* best_res, int* n_tried) {
+    if (w == nullptr || best_cfg == nullptr || runs < 1) return RA_ERR_INVALID_ARG;
+    ra_suggestion s{};
+    RA_TRY(ra_overlap_suggest(w, peaks, &s));
+    ra::DeviceInfo di;
+    RA_TRY(ra::device_info(&di));
+    RA_TRY(ra::require_sm100(di));
+
+    ra_overlap_cfg cand[32];
+    int n = 0;
+    auto push = [&](const ra_overlap_cfg& c) {
+        for (int i = 0; i < n; ++i)
+            if (memcmp(&cand[i], &c, sizeof(c)) == 0) return;
+        if (n < 32) cand[n++] = c;
+    };
+    const bool has_gemm = w->M > 0 && w->N > 0;
+    const int variants = w->kind == RA_COLL_ALLTOALL ? 3 : 1;
+    push(s.cfg);
+    for (int v = 0; v < variants; ++v) {
+        ra_overlap_cfg c = s.cfg;
+        c.coll_variant = v;
+        push(c);
+        if (has_gemm && s.gemm_bound == 0 && v != 2) {      // the copy engines have no SM budget
+            for (int csb : {24, 32, 48}) {
+                ra_overlap_cfg t = c;
+                t.coll_sm_budget = csb;
+                push(t);
+            }
+        }
+    }
+    {
+        ra_overlap_cfg c = s.cfg;
+        c.prio_comm = di.prio_greatest;
+        push(c);
+    }
+    ra_overlap_result res[32];
+    memset(res, 0, sizeof(res));
+    int best = -1;
+    RA_TRY(ra_overlap_sweep(w, cand, n, runs, res, &best));
+    if (best < 0) return RA_ERR_INVALID_ARG;
+    *best_cfg = cand[best];
+    if (best_res) {
+        float* kt = best_res->kernel_times;
+        *best_res = res[best];
+        best_res->kernel_times = kt;
+    }
+    if (n_tried) *n_tried = n;
     return RA_OK;
 }
 

@@ -307,3 +307,27 @@ def test_host_pipeline_gemm_only_and_collective_only(ra, mode):
     io3, k4 = ra.make_host_io(ar_in=[_pinned(b) for b in bufs], ar_out=h_out)
     ra.ra_overlap_run_host(wc, None, io3, ra.make_cfg(mode=mode), 2)
     assert h_out.numpy().tobytes() == ref_bufs[0].tobytes()
+
+
+def test_autotune_returns_a_valid_setting_and_keeps_results_exact(ra):
+    """ra_overlap_autotune = model pick + neighbours through ra_overlap_sweep: the returned setting must run, and every
+    run it made must have left oracle-exact data behind (allreduce in place: replay the number of iterations it ran)."""
+    import torch
+    M, N, K = 512, 1024, 2048
+    A, B, g, dC = _gemm_side(ra, M, N, K, 17)
+    P, chunk = 4, 96 * 1024
+    send = ra_inputs.bits_u64(P * P * chunk // 8, 17, ra_inputs.STREAM_A2A)
+    da = to_dev(send)
+    db = torch.zeros_like(da)
+    w, keep = ra.make_workload(gemm=g, alltoall=dict(a=da, b=db, P=P, chunk_bytes=chunk), n_iters=2)
+    cfg, res, n = ra.ra_overlap_autotune(w, runs=3)
+    assert 3 <= n <= 16 and res["total_ms"] > 0 and cfg.mode == ra.RA_MODE_OVERLAP and 0 <= cfg.coll_variant <= 2
+    torch.cuda.synchronize()
+    # n_iters = 2 per run: the ping-pong always ends with a restored and b = transpose(a)
+    assert to_host(da, np.uint64).tobytes() == send.tobytes()
+    assert to_host(db, np.uint64).tobytes() == oracle.alltoall(send, P, chunk).tobytes()
+    ref, _ = oracle.gemm(0, 1, M, N, K, 1.0, A, B)
+    rowA, colB = oracle.gemm_norms(0, 1, M, N, K, A, B)
+    assert gemm_norm_err(to_host(dC, np.uint16).reshape(M, N), ref, rowA, colB) <= GEMM_TOL
+    r2 = ra.ra_overlap_run(w, cfg)                               # the returned setting is directly usable
+    assert r2["total_ms"] > 0
