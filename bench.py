@@ -198,7 +198,8 @@ def cfg_label(kw):
     return {"smem_reserve_bytes": o.get("smem_reserve_bytes", 0), "sm_budget": o.get("sm_budget", 0),
             "tiles_per_cta": o.get("tiles_per_cta", 0), "priority": "on" if kw.get("prio_comm", 0) != kw.get("prio_compute", 0) else "off",
             "coll_sm_budget": kw.get("coll_sm_budget", 0), "coll_smem_bytes": kw.get("coll_smem_bytes", 0),
-            "coll_variant": kw.get("coll_variant", 0), "coll_ctas_per_sm": kw.get("coll_ctas_per_sm", 0)}
+            "coll_variant": kw.get("coll_variant", 0), "coll_ctas_per_sm": kw.get("coll_ctas_per_sm", 0),
+            "use_graph": kw.get("use_graph", 0)}
 
 
 def residency_map(ra, w, cfg_kw, n_sms):

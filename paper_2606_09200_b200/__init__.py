@@ -351,7 +351,8 @@ def cfg_to_kw(c: OverlapCfg) -> dict:
                                       tiles_per_cta=c.occ.tiles_per_cta, cta_group=c.occ.cta_group, m_blocks=c.occ.m_blocks,
                                       cluster_k=c.occ.cluster_k),
                 coll_sm_budget=c.coll_sm_budget, coll_smem_bytes=c.coll_smem_bytes, coll_ctas_per_sm=c.coll_ctas_per_sm,
-                coll_variant=c.coll_variant, prio_compute=c.prio_compute, prio_comm=c.prio_comm, dependent=c.dependent)
+                coll_variant=c.coll_variant, prio_compute=c.prio_compute, prio_comm=c.prio_comm, dependent=c.dependent,
+                use_graph=c.use_graph)
 
 
 def ra_overlap_suggest(workload: Workload, tensor_tflops: float = 0.0, hbm_gbs: float = 0.0) -> dict:

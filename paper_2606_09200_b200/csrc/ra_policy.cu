@@ -113,6 +113,9 @@ ra_status ra_overlap_suggest(const ra_workload* w, const ra_peaks* peaks, ra_sug
     s.t_overlap_ms = (w->kind == RA_COLL_NONE || !has_gemm) ? best_t : (t_gemm_alone + (n - 1) * best_t + t_coll) / n;
     s.t_serial_ms = t_gemm_alone + t_coll;
     s.t_roofline_ms = (has_gemm && t_tensor_all > t_bytes) ? t_tensor_all : t_bytes;
+    // launch-bound steps (kernels of a few microseconds: Tiny): replay the schedule as one CUDA graph
+    // (measured 12.2 -> 8.2 us per overlapped iteration on Tiny; no effect on the full-size workloads)
+    s.cfg.use_graph = (s.t_serial_ms < 0.05) ? 1 : 0;
     *out = s;
     return RA_OK;
 }

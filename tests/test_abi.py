@@ -219,6 +219,9 @@ def test_policy_rooflines_and_choices(ra):
     assert s["gemm_bound"] == "hbm" and s["kw"]["coll_variant"] == 0
     assert abs(s["t_roofline_ms"] - (gb + float(1 << 30)) / (H * 1e6)) < 1e-9
     assert abs(s["t_overlap_ms"] - s["t_serial_ms"]) < 1e-9     # bytes-bound on both sides: nothing to hide
+    assert s["kw"]["use_graph"] == 0                             # full-size kernels: nothing launch-bound to capture
+    wt, keept = _workload(ra, 256, 256, 256, "allreduce", 4, count=65536, n_iters=4)
+    assert ra.ra_overlap_suggest(wt, T, H)["kw"]["use_graph"] == 1     # Tiny: microsecond kernels -> CUDA-graph replay
     # one pipelined iteration has no partner for either kernel: the prediction is the serial time
     w, keep = _workload(ra, 8192, 8192, 8192, "allreduce", 8, count=16 << 20, n_iters=1)
     s = ra.ra_overlap_suggest(w, T, H)
