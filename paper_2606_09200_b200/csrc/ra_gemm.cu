@@ -200,13 +200,13 @@ __device__ __forceinline__ void umma_bf16(uint32_t tmem_d, uint64_t adesc, uint6
 // mbarrier arrive when all MMAs issued so far have retired.  CG == 2: multicast to the same barrier
 // offset in both CTAs of the pair.
 template <int CG>
-__device__ __forceinline__ void umma_commit(uint32_t bar) {
+__device__ __forceinline__ void umma_commit(uint32_t bar, uint16_t pair_mask) {
     if constexpr (CG == 1) {
         asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
     } else {
         asm volatile(
             "tcgen05.commit.cta_group::2.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;"
-            ::"r"(bar), "h"((uint16_t)3)
+            ::"r"(bar), "h"(pair_mask)
             : "memory");
     }
 }
@@ -525,10 +525,14 @@ gemm_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constant__ CU
 
     const int warp = threadIdx.x >> 5;
     const int lane = threadIdx.x & 31;
-    const uint32_t rank = (CG == 2) ? cluster_ctarank() : 0u;          // 0 = leader
-    const int kdiv = (CG == 2) ? 2 : p.ks;                             // CTAs per worker
+    // cluster layout: [k-half (cluster split-K)][pair rank (CG == 2)] -- a CTA pair is two consecutive cluster ranks
+    const uint32_t crank = (CG == 2 || p.ks == 2) ? cluster_ctarank() : 0u;
+    const uint32_t rank = (CG == 2) ? (crank & 1u) : 0u;               // rank inside the CTA pair, 0 = leader
+    const uint32_t lead = (CG == 2) ? (crank & ~1u) : crank;           // cluster rank of this CTA's pair leader
+    const uint16_t pair_mask = (uint16_t)(3u << lead);                 // both CTAs of the pair (CG == 2 commits)
+    const int kdiv = CG * p.ks;                                        // CTAs per worker
     const int wid = (int)(blockIdx.x / kdiv), nw = (int)(gridDim.x / kdiv);
-    const int krank = (CG == 1 && p.ks == 2) ? (int)cluster_ctarank() : 0;
+    const int krank = (p.ks == 2) ? (int)(crank / CG) : 0;
     uint64_t* rec = (threadIdx.x == 0) ? trace_begin(tr, KID_GEMM) : nullptr;
 
     if (warp == 0 && lane == 0) {
@@ -584,7 +588,7 @@ gemm_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constant__ CU
                         bar = full_bar(stage);
                         mbar_expect_tx(bar, kStageBytes);
                     } else {
-                        bar = mapa(full_bar(stage), 0);               // the leader's barrier collects both halves
+                        bar = mapa(full_bar(stage), lead);            // the leader's barrier collects both halves
                         mbar_expect_tx_cluster(bar, kStageBytes);
                     }
                     // K-major operand: one box (64 k x rows).  MN-major operand: one box (64 rows x 64 k) per 64 rows.
@@ -644,10 +648,10 @@ gemm_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constant__ CU
                     for (int kb = sg.kb0; kb < sg.kb1; ++kb) {
                         wait_full(stage, phase);
                         issue_block(stage, 0, (uint32_t)(buf * BN), kb == sg.kb0);
-                        umma_commit<CG>(empty_bar(stage));   // frees the smem stage (in both CTAs) when these MMAs retire
+                        umma_commit<CG>(empty_bar(stage), pair_mask);   // frees the smem stage (in both CTAs) when these MMAs retire
                         if (++stage == p.stages) { stage = 0; phase ^= 1u; }
                     }
-                    umma_commit<CG>(tfull_bar(buf));         // accumulator complete (signals both CTAs' epilogues)
+                    umma_commit<CG>(tfull_bar(buf), pair_mask);         // accumulator complete (signals both CTAs' epilogues)
                 } else {
                     // X block h accumulates in columns [h*BN, h*BN + BN); both belong to this tile, so the TMEM drain
                     // (64 B/clk: ~2k cycles per block) cannot hide behind a second buffer.  Instead the two blocks are
@@ -669,7 +673,7 @@ gemm_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constant__ CU
                     auto step_b = [&]() {
                         if (ib == 0) wait_drained(1, aph ^ 1u);
                         issue_block(sb, 1, (uint32_t)BN, ib == 0);
-                        umma_commit<CG>(empty_bar(sb));       // frees the smem stage (in both CTAs) when these MMAs retire
+                        umma_commit<CG>(empty_bar(sb), pair_mask);       // frees the smem stage (in both CTAs) when these MMAs retire
                         if (++sb == p.stages) sb = 0;
                         ++ib;
                     };
@@ -677,9 +681,9 @@ gemm_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constant__ CU
                     while (ib < D) step_b();                 //       block 1 catches up
                     while (ia < nkb - D) { step_a(); step_b(); }
                     while (ia < nkb) step_a();               // tail: block 0 finishes first ...
-                    umma_commit<CG>(tfull_bar(0));
+                    umma_commit<CG>(tfull_bar(0), pair_mask);
                     while (ib < nkb) step_b();               //       ... and is drained while block 1 finishes
-                    umma_commit<CG>(tfull_bar(1));
+                    umma_commit<CG>(tfull_bar(1), pair_mask);
                 }
                 ++acc_it;
             }
@@ -700,7 +704,7 @@ gemm_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constant__ CU
             tile_xy(p, sg.tile, tx, ty);
             const bool whole = (sg.kb0 == 0 && sg.kb1 == p.kb_per_tile);
             const int x = tx * kTileX + (int)rank * (kBM * XH) + xl;   // row of X block 0
-            if (CG == 1 && XH == 1 && p.ks == 2) {
+            if (XH == 1 && p.ks == 2) {
                 // ---- cluster split-K: each CTA of the pair holds the sum over half of the k-blocks.  CTA 1 writes its
                 // accumulator into CTA 0's (now idle) stage ring through distributed shared memory -- layout
                 // [32-column chunk][row][32 floats], the eight 16-byte pieces of a row XOR-swizzled by (row & 7) so that
@@ -712,7 +716,7 @@ gemm_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constant__ CU
                 const uint32_t sw = (uint32_t)(xl & 7);
                 if (krank == 1) {
                     mbar_wait_acquire_cluster(ks_ready_bar, 0);                // CTA 0's MMAs no longer read its stages
-                    const uint32_t dst0 = mapa(smem_base, 0);
+                    const uint32_t dst0 = mapa(smem_base, crank - CG);         // same CTA of the pair / tile, k-half 0
 #pragma unroll 1
                     for (int c = 0; c < BN / 32; ++c) {
                         uint32_t v[32];
@@ -723,10 +727,10 @@ gemm_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constant__ CU
                         for (int q = 0; q < 8; ++q)
                             st_cluster_v4(drow + (((uint32_t)q ^ sw) << 4), v[4 * q], v[4 * q + 1], v[4 * q + 2], v[4 * q + 3]);
                     }
-                    mbar_arrive_release_cluster(mapa(ks_data_bar, 0));
+                    mbar_arrive_release_cluster(mapa(ks_data_bar, crank - CG));
                 } else {
                     __syncwarp();
-                    if (lane == 0) mbar_arrive_release_cluster(mapa(ks_ready_bar, 1));
+                    if (lane == 0) mbar_arrive_release_cluster(mapa(ks_ready_bar, crank + CG));
                     mbar_wait_acquire_cluster(ks_data_bar, 0);
 #pragma unroll 1
                     for (int c = 0; c < BN / 32; ++c) {
@@ -749,7 +753,10 @@ gemm_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constant__ CU
                 }
                 tc_fence_before();
                 __syncwarp();
-                if (lane == 0) mbar_arrive(tempty_bar(buf));
+                if (lane == 0) {
+                    if constexpr (CG == 1) mbar_arrive(tempty_bar(buf));
+                    else mbar_arrive_cluster(mapa(tempty_bar(buf), lead));
+                }
                 ++acc_it;
                 continue;
             }
@@ -833,7 +840,7 @@ gemm_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constant__ CU
                 __syncwarp();
                 if (lane == 0) {
                     if constexpr (CG == 1) mbar_arrive(tempty_bar(acc_idx));
-                    else mbar_arrive_cluster(mapa(tempty_bar(acc_idx), 0));
+                    else mbar_arrive_cluster(mapa(tempty_bar(acc_idx), lead));
                 }
             }
             ++acc_it;
@@ -1011,8 +1018,18 @@ static ra_status make_plan(int transA, int transB, int M, int N, int K, const ra
     bool one_wave = false;
     if (!swap && occ.cta_group != 2 && occ.m_blocks != 2 && occ.tiles_per_cta == 0 && occ.cluster_k != 2) {
         const long long tx1 = (RX + kBM - 1) / kBM;
+        // the alternative for mid-size problems with a long K: 256 x 256 pair tiles with the K range split over two
+        // pairs of a 4-CTA cluster (half the L2->SM bytes per flop of a narrow single-CTA tile).  Cycle estimates per
+        // CTA: narrow tile kb * (128 + bn) * 2 (load-bound), split pair tile kb/2 * 512 + ~4k for the hand-over.
+        long long pair_ks_cost = -1;
+        if (bn == 256 && RX >= 2 * kBM && occ.cta_group != 1 && occ.cluster_k != 1 && kb >= 16) {
+            const long long T = (long long)((RX + 2 * kBM - 1) / (2 * kBM)) * ((RY + 255) / 256);
+            const int pairs = budget / 2;
+            if (2 * T <= pairs && 4 * T >= pairs) pair_ks_cost = (long long)(kb / 2) * 512 + 4096;
+        }
         for (int cand = 64; cand < bn; cand <<= 1) {
             if (tx1 * ((RY + cand - 1) / cand) <= budget) {
+                if (pair_ks_cost >= 0 && pair_ks_cost < (long long)kb * (kBM + cand) * 2) break;   // split pair tiles win
                 bn = cand;
                 one_wave = true;
                 break;
@@ -1125,11 +1142,11 @@ static ra_status make_plan(int transA, int transB, int M, int N, int K, const ra
         // and hands one accumulator over through distributed shared memory -- twice the CTAs streaming operands and
         // no global-memory partials, counters or memset.  Taken when it fills at least half of the budgeted SMs (below
         // that stream-K's finer split wins) and the receiving stage ring can hold a 128 x BN fp32 accumulator.
-        const bool ks_fits = cg == 1 && xh == 1 && n_tiles > 0 && 2 * n_tiles <= workers && kb >= 2 &&
-                             (long)stages * stage_bytes(bn, 1, 1) >= (long)kBM * bn * 4;
+        const bool ks_fits = xh == 1 && n_tiles > 0 && 2 * n_tiles <= workers && kb >= 2 &&
+                             (long)stages * stage_bytes(bn, cg, 1) >= (long)kBM * bn * 4;
         if (ks_fits && occ.cluster_k != 1 && ((kb >= 16 && 4 * n_tiles >= workers) || occ.cluster_k == 2)) {
             ks = 2;
-            w = (int)(2 * n_tiles);
+            w = (int)(2 * n_tiles);                   // workers: CTAs, or CTA pairs (4-CTA clusters)
         } else if (occ.cluster_k == 2) {
             if (!occ.allow_clamp) return RA_ERR_INFEASIBLE_KNOB;
             clamped = 1;
@@ -1173,7 +1190,7 @@ static ra_status make_plan(int transA, int transB, int M, int N, int K, const ra
 template <int BN, int CG, int XH>
 static ra_status launch_gemm(const CUtensorMap& mx, const CUtensorMap& my, const CUtensorMap& mc, const GemmParams& p, int grid, int dyn,
                              cudaStream_t stream) {
-    const int cluster = (CG == 2) ? 2 : p.ks;           // CTA pair (tcgen05 cta_group::2) or split-K cluster
+    const int cluster = CG * p.ks;                      // CTA pair (tcgen05 cta_group::2) x split-K halves
     RA_CUDA(cudaFuncSetAttribute(gemm_kernel<BN, CG, XH>, cudaFuncAttributeMaxDynamicSharedMemorySize, dyn));
     if (cluster == 1) {
         gemm_kernel<BN, CG, XH><<<grid, kGemmThreads, dyn, stream>>>(mx, my, mc, p, g_trace);

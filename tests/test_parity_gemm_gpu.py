@@ -178,8 +178,8 @@ def test_big_tiles_integer_exact_and_bit_identical(ra):
     An = ra_inputs.normal_bf16((M, K), 44, ra_inputs.STREAM_A)
     Bn = ra_inputs.normal_bf16((N, K), 44, ra_inputs.STREAM_B)
     c4, _ = run_gemm(ra, M, N, K, An, Bn, occ=dict(cta_group=2, m_blocks=2))
-    c2, _ = run_gemm(ra, M, N, K, An, Bn, occ=dict(cta_group=2, m_blocks=1))
-    c1, _ = run_gemm(ra, M, N, K, An, Bn, occ=dict(cta_group=1, sm_budget=24))
+    c2, _ = run_gemm(ra, M, N, K, An, Bn, occ=dict(cta_group=2, m_blocks=1, cluster_k=1))   # (no K split: same association)
+    c1, _ = run_gemm(ra, M, N, K, An, Bn, occ=dict(cta_group=1, sm_budget=24, cluster_k=1))
     assert np.array_equal(c4, c2) and np.array_equal(c4, c1)
 
 
@@ -193,8 +193,8 @@ def test_cta_pairs_integer_exact_and_bit_identical_to_single(ra):
     # same per-element K order (k-blocks ascending, one accumulator) => pairs and single CTAs agree bit for bit
     An = ra_inputs.normal_bf16((M, K), 42, ra_inputs.STREAM_A)
     Bn = ra_inputs.normal_bf16((N, K), 42, ra_inputs.STREAM_B)
-    c2, _ = run_gemm(ra, M, N, K, An, Bn, occ=dict(cta_group=2, sm_budget=148))
-    c1, _ = run_gemm(ra, M, N, K, An, Bn, occ=dict(cta_group=1, sm_budget=24))
+    c2, _ = run_gemm(ra, M, N, K, An, Bn, occ=dict(cta_group=2, sm_budget=148, cluster_k=1))
+    c1, _ = run_gemm(ra, M, N, K, An, Bn, occ=dict(cta_group=1, sm_budget=24, cluster_k=1))
     assert ra.ra_gemm_plan_query(0, 1, M, N, K, dict(cta_group=1, sm_budget=24))["split_k"] == 1
     assert np.array_equal(c1, c2)
 
@@ -388,3 +388,35 @@ def test_f32_output_integer_exact_and_errors(ra):
     with pytest.raises(ra.RaError) as e:
         ra.ra_gemm_ex(0, 1, M, N, K, 1.0, to_dev(A), K, to_dev(B), K, 0.0, dC, N + 2, ra.RA_DTYPE_F32)   # ldc % 4 != 0
     assert e.value.status == ra.RA_ERR_UNSUPPORTED
+
+
+# ---- cluster split-K on CTA pairs: 4-CTA clusters, two pairs split one 256 x 256 tile's K range ----------------------
+@pytest.mark.parametrize("M,N,K", [(512, 512, 4096), (300, 264, 2048), (1000, 520, 1032), (256, 256, 128), (257, 1001, 333)])
+def test_pair_cluster_split_k(ra, M, N, K):
+    occ = dict(cluster_k=2, cta_group=2, m_blocks=1)
+    plan = ra.ra_gemm_plan_query(0, 1, M, N, K, occ)
+    assert plan["cluster_k"] == 2 and plan["cta_group"] == 2 and plan["grid"] == 4 * plan["n_tiles"], plan
+    check(ra, M, N, K, seed=8300 + M + N + K, occ=occ)
+    check(ra, M, N, K, seed=8400 + M + N + K, alpha=2.0, beta=-0.5, occ=occ)
+    for transA, transB in ((0, 0), (1, 0), (1, 1)):
+        check(ra, M, N, K, seed=8500 + M + 2 * transA + transB, occ=occ, transA=transA, transB=transB)
+
+
+def test_pair_cluster_split_k_auto_exact_and_reproducible(ra):
+    M, N, K = 384, 4096, 4096                                   # 32 pair tiles, 64 k-blocks: picked by the planner
+    plan = ra.ra_gemm_plan_query(0, 1, M, N, K)
+    assert plan["cluster_k"] == 2 and plan["cta_group"] == 2 and plan["grid"] == 128, plan
+    A = ra_inputs.smallint_bf16((M, K), 71, ra_inputs.STREAM_A)
+    B = ra_inputs.smallint_bf16((N, K), 71, ra_inputs.STREAM_B)
+    _, ref16 = oracle.gemm(0, 1, M, N, K, 1.0, A, B)
+    got, _ = run_gemm(ra, M, N, K, A, B)
+    assert np.array_equal(got, ref16)
+    An = ra_inputs.normal_bf16((M, K), 72, ra_inputs.STREAM_A)
+    Bn = ra_inputs.normal_bf16((N, K), 72, ra_inputs.STREAM_B)
+    first, _ = run_gemm(ra, M, N, K, An, Bn)
+    for _ in range(3):
+        again, _ = run_gemm(ra, M, N, K, An, Bn)
+        assert np.array_equal(first, again)
+    ref, _ = oracle.gemm(0, 1, M, N, K, 1.0, An, Bn)
+    rowA, colB = oracle.gemm_norms(0, 1, M, N, K, An, Bn)
+    assert gemm_norm_err(first, ref, rowA, colB) <= GEMM_TOL
