@@ -80,10 +80,12 @@ typedef struct {
     int32_t m_blocks;         /* 0 = planner decides; 1 = one 128-row MMA block per CTA (two TMEM accumulators, the
                                  epilogue fully overlaps the next tile); 2 = two blocks sharing one B stage (CTA
                                  pairs only: 512 x 256 tiles, 25 % less operand traffic per flop, one accumulator set) */
-    int32_t cluster_k;        /* 0 = planner decides; 1 = never; 2 = cluster split-K where the shape allows: the K
-                                 range of one tile is split over the two CTAs of a 2-CTA cluster (single-CTA tiles) or
-                                 the two CTA pairs of a 4-CTA cluster (256 x 256 pair tiles) and reduced through
-                                 distributed shared memory; needs at most #SMs/2 CTAs' worth of tiles */
+    int32_t cluster_k;        /* 0 = planner decides; 1 = never; 2 / 4 = cluster split-K in that many parts where the
+                                 shape allows: the K range of one tile is split over the 2 or 4 CTAs of a cluster
+                                 (single-CTA tiles) or the two CTA pairs of a 4-CTA cluster (256 x 256 pair tiles,
+                                 2 parts only) and reduced through distributed shared memory in ascending-k order;
+                                 needs parts * tiles <= #SMs (pairs: 4 * tiles) and room for the parts' accumulators
+                                 in part 0's stage ring */
 } ra_occupancy;
 
 /* What S3 decided -- for tests, logs and the sweep tables. */
@@ -100,7 +102,7 @@ typedef struct {
     int32_t clamped;          /* 1 if a knob was clamped */
     int32_t cta_group;        /* 1, or 2 = CTA pairs: `grid` counts CTAs (2 per tile), sm_budget rounded down to even */
     int32_t m_blocks;         /* 128-row MMA blocks per CTA (1 or 2); tile_m = 128 * cta_group * m_blocks */
-    int32_t cluster_k;        /* 1, or 2 = cluster split-K: `grid` = 2 * cta_group CTAs per tile, no workspace */
+    int32_t cluster_k;        /* 1, or 2 / 4 = cluster split-K parts: `grid` = cluster_k * cta_group CTAs per tile, no workspace */
 } ra_gemm_plan;
 
 /* Host-only: computes the plan ra_gemm would use.  `occ` NULL = defaults {0,0,0,1,0,0,0}. */

@@ -315,10 +315,9 @@ struct Sched {
         s.tile = (int)t;
         s.kb0 = 0;
         s.kb1 = p.kb_per_tile;
-        if (p.ks == 2) {                       // CTA 0: k-blocks [0, h), CTA 1: [h, KB)
-            const int h = p.kb_per_tile >> 1;
-            if (krank == 0) s.kb1 = h;
-            else s.kb0 = h;
+        if (p.ks > 1) {                        // part r of ks takes k-blocks [KB*r/ks, KB*(r+1)/ks)
+            s.kb0 = p.kb_per_tile * krank / p.ks;
+            s.kb1 = p.kb_per_tile * (krank + 1) / p.ks;
         }
         s.start_unit = 0;
         return true;
@@ -526,13 +525,13 @@ gemm_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constant__ CU
     const int warp = threadIdx.x >> 5;
     const int lane = threadIdx.x & 31;
     // cluster layout: [k-half (cluster split-K)][pair rank (CG == 2)] -- a CTA pair is two consecutive cluster ranks
-    const uint32_t crank = (CG == 2 || p.ks == 2) ? cluster_ctarank() : 0u;
+    const uint32_t crank = (CG == 2 || p.ks > 1) ? cluster_ctarank() : 0u;
     const uint32_t rank = (CG == 2) ? (crank & 1u) : 0u;               // rank inside the CTA pair, 0 = leader
     const uint32_t lead = (CG == 2) ? (crank & ~1u) : crank;           // cluster rank of this CTA's pair leader
     const uint16_t pair_mask = (uint16_t)(3u << lead);                 // both CTAs of the pair (CG == 2 commits)
     const int kdiv = CG * p.ks;                                        // CTAs per worker
     const int wid = (int)(blockIdx.x / kdiv), nw = (int)(gridDim.x / kdiv);
-    const int krank = (p.ks == 2) ? (int)(crank / CG) : 0;
+    const int krank = (p.ks > 1) ? (int)(crank / CG) : 0;
     uint64_t* rec = (threadIdx.x == 0) ? trace_begin(tr, KID_GEMM) : nullptr;
 
     if (warp == 0 && lane == 0) {
@@ -547,7 +546,7 @@ gemm_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constant__ CU
             mbar_init(tempty_bar(b), 4 * CG);     // one arrive per epilogue warp of the pair
         }
         mbar_init(ks_ready_bar, 4);               // one arrive per epilogue warp of CTA 0
-        mbar_init(ks_data_bar, kEpiThreads);      // every epilogue thread of CTA 1 releases its own writes
+        mbar_init(ks_data_bar, (p.ks > 1 ? p.ks - 1 : 1) * kEpiThreads);   // every epilogue thread of every sender releases its writes
         mbar_fence_init();
     }
     if (warp == 1) {
@@ -562,7 +561,7 @@ gemm_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constant__ CU
         }
     }
     tc_fence_before();
-    if (CG == 2 || p.ks == 2) cluster_sync_all(); // the peer's barriers exist before anything remote touches them
+    if (CG == 2 || p.ks > 1) cluster_sync_all();  // the peer's barriers exist before anything remote touches them
     else __syncthreads();
     tc_fence_after();
     const uint32_t tmem_base = *reinterpret_cast<volatile uint32_t*>(smem_gen + (tmem_slot - smem_base));
@@ -704,19 +703,22 @@ gemm_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constant__ CU
             tile_xy(p, sg.tile, tx, ty);
             const bool whole = (sg.kb0 == 0 && sg.kb1 == p.kb_per_tile);
             const int x = tx * kTileX + (int)rank * (kBM * XH) + xl;   // row of X block 0
-            if (XH == 1 && p.ks == 2) {
-                // ---- cluster split-K: each CTA of the pair holds the sum over half of the k-blocks.  CTA 1 writes its
-                // accumulator into CTA 0's (now idle) stage ring through distributed shared memory -- layout
-                // [32-column chunk][row][32 floats], the eight 16-byte pieces of a row XOR-swizzled by (row & 7) so that
-                // neither side has bank conflicts -- and CTA 0 adds its own half FIRST (k ascending), applies alpha/beta
-                // and stores.  One hand-over per tile, no global-memory round trip, bit-reproducible.
+            if (XH == 1 && p.ks > 1) {
+                // ---- cluster split-K: part r of the cluster holds the sum over the r-th slice of the k-blocks.  Parts
+                // 1 .. ks-1 write their accumulators into part 0's (now idle) stage ring through distributed shared
+                // memory -- one slot per sender, layout [32-column chunk][row][32 floats], the eight 16-byte pieces of
+                // a row XOR-swizzled by (row & 7) so that neither side has bank conflicts -- and part 0 adds its own
+                // slice FIRST, then the slots in ascending k, applies alpha/beta and stores.  One hand-over per tile,
+                // no global-memory round trip, bit-reproducible.
                 mbar_wait(tfull_bar(buf), aphase);
                 tc_fence_after();
                 const uint32_t taddr = tmem_base + ((uint32_t)(quarter * 32) << 16) + (uint32_t)(buf * BN);
                 const uint32_t sw = (uint32_t)(xl & 7);
-                if (krank == 1) {
-                    mbar_wait_acquire_cluster(ks_ready_bar, 0);                // CTA 0's MMAs no longer read its stages
-                    const uint32_t dst0 = mapa(smem_base, crank - CG);         // same CTA of the pair / tile, k-half 0
+                constexpr uint32_t kSlotBytes = (uint32_t)kBM * BN * 4;
+                if (krank >= 1) {
+                    mbar_wait_acquire_cluster(ks_ready_bar, 0);                // part 0's MMAs no longer read its stages
+                    const uint32_t home = crank - (uint32_t)krank * CG;        // same CTA of the pair / tile, k-slice 0
+                    const uint32_t dst0 = mapa(smem_base, home) + (uint32_t)(krank - 1) * kSlotBytes;
 #pragma unroll 1
                     for (int c = 0; c < BN / 32; ++c) {
                         uint32_t v[32];
@@ -727,26 +729,32 @@ gemm_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constant__ CU
                         for (int q = 0; q < 8; ++q)
                             st_cluster_v4(drow + (((uint32_t)q ^ sw) << 4), v[4 * q], v[4 * q + 1], v[4 * q + 2], v[4 * q + 3]);
                     }
-                    mbar_arrive_release_cluster(mapa(ks_data_bar, crank - CG));
+                    mbar_arrive_release_cluster(mapa(ks_data_bar, home));
                 } else {
                     __syncwarp();
-                    if (lane == 0) mbar_arrive_release_cluster(mapa(ks_ready_bar, crank + CG));
+                    if (lane == 0)
+                        for (int r = 1; r < p.ks; ++r) mbar_arrive_release_cluster(mapa(ks_ready_bar, crank + (uint32_t)r * CG));
                     mbar_wait_acquire_cluster(ks_data_bar, 0);
 #pragma unroll 1
                     for (int c = 0; c < BN / 32; ++c) {
                         uint32_t v[32];
                         tmem_ld32(taddr + c * 32, v);
                         tmem_ld_wait();
-                        const uint32_t srow = smem_base + (uint32_t)((c * kBM + xl) * 128);
                         float acc[32];
 #pragma unroll
-                        for (int q = 0; q < 8; ++q) {
-                            uint32_t a, b, cc, d;
-                            ld_shared_v4(srow + (((uint32_t)q ^ sw) << 4), a, b, cc, d);
-                            acc[4 * q + 0] = __fadd_rn(__uint_as_float(v[4 * q + 0]), __uint_as_float(a));
-                            acc[4 * q + 1] = __fadd_rn(__uint_as_float(v[4 * q + 1]), __uint_as_float(b));
-                            acc[4 * q + 2] = __fadd_rn(__uint_as_float(v[4 * q + 2]), __uint_as_float(cc));
-                            acc[4 * q + 3] = __fadd_rn(__uint_as_float(v[4 * q + 3]), __uint_as_float(d));
+                        for (int j = 0; j < 32; ++j) acc[j] = __uint_as_float(v[j]);
+#pragma unroll 1
+                        for (int r = 1; r < p.ks; ++r) {                       // slots in ascending k
+                            const uint32_t srow = smem_base + (uint32_t)(r - 1) * kSlotBytes + (uint32_t)((c * kBM + xl) * 128);
+#pragma unroll
+                            for (int q = 0; q < 8; ++q) {
+                                uint32_t a, b, cc, d;
+                                ld_shared_v4(srow + (((uint32_t)q ^ sw) << 4), a, b, cc, d);
+                                acc[4 * q + 0] = __fadd_rn(acc[4 * q + 0], __uint_as_float(a));
+                                acc[4 * q + 1] = __fadd_rn(acc[4 * q + 1], __uint_as_float(b));
+                                acc[4 * q + 2] = __fadd_rn(acc[4 * q + 2], __uint_as_float(cc));
+                                acc[4 * q + 3] = __fadd_rn(acc[4 * q + 3], __uint_as_float(d));
+                            }
                         }
                         store_out(p, acc, x, ty * BN + c * 32);
                     }
@@ -894,7 +902,7 @@ gemm_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constant__ CU
 
     // teardown: nobody may exit (or free TMEM) while the peer can still signal its barriers / read its stages
     tc_fence_before();
-    if (CG == 2 || p.ks == 2) cluster_sync_all();
+    if (CG == 2 || p.ks > 1) cluster_sync_all();
     else __syncthreads();
     if (warp == 1) {
         tc_fence_after();
@@ -1016,7 +1024,7 @@ static ra_status make_plan(int transA, int transB, int M, int N, int K, const ra
     // serial tail (TMEM drain + stores, ~0.45 us per 64-column box per warp) shrinks with the tile; operand re-use per
     // byte is worse but nothing is bandwidth-bound at this size (1024^3: 13 us with 256 x 256 pair tiles on 32 CTAs).
     bool one_wave = false;
-    if (!swap && occ.cta_group != 2 && occ.m_blocks != 2 && occ.tiles_per_cta == 0 && occ.cluster_k != 2) {
+    if (!swap && occ.cta_group != 2 && occ.m_blocks != 2 && occ.tiles_per_cta == 0 && occ.cluster_k < 2) {
         const long long tx1 = (RX + kBM - 1) / kBM;
         // the alternative for mid-size problems with a long K: 256 x 256 pair tiles with the K range split over two
         // pairs of a 4-CTA cluster (half the L2->SM bytes per flop of a narrow single-CTA tile).  Cycle estimates per
@@ -1038,7 +1046,7 @@ static ra_status make_plan(int transA, int transB, int M, int N, int K, const ra
     }
     if (occ.cta_group < 0 || occ.cta_group > 2) return RA_ERR_INVALID_ARG;
     if (occ.m_blocks < 0 || occ.m_blocks > 2) return RA_ERR_INVALID_ARG;
-    if (occ.cluster_k < 0 || occ.cluster_k > 2) return RA_ERR_INVALID_ARG;
+    if (occ.cluster_k < 0 || occ.cluster_k > 4 || occ.cluster_k == 3) return RA_ERR_INVALID_ARG;
 
     // shared memory the GEMM may allocate on an SM
     long avail = (long)smem_per_sm - occ.smem_reserve_bytes - reserved;
@@ -1116,7 +1124,7 @@ static ra_status make_plan(int transA, int transB, int M, int N, int K, const ra
         // bounded work: more CTAs than SMs.  Residency must stay at one GEMM CTA per SM (TMEM holds
         // two accumulators), so pad the request past half of what an SM can give.
         grid = cg * (int)((n_tiles + occ.tiles_per_cta - 1) / occ.tiles_per_cta);
-        if (occ.cluster_k == 2) {                 // cluster split-K is a one-tile-per-cluster schedule
+        if (occ.cluster_k >= 2) {                 // cluster split-K is a one-tile-per-cluster schedule
             if (!occ.allow_clamp) return RA_ERR_INFEASIBLE_KNOB;
             clamped = 1;
         }
@@ -1142,12 +1150,16 @@ static ra_status make_plan(int transA, int transB, int M, int N, int K, const ra
         // and hands one accumulator over through distributed shared memory -- twice the CTAs streaming operands and
         // no global-memory partials, counters or memset.  Taken when it fills at least half of the budgeted SMs (below
         // that stream-K's finer split wins) and the receiving stage ring can hold a 128 x BN fp32 accumulator.
-        const bool ks_fits = xh == 1 && n_tiles > 0 && 2 * n_tiles <= workers && kb >= 2 &&
-                             (long)stages * stage_bytes(bn, cg, 1) >= (long)kBM * bn * 4;
-        if (ks_fits && occ.cluster_k != 1 && ((kb >= 16 && 4 * n_tiles >= workers) || occ.cluster_k == 2)) {
+        const long ring = (long)stages * stage_bytes(bn, cg, 1), slot = (long)kBM * bn * 4;
+        const bool ks2_fits = xh == 1 && n_tiles > 0 && 2 * n_tiles <= workers && kb >= 2 && ring >= slot;
+        const bool ks4_fits = xh == 1 && cg == 1 && n_tiles > 0 && 4 * n_tiles <= workers && kb >= 4 && ring >= 3 * slot;
+        if (ks4_fits && occ.cluster_k != 1 && occ.cluster_k != 2 && (kb >= 32 || occ.cluster_k == 4)) {
+            ks = 4;                                   // four single-CTA parts per tile, three slots in part 0's ring
+            w = (int)(4 * n_tiles);
+        } else if (ks2_fits && occ.cluster_k != 1 && occ.cluster_k != 4 && (kb >= 16 || occ.cluster_k == 2)) {
             ks = 2;
             w = (int)(2 * n_tiles);                   // workers: CTAs, or CTA pairs (4-CTA clusters)
-        } else if (occ.cluster_k == 2) {
+        } else if (occ.cluster_k >= 2) {
             if (!occ.allow_clamp) return RA_ERR_INFEASIBLE_KNOB;
             clamped = 1;
         }

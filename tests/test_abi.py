@@ -90,7 +90,9 @@ def test_cluster_split_k_plans(ra):
     assert ra.ra_gemm_workspace_bytes(0, 1, 8192, 64, 8192) == 0
     assert ra.ra_gemm_plan_query(0, 1, 8192, 64, 8192, dict(cluster_k=1))["cluster_k"] == 1
     # not available for CTA-pair tiles or in bounded-work mode: clamped, or refused without allow_clamp
-    for occ in (dict(cluster_k=2, cta_group=2), dict(cluster_k=2, tiles_per_cta=1)):
+    p4 = ra.ra_gemm_plan_query(0, 1, 128, 1024, 16384)               # 8 weight tiles, 256 k-blocks: four parts per tile
+    assert p4["cluster_k"] == 4 and p4["grid"] == 32 and ra.ra_gemm_workspace_bytes(0, 1, 128, 1024, 16384) == 0
+    for occ in (dict(cluster_k=2, m_blocks=2), dict(cluster_k=2, tiles_per_cta=1)):
         q = ra.ra_gemm_plan_query(0, 1, 2048, 2048, 2048, occ)
         assert q["cluster_k"] == 1 and q["clamped"] == 1, q
         with pytest.raises(ra.RaError) as e:

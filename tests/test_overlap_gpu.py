@@ -248,16 +248,19 @@ def test_graph_replay_matches_oracle_and_streams(ra):
     """use_graph: first call captures + runs, later calls replay the cached graph; the in-place allreduce and the
     stream-K GEMM (memset node + workspace) must behave exactly as the stream schedule does."""
     import torch
-    M, N, K = 64, 4096, 8192                       # stream-K plan (workspace, counter memset)
+    M, N, K = 64, 4096, 8192                       # stream-K plan (workspace, counter memset) once cluster split-K is off
+    sk = dict(cluster_k=1)
     A, B, g, dC = _gemm_side(ra, M, N, K, 123)
-    assert ra.ra_gemm_plan_query(0, 1, M, N, K)["split_k"] > 1
+    import torch as _t
+    g["workspace"] = _t.empty(ra.ra_gemm_workspace_bytes(0, 1, M, N, K, sk), dtype=_t.uint8, device="cuda")
+    assert ra.ra_gemm_plan_query(0, 1, M, N, K, sk)["split_k"] > 1
     bufs = [ra_inputs.uniform_f32(100003, 123, ra_inputs.STREAM_AR + r) for r in range(3)]
     n_iters, calls = 3, 3
     ref_bufs = [b.copy() for b in bufs]
     oracle.overlap_replay(n_iters * calls, ar_bufs=ref_bufs)
     dev = [to_dev(b) for b in bufs]
     w, keep = ra.make_workload(gemm=g, allreduce=dev, n_iters=n_iters)
-    cfg = ra.make_cfg(mode=1, prio_comm=ra.ra_device_info()["prio_greatest"], use_graph=1)
+    cfg = ra.make_cfg(mode=1, prio_comm=ra.ra_device_info()["prio_greatest"], use_graph=1, occ=sk)
     outs = []
     for _ in range(calls):
         dC.fill_(0x7FC0)
@@ -267,7 +270,7 @@ def test_graph_replay_matches_oracle_and_streams(ra):
     for d, r in zip(dev, ref_bufs):
         assert to_host(d, np.float32).tobytes() == r.tobytes()
     dC.fill_(0x7FC0)
-    ra.ra_overlap_run(w, ra.make_cfg(mode=1))      # plain streams
+    ra.ra_overlap_run(w, ra.make_cfg(mode=1, occ=sk))      # plain streams
     plain = to_host(dC, np.uint16)
     assert all(np.array_equal(o, plain) for o in outs)
     ref, _ = oracle.gemm(0, 1, M, N, K, 1.0, A, B)

@@ -243,12 +243,13 @@ def test_knobs_do_not_change_results(ra, occ, M, N, K):
 
 def test_run_to_run_reproducible_stream_k(ra):
     M, N, K = 64, 4096, 8192
-    assert ra.ra_gemm_plan_query(0, 1, M, N, K)["split_k"] > 1
+    sk = dict(cluster_k=1)                                   # without cluster split-K this shape is a stream-K plan
+    assert ra.ra_gemm_plan_query(0, 1, M, N, K, sk)["split_k"] > 1
     A = ra_inputs.normal_bf16((M, K), 21, ra_inputs.STREAM_A)
     B = ra_inputs.normal_bf16((N, K), 21, ra_inputs.STREAM_B)
-    first, _ = run_gemm(ra, M, N, K, A, B)
+    first, _ = run_gemm(ra, M, N, K, A, B, occ=sk)
     for _ in range(5):
-        again, _ = run_gemm(ra, M, N, K, A, B)
+        again, _ = run_gemm(ra, M, N, K, A, B, occ=sk)
         assert np.array_equal(first, again)
 
 
@@ -420,3 +421,21 @@ def test_pair_cluster_split_k_auto_exact_and_reproducible(ra):
     ref, _ = oracle.gemm(0, 1, M, N, K, 1.0, An, Bn)
     rowA, colB = oracle.gemm_norms(0, 1, M, N, K, An, Bn)
     assert gemm_norm_err(first, ref, rowA, colB) <= GEMM_TOL
+
+
+@pytest.mark.parametrize("M,N,K", [(200, 128, 8192), (130, 100, 1000), (128, 64, 256), (64, 1024, 2048), (17, 640, 1536),
+                                   (257, 120, 336), (128, 1024, 4096)])
+def test_cluster_split_k_four_parts(ra, M, N, K):
+    occ = dict(cluster_k=4, cta_group=1)
+    plan = ra.ra_gemm_plan_query(0, 1, M, N, K, occ)
+    assert plan["cluster_k"] == 4 and plan["split_k"] == 1 and plan["grid"] == 4 * plan["n_tiles"], plan
+    assert ra.ra_gemm_workspace_bytes(0, 1, M, N, K, occ) == 0
+    check(ra, M, N, K, seed=8600 + M + N + K, occ=occ)
+    check(ra, M, N, K, seed=8700 + M + N + K, alpha=-0.5, beta=2.0, occ=occ, transA=1, transB=0)
+    A = ra_inputs.smallint_bf16((M, K), 81, ra_inputs.STREAM_A)
+    B = ra_inputs.smallint_bf16((N, K), 81, ra_inputs.STREAM_B)
+    _, ref16 = oracle.gemm(0, 1, M, N, K, 1.0, A, B)
+    got, _ = run_gemm(ra, M, N, K, A, B, occ=occ, ldc=(N + 7) // 8 * 8)
+    assert np.array_equal(got, ref16)                          # integer inputs: exact whatever the association
+    again, _ = run_gemm(ra, M, N, K, A, B, occ=occ, ldc=(N + 7) // 8 * 8)
+    assert np.array_equal(got, again)
