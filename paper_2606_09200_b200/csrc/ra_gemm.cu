@@ -245,6 +245,11 @@ __device__ __forceinline__ void st_cluster_v4(uint32_t addr_cluster, uint32_t a,
 __device__ __forceinline__ void ld_shared_v4(uint32_t addr, uint32_t& a, uint32_t& b, uint32_t& c, uint32_t& d) {
     asm volatile("ld.shared.v4.b32 {%0, %1, %2, %3}, [%4];" : "=r"(a), "=r"(b), "=r"(c), "=r"(d) : "r"(addr) : "memory");
 }
+// bulk copy local shared memory -> another CTA's shared memory, completing `bytes` on that CTA's mbarrier
+__device__ __forceinline__ void dsmem_bulk_copy(uint32_t dst_cluster, uint32_t src_cta, uint32_t bytes, uint32_t bar_cluster) {
+    asm volatile("cp.async.bulk.shared::cluster.shared::cta.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(dst_cluster), "r"(src_cta), "r"(bytes), "r"(bar_cluster) : "memory");
+}
 // arrive on a barrier of another CTA of the cluster, releasing this thread's prior (distributed) shared-memory writes
 __device__ __forceinline__ void mbar_arrive_release_cluster(uint32_t bar_cluster) {
     asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(bar_cluster) : "memory");
@@ -546,7 +551,7 @@ gemm_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constant__ CU
             mbar_init(tempty_bar(b), 4 * CG);     // one arrive per epilogue warp of the pair
         }
         mbar_init(ks_ready_bar, 4);               // one arrive per epilogue warp of CTA 0
-        mbar_init(ks_data_bar, (p.ks > 1 ? p.ks - 1 : 1) * kEpiThreads);   // every epilogue thread of every sender releases its writes
+        mbar_init(ks_data_bar, 1);                // one arrive.expect_tx by part 0; the senders' bulk copies complete the bytes
         mbar_fence_init();
     }
     if (warp == 1) {
@@ -705,35 +710,41 @@ gemm_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constant__ CU
             const int x = tx * kTileX + (int)rank * (kBM * XH) + xl;   // row of X block 0
             if (XH == 1 && p.ks > 1) {
                 // ---- cluster split-K: part r of the cluster holds the sum over the r-th slice of the k-blocks.  Parts
-                // 1 .. ks-1 write their accumulators into part 0's (now idle) stage ring through distributed shared
-                // memory -- one slot per sender, layout [32-column chunk][row][32 floats], the eight 16-byte pieces of
-                // a row XOR-swizzled by (row & 7) so that neither side has bank conflicts -- and part 0 adds its own
-                // slice FIRST, then the slots in ascending k, applies alpha/beta and stores.  One hand-over per tile,
-                // no global-memory round trip, bit-reproducible.
+                // 1 .. ks-1 stage their accumulators in their OWN (now idle) stage ring -- layout [32-column chunk][row]
+                // [32 floats], the eight 16-byte pieces of a row XOR-swizzled by (row & 7) against bank conflicts -- and
+                // ship them with one bulk copy each through distributed shared memory into a slot of part 0's ring
+                // (register -> remote st.shared measured 6-7 us per 128 KiB accumulator; the bulk copy is asynchronous
+                // and completes bytes on part 0's mbarrier).  Part 0 adds its own slice FIRST, then the slots in
+                // ascending k, applies alpha/beta and stores.  No global-memory round trip, bit-reproducible.
                 mbar_wait(tfull_bar(buf), aphase);
                 tc_fence_after();
                 const uint32_t taddr = tmem_base + ((uint32_t)(quarter * 32) << 16) + (uint32_t)(buf * BN);
                 const uint32_t sw = (uint32_t)(xl & 7);
                 constexpr uint32_t kSlotBytes = (uint32_t)kBM * BN * 4;
                 if (krank >= 1) {
-                    mbar_wait_acquire_cluster(ks_ready_bar, 0);                // part 0's MMAs no longer read its stages
                     const uint32_t home = crank - (uint32_t)krank * CG;        // same CTA of the pair / tile, k-slice 0
-                    const uint32_t dst0 = mapa(smem_base, home) + (uint32_t)(krank - 1) * kSlotBytes;
 #pragma unroll 1
                     for (int c = 0; c < BN / 32; ++c) {
                         uint32_t v[32];
                         tmem_ld32(taddr + c * 32, v);
                         tmem_ld_wait();
-                        const uint32_t drow = dst0 + (uint32_t)((c * kBM + xl) * 128);
+                        const uint32_t drow = smem_base + (uint32_t)((c * kBM + xl) * 128);   // own ring: the MMAs are done
 #pragma unroll
                         for (int q = 0; q < 8; ++q)
-                            st_cluster_v4(drow + (((uint32_t)q ^ sw) << 4), v[4 * q], v[4 * q + 1], v[4 * q + 2], v[4 * q + 3]);
+                            st_shared_v4(drow + (((uint32_t)q ^ sw) << 4), v[4 * q], v[4 * q + 1], v[4 * q + 2], v[4 * q + 3]);
                     }
-                    mbar_arrive_release_cluster(mapa(ks_data_bar, home));
+                    fence_async_smem();
+                    epi_bar_sync();
+                    if (et == 0) {
+                        mbar_wait_acquire_cluster(ks_ready_bar, 0);            // part 0's MMAs no longer read its stages
+                        dsmem_bulk_copy(mapa(smem_base, home) + (uint32_t)(krank - 1) * kSlotBytes, smem_base, kSlotBytes,
+                                        mapa(ks_data_bar, home));
+                    }
                 } else {
                     __syncwarp();
                     if (lane == 0)
                         for (int r = 1; r < p.ks; ++r) mbar_arrive_release_cluster(mapa(ks_ready_bar, crank + (uint32_t)r * CG));
+                    if (et == 0) mbar_expect_tx(ks_data_bar, (uint32_t)(p.ks - 1) * kSlotBytes);
                     mbar_wait_acquire_cluster(ks_data_bar, 0);
 #pragma unroll 1
                     for (int c = 0; c < BN / 32; ++c) {
