@@ -7,7 +7,7 @@
 //   t_bytes     = (gemm_bytes + coll_bytes) / hbm_peak                     both kernels share HBM
 //   t_overlap(b) = max(t_tensor(b), t_bytes)                               per pipelined iteration
 //   t_step       = (t_gemm_alone + (n-1) * t_overlap + t_coll_alone) / n   K_g^0 and K_c^{n-1} have no partner
-// What the B200 sweeps showed and the model encodes (profiles/r01c_sweeps.md):
+// What the B200 sweeps showed and the model encodes (profiles/r01d_sweeps.md):
 //   * the collective stand-ins need no shared memory (allreduce, LDG alltoall) or 64 KiB (TMA alltoall) and
 //     <= 64 registers/thread, and the tcgen05 GEMM is one 192-thread CTA of 128 registers per SM, so they
 //     co-reside on every SM without any reserve: constraining the GEMM's SM budget only costs tensor time.
