@@ -251,3 +251,24 @@ def test_policy_errors(ra):
     import ctypes
     lib = ctypes.CDLL(ra.lib_path())
     assert lib.ra_overlap_suggest(None, None, None) == ra.RA_ERR_INVALID_ARG
+
+
+def test_header_is_plain_c_and_links_from_c(ra, tmp_path):
+    """include/ra.h is the boundary: it must compile as C99 without any CUDA or C++ header, and a plain C program
+    linked against libra.so must be able to call the host-only entry points."""
+    import subprocess
+    src = tmp_path / "use_ra.c"
+    src.write_text(
+        '#include "ra.h"\n#include <stdio.h>\n'
+        "int main(void) {\n"
+        "  ra_gemm_plan p; ra_occupancy o = {0, 0, 0, 1, 0, 0, 0};\n"
+        "  if (ra_gemm_plan_query(0, 1, 8192, 8192, 8192, &o, &p) != RA_OK) return 1;\n"
+        '  printf("%d %d %d %s\\n", p.tile_m, p.tile_n, p.grid, ra_status_str(RA_ERR_ARCH));\n'
+        "  return ra_gemm_plan_query(0, 1, 8, 8, 8, &o, (ra_gemm_plan*)0) == RA_ERR_INVALID_ARG ? 0 : 2;\n"
+        "}\n")
+    exe = tmp_path / "use_ra"
+    libdir = os.path.dirname(ra.lib_path())
+    subprocess.check_call(["gcc", "-std=c99", "-Wall", "-Werror", "-pedantic", "-I", os.path.join(ROOT, "include"), str(src),
+                           "-o", str(exe), "-L", libdir, "-l:libra.so", "-Wl,-rpath," + libdir])
+    out = subprocess.check_output([str(exe)]).decode().split()
+    assert out == ["512", "256", "148", "RA_ERR_ARCH"]
