@@ -272,3 +272,42 @@ def test_header_is_plain_c_and_links_from_c(ra, tmp_path):
                            "-o", str(exe), "-L", libdir, "-l:libra.so", "-Wl,-rpath," + libdir])
     out = subprocess.check_output([str(exe)]).decode().split()
     assert out == ["512", "256", "148", "RA_ERR_ARCH"]
+
+
+# ---- planner invariants over random shapes and knobs (host only) -------------------------------------------------
+def test_planner_invariants_random(ra):
+    from hypothesis import given, settings, strategies as st
+
+    dims = st.one_of(st.integers(1, 300), st.sampled_from([64, 128, 256, 512, 1024, 4096, 8192, 16384, 57344]))
+    occs = st.fixed_dictionaries(dict(
+        smem_reserve_bytes=st.sampled_from([0, 0, 0, 32 * KB, 64 * KB, 96 * KB, 128 * KB, 160 * KB, 200 * KB]),
+        sm_budget=st.sampled_from([0, 0, 0, 1, 2, 9, 33, 74, 92, 110, 128, 140, 148]),
+        tiles_per_cta=st.sampled_from([0, 0, 0, 1, 2, 4]), cta_group=st.sampled_from([0, 0, 1, 2]),
+        m_blocks=st.sampled_from([0, 0, 1, 2]), cluster_k=st.sampled_from([0, 0, 1, 2, 4])))
+
+    @settings(max_examples=400, deadline=None)
+    @given(dims, dims, dims, st.integers(0, 1), st.integers(0, 1), occs)
+    def prop(M, N, K, tA, tB, occ):
+        p = ra.ra_gemm_plan_query(tA, tB, M, N, K, occ)          # allow_clamp = 1: never refuses a valid shape
+        budget = occ["sm_budget"] or 148
+        assert p["grid"] >= 1 and p["stages"] >= 1 and p["tile_k"] == 64
+        assert p["dyn_smem_bytes"] <= 227 * KB
+        assert p["clamped"] or p["smem_left_per_sm"] >= occ["smem_reserve_bytes"], p
+        assert p["n_tiles"] == -(-M // p["tile_m"]) * -(-N // p["tile_n"]), p
+        assert p["cta_group"] in (1, 2) and p["m_blocks"] in (1, 2) and p["cluster_k"] in (1, 2, 4)
+        if p["m_blocks"] == 2:
+            assert p["cta_group"] == 2 and p["tile_m"] == 512
+        per_tile = p["cta_group"] * p["cluster_k"]
+        assert p["grid"] % per_tile == 0
+        if occ["tiles_per_cta"] == 0:
+            assert p["grid"] <= budget or p["clamped"], p            # persistent: at most one CTA per budgeted SM
+        if p["cluster_k"] > 1:
+            assert p["grid"] == per_tile * p["n_tiles"] and p["split_k"] == 1, p
+        ws = ra.ra_gemm_workspace_bytes(tA, tB, M, N, K, occ)
+        assert (ws > 0) == (p["split_k"] > 1), p
+        if occ["cta_group"] == 1:
+            assert p["cta_group"] == 1
+        if occ["cluster_k"] == 1:
+            assert p["cluster_k"] == 1
+
+    prop()

@@ -112,13 +112,14 @@ def test_alltoall_writes_stay_inside_recv(ra, variant, P, chunk):
 
 
 def test_gemm_fuzz_shapes_layouts_knobs(ra):
-    """Seeded fuzz: 48 random problems over all four (transA, transB), ragged sizes, alpha/beta and planner knobs."""
+    """Seeded fuzz: 72 random problems over all four (transA, transB), ragged sizes, alpha/beta and planner knobs."""
     rng = np.random.default_rng(20260609)
     sizes = [1, 7, 8, 63, 64, 65, 127, 128, 129, 200, 255, 256, 257, 384, 511, 512, 520, 777, 1024, 1100]
     ks = [8, 24, 64, 72, 136, 512, 1000, 2048]
     knobs = [None, dict(cta_group=1), dict(cta_group=2), dict(cta_group=2, m_blocks=2), dict(sm_budget=9),
-             dict(smem_reserve_bytes=96 * 1024), dict(tiles_per_cta=2), dict(sm_budget=33, smem_reserve_bytes=160 * 1024)]
-    for case in range(48):
+             dict(smem_reserve_bytes=96 * 1024), dict(tiles_per_cta=2), dict(sm_budget=33, smem_reserve_bytes=160 * 1024),
+             dict(cluster_k=2), dict(cluster_k=4), dict(cta_group=2, m_blocks=1, cluster_k=2), dict(cluster_k=1)]
+    for case in range(72):
         M, N = int(rng.choice(sizes)), int(rng.choice(sizes))
         K = int(rng.choice(ks))
         tA, tB = int(rng.integers(0, 2)), int(rng.integers(0, 2))
