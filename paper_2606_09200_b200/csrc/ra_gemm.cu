@@ -1034,6 +1034,11 @@ static ra_status make_plan(int transA, int transB, int M, int N, int K, const ra
     // Small problems: when narrower tiles still fit in ONE wave, take them -- more CTAs share the work and each CTA's
     // serial tail (TMEM drain + stores, ~0.45 us per 64-column box per warp) shrinks with the tile; operand re-use per
     // byte is worse but nothing is bandwidth-bound at this size (1024^3: 13 us with 256 x 256 pair tiles on 32 CTAs).
+    // Clusters of 4 CTAs cannot use every SM: cudaOccupancyMaxActiveClusters reports 33 of them (132 SMs) on B200 with
+    // this kernel's shared memory (74 clusters of 2 = all 148 SMs; 15 of 8) -- GPC sizes are not multiples of 4.  One-wave
+    // cluster plans are held to that count, scaled by the SM budget.  (It is also why the big-tile GEMM does not share
+    // its Y tile between two pairs by TMA multicast: 11 % of the SMs would idle.)
+    const int max_clusters4 = 33 * budget / sm_count;
     bool one_wave = false;
     if (!swap && occ.cta_group != 2 && occ.m_blocks != 2 && occ.tiles_per_cta == 0 && occ.cluster_k < 2) {
         const long long tx1 = (RX + kBM - 1) / kBM;
@@ -1044,7 +1049,7 @@ static ra_status make_plan(int transA, int transB, int M, int N, int K, const ra
         if (bn == 256 && RX >= 2 * kBM && occ.cta_group != 1 && occ.cluster_k != 1 && kb >= 16) {
             const long long T = (long long)((RX + 2 * kBM - 1) / (2 * kBM)) * ((RY + 255) / 256);
             const int pairs = budget / 2;
-            if (2 * T <= pairs && 4 * T >= pairs) pair_ks_cost = (long long)(kb / 2) * 512 + 4096;
+            if (2 * T <= pairs && 4 * T >= pairs && T <= max_clusters4) pair_ks_cost = (long long)(kb / 2) * 512 + 4096;
         }
         for (int cand = 64; cand < bn; cand <<= 1) {
             if (tx1 * ((RY + cand - 1) / cand) <= budget) {
@@ -1162,8 +1167,11 @@ static ra_status make_plan(int transA, int transB, int M, int N, int K, const ra
         // no global-memory partials, counters or memset.  Taken when it fills at least half of the budgeted SMs (below
         // that stream-K's finer split wins) and the receiving stage ring can hold a 128 x BN fp32 accumulator.
         const long ring = (long)stages * stage_bytes(bn, cg, 1), slot = (long)kBM * bn * 4;
-        const bool ks2_fits = xh == 1 && n_tiles > 0 && 2 * n_tiles <= workers && kb >= 2 && ring >= slot;
-        const bool ks4_fits = xh == 1 && cg == 1 && n_tiles > 0 && 4 * n_tiles <= workers && kb >= 4 && ring >= 3 * slot;
+        // 4-CTA clusters (four single-CTA parts, or two CTA pairs) must also fit the chip's cluster capacity
+        const bool ks2_fits = xh == 1 && n_tiles > 0 && 2 * n_tiles <= workers && kb >= 2 && ring >= slot &&
+                              (cg == 1 || n_tiles <= max_clusters4);
+        const bool ks4_fits = xh == 1 && cg == 1 && n_tiles > 0 && 4 * n_tiles <= workers && kb >= 4 && ring >= 3 * slot &&
+                              n_tiles <= max_clusters4;
         if (ks4_fits && occ.cluster_k != 1 && occ.cluster_k != 2 && (kb >= 32 || occ.cluster_k == 4)) {
             ks = 4;                                   // four single-CTA parts per tile, three slots in part 0's ring
             w = (int)(4 * n_tiles);
