@@ -257,11 +257,12 @@ static ra_status run_host(const ra_workload* const* dev, int n_sets, const ra_ho
     else s_comm = s_comp;
     RA_TRY(get_stream(2, 0, &s_h2d));
     RA_TRY(get_stream(3, 0, &s_d2h));
-    // dep events: [0, n] per-iteration + join (enqueue_step), then 3 per buffer set
-    RA_TRY(ensure_events(g_cache.dep_events, (size_t)n + 2 + 3 * (size_t)n_sets, cudaEventDisableTiming));
+    // dep events: [0, n] per-iteration + join (enqueue_step), then 4 per buffer set
+    RA_TRY(ensure_events(g_cache.dep_events, (size_t)n + 2 + 4 * (size_t)n_sets, cudaEventDisableTiming));
     RA_TRY(ensure_events(g_cache.timed_events, 2, cudaEventDefault));
     cudaEvent_t ev_start = g_cache.timed_events[0], ev_end = g_cache.timed_events[1];
-    auto set_ev = [&](int k, int which) { return g_cache.dep_events[(size_t)n + 2 + 3 * (size_t)k + which]; };   // 0 h2d, 1 compute, 2 d2h
+    // per set: 0 GEMM operands on the device, 1 compute done, 2 d2h done, 3 collective inputs on the device
+    auto set_ev = [&](int k, int which) { return g_cache.dep_events[(size_t)n + 2 + 4 * (size_t)k + which]; };
 
     ra_gemm_plan plan{};
     RA_CUDA(cudaEventRecord(ev_start, s_h2d));
@@ -270,19 +271,22 @@ static ra_status run_host(const ra_workload* const* dev, int n_sets, const ra_ho
         const ra_workload* w = dev[k];
         // the set is free once the D2H of the step that last used it has finished
         if (s >= n_sets) RA_CUDA(cudaStreamWaitEvent(s_h2d, set_ev(k, 2), 0));
+        // the GEMM's operands go first and release the compute stream on their own: K_g^0 starts while the collective's
+        // buffers (needed only at K_c^0) are still on the wire
         if (has_gemm) {
             RA_CUDA(cudaMemcpyAsync(const_cast<void*>(w->A), io->A, a_bytes(w), cudaMemcpyHostToDevice, s_h2d));
             RA_CUDA(cudaMemcpyAsync(const_cast<void*>(w->B), io->B, b_bytes(w), cudaMemcpyHostToDevice, s_h2d));
         }
+        RA_CUDA(cudaEventRecord(set_ev(k, 0), s_h2d));
+        RA_CUDA(cudaStreamWaitEvent(s_comp, set_ev(k, 0), 0));
         if (w->kind == RA_COLL_ALLREDUCE) {
             for (int r = 0; r < w->P; ++r)
                 RA_CUDA(cudaMemcpyAsync(w->ar_bufs[r], io->ar_in[r], w->ar_count * sizeof(float), cudaMemcpyHostToDevice, s_h2d));
         } else if (w->kind == RA_COLL_ALLTOALL) {
             RA_CUDA(cudaMemcpyAsync(w->a2a_a, io->a2a_in, (size_t)w->P * w->P * w->chunk_bytes, cudaMemcpyHostToDevice, s_h2d));
         }
-        RA_CUDA(cudaEventRecord(set_ev(k, 0), s_h2d));
-        RA_CUDA(cudaStreamWaitEvent(s_comp, set_ev(k, 0), 0));
-        if (overlap) RA_CUDA(cudaStreamWaitEvent(s_comm, set_ev(k, 0), 0));
+        RA_CUDA(cudaEventRecord(set_ev(k, 3), s_h2d));
+        RA_CUDA(cudaStreamWaitEvent(overlap ? s_comm : s_comp, set_ev(k, 3), 0));
         RA_TRY(enqueue_step(w, cfg, s_comp, s_comm, false, &plan));
         RA_CUDA(cudaEventRecord(set_ev(k, 1), s_comp));
         RA_CUDA(cudaStreamWaitEvent(s_d2h, set_ev(k, 1), 0));
