@@ -178,18 +178,17 @@ def sweep_candidates(ra, cfg, quick: bool):
                 # collective on 24-48 SMs that still finishes inside the GEMM's time but disturbs fewer SMs
                 for csb in sorted({0, info["sm_count"] - b} if b < info["sm_count"] else ({0, 24, 32, 48} if r == 0 else {0})):
                     base = dict(mode=1, occ=dict(smem_reserve_bytes=r, sm_budget=b), prio_compute=0, prio_comm=prio, coll_sm_budget=csb)
-                    if cfg.coll == "alltoall":
-                        # TMA ring sized to fit INSIDE the reserve (ring + 1 KiB system + barriers), and the
-                        # shared-memory-free LDG/STG variant, which can co-reside on a full GEMM SM
-                        if r >= 20 * KB:
-                            cands.append(dict(base, coll_variant=0, coll_smem_bytes=min(r - 4 * KB, 64 * KB), coll_ctas_per_sm=1))
-                        elif b < info["sm_count"]:
-                            cands.append(dict(base, coll_variant=0))
-                        cands.append(dict(base, coll_variant=1))
-                        if csb == 0:
-                            cands.append(dict(base, coll_variant=2))     # copy engines: no SM residency at all
-                    else:
-                        cands.append(base)
+                    # both collectives have a shared-memory-free LDG/STG variant (co-resides on a full GEMM SM) and a TMA-ring
+                    # variant whose ring must fit somewhere: INSIDE the reserve (ring + 1 KiB system + barriers) or on SMs
+                    # the GEMM leaves free; the alltoall also has the copy engines (no SM residency at all)
+                    tma, ldg = (0, 1) if cfg.coll == "alltoall" else (1, 0)
+                    if r >= 20 * KB:
+                        cands.append(dict(base, coll_variant=tma, coll_smem_bytes=min(r - 4 * KB, 64 * KB), coll_ctas_per_sm=1))
+                    elif b < info["sm_count"] or cfg.M <= 128:
+                        cands.append(dict(base, coll_variant=tma))
+                    cands.append(dict(base, coll_variant=ldg))
+                    if cfg.coll == "alltoall" and csb == 0:
+                        cands.append(dict(base, coll_variant=2))
     return cands
 
 

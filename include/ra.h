@@ -157,8 +157,14 @@ ra_status ra_gemm_ex(int transA, int transB, int M, int N, int K, float alpha, c
  * sm_budget: SMs' worth of CTAs to launch (0 = all SMs).
  * ------------------------------------------------------------------------------------------- */
 ra_status ra_allreduce_emul(float* const* bufs, int P, size_t count, int sm_budget, void* stream);
-/* Extended form: ctas_per_sm = CTAs (256 threads each) launched per budgeted SM, 1..4 (0 = default 2). */
-ra_status ra_allreduce_emul_ex(float* const* bufs, int P, size_t count, int sm_budget, int ctas_per_sm, void* stream);
+/* Extended form.  variant 0: 128-bit loads/stores from registers, no shared memory; ctas_per_sm = CTAs (256 threads
+ * each) per budgeted SM, 1..4 (0 = default 2).  variant 1: TMA ring -- a thread bulk-copies the P rank slices of a unit
+ * into a shared-memory slot, 128 threads sum them there in the same rank order (bit-identical result), the first slice is
+ * bulk-stored to all P buffers; smem_bytes_per_cta = two slots of P slices (0 = 64 KiB), ctas_per_sm 0 = 2.  This is
+ * the variant whose co-residency with the GEMM depends on smem_reserve_bytes.  (Same argument order as
+ * ra_alltoall_emul_ex.) */
+ra_status ra_allreduce_emul_ex(float* const* bufs, int P, size_t count, int sm_budget, int smem_bytes_per_cta, int ctas_per_sm,
+                               int variant, void* stream);
 
 /* ---------------------------------------------------------------------------------------------
  * S5  Alltoall stand-in   ("expert-parallel workloads rely on alltoall to route
@@ -211,9 +217,9 @@ typedef struct {
     int32_t mode;               /* ra_mode */
     ra_occupancy occ;           /* GEMM knobs */
     int32_t coll_sm_budget;     /* 0 = all SMs */
-    int32_t coll_smem_bytes;    /* alltoall ring bytes per CTA (0 = default) */
+    int32_t coll_smem_bytes;    /* TMA-ring variants: ring bytes per CTA (0 = default 64 KiB) */
     int32_t coll_ctas_per_sm;   /* collective CTAs per budgeted SM; 0 = default */
-    int32_t coll_variant;       /* alltoall: 0 = TMA ring, 1 = LDG/STG, 2 = copy engines */
+    int32_t coll_variant;       /* alltoall: 0 = TMA ring, 1 = LDG/STG, 2 = copy engines;  allreduce: 0 = LDG/STG, 1 = TMA ring */
     int32_t prio_compute, prio_comm; /* cudaStreamCreateWithPriority values; equal = "priority off" */
     int32_t dependent;          /* 1: K_c^i waits for K_g^i (the paper's schedule); 0: free-running streams */
     int32_t record_kernel_times;/* 1: per-kernel event pairs (perturbs the schedule slightly) */

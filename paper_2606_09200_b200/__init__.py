@@ -114,7 +114,7 @@ def _L():
     lib.ra_gemm_ex.argtypes = [c_int, c_int, c_int, c_int, c_int, c_float, c_void_p, c_int, c_void_p, c_int, c_float,
                                c_void_p, c_int, c_int, POINTER(Occupancy), c_void_p, c_size_t, c_void_p]
     lib.ra_allreduce_emul.argtypes = [POINTER(c_void_p), c_int, c_size_t, c_int, c_void_p]
-    lib.ra_allreduce_emul_ex.argtypes = [POINTER(c_void_p), c_int, c_size_t, c_int, c_int, c_void_p]
+    lib.ra_allreduce_emul_ex.argtypes = [POINTER(c_void_p), c_int, c_size_t, c_int, c_int, c_int, c_int, c_void_p]
     lib.ra_alltoall_emul.argtypes = [c_void_p, c_void_p, c_int, c_size_t, c_int, c_void_p]
     lib.ra_alltoall_emul_ex.argtypes = [c_void_p, c_void_p, c_int, c_size_t, c_int, c_int, c_int, c_int, c_void_p]
     lib.ra_overlap_run.argtypes = [POINTER(Workload), POINTER(OverlapCfg), POINTER(OverlapResult)]
@@ -234,12 +234,12 @@ def ra_allreduce_emul(bufs, count=None, sm_budget=0, stream=None) -> None:
     _check(_L().ra_allreduce_emul(arr, len(bufs), int(count), int(sm_budget), _stream(stream)), "ra_allreduce_emul")
 
 
-def ra_allreduce_emul_ex(bufs, count=None, sm_budget=0, ctas_per_sm=0, stream=None) -> None:
+def ra_allreduce_emul_ex(bufs, count=None, sm_budget=0, ctas_per_sm=0, smem_bytes_per_cta=0, variant=0, stream=None) -> None:
     if count is None:
         count = bufs[0].numel()
     arr = _ptr_array(bufs)
-    _check(_L().ra_allreduce_emul_ex(arr, len(bufs), int(count), int(sm_budget), int(ctas_per_sm), _stream(stream)),
-           "ra_allreduce_emul_ex")
+    _check(_L().ra_allreduce_emul_ex(arr, len(bufs), int(count), int(sm_budget), int(smem_bytes_per_cta), int(ctas_per_sm),
+                                     int(variant), _stream(stream)), "ra_allreduce_emul_ex")
 
 
 def ra_alltoall_emul(send, recv, P, chunk_bytes, sm_budget=0, stream=None) -> None:

@@ -19,7 +19,8 @@ namespace ra {
 ra_status gemm_launch(int transA, int transB, int M, int N, int K, float alpha, const void* A, int lda, const void* B,
                       int ldb, float beta, void* C, int ldc, const ra_occupancy* occ, void* workspace,
                       size_t workspace_bytes, cudaStream_t stream, ra_gemm_plan* plan_out, int c_f32);
-ra_status allreduce_launch(float* const* bufs, int P, size_t count, int sm_budget, int ctas_per_sm, cudaStream_t stream);
+ra_status allreduce_launch(float* const* bufs, int P, size_t count, int sm_budget, int ctas_per_sm, int smem_bytes_per_cta,
+                           int variant, cudaStream_t stream);
 ra_status alltoall_launch(const void* send, void* recv, int P, size_t chunk_bytes, int sm_budget,
                           int smem_bytes_per_cta, int ctas_per_sm, int variant, cudaStream_t stream);
 
@@ -65,7 +66,9 @@ static ra_status validate(const ra_workload* w, const ra_overlap_cfg* cfg, ra_ov
 }
 
 static ra_status launch_coll(const ra_workload* w, const ra_overlap_cfg* cfg, int iter, cudaStream_t s) {
-    if (w->kind == RA_COLL_ALLREDUCE) return allreduce_launch(w->ar_bufs, w->P, w->ar_count, cfg->coll_sm_budget, cfg->coll_ctas_per_sm, s);
+    if (w->kind == RA_COLL_ALLREDUCE)
+        return allreduce_launch(w->ar_bufs, w->P, w->ar_count, cfg->coll_sm_budget, cfg->coll_ctas_per_sm, cfg->coll_smem_bytes,
+                                cfg->coll_variant == 1 ? 1 : 0, s);
     if (w->kind == RA_COLL_ALLTOALL) {
         const void* src = (iter & 1) ? w->a2a_b : w->a2a_a;
         void* dst = (iter & 1) ? w->a2a_a : w->a2a_b;

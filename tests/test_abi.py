@@ -211,8 +211,12 @@ def test_policy_rooflines_and_choices(ra):
     assert s["t_gemm_ms"] <= s["t_overlap_ms"] <= s["t_serial_ms"]
     kw = s["kw"]
     assert kw["occ"]["sm_budget"] == 0 and kw["occ"]["smem_reserve_bytes"] == 0 and kw["prio_comm"] == kw["prio_compute"]
+    assert kw["coll_variant"] == 0                              # tensor-bound GEMM: the register allreduce co-resides everywhere
     # the same GEMM fills shared memory, so the alltoall must be the shared-memory-free variant
     w, keep = _workload(ra, 8192, 8192, 8192, "alltoall", 8, chunk=8 << 20)
+    assert ra.ra_overlap_suggest(w, T, H)["kw"]["coll_variant"] == 1
+    # skinny GEMM + allreduce: the TMA-ring allreduce (variant 1) on the SMs the GEMM leaves free
+    w, keep = _workload(ra, 64, 16384, 16384, "allreduce", 8, count=16 << 20)
     assert ra.ra_overlap_suggest(w, T, H)["kw"]["coll_variant"] == 1
     # skinny GEMM: HBM-bound, leaves 20 SMs free -> TMA-ring alltoall; overlap cannot beat total bytes / bandwidth
     w, keep = _workload(ra, 64, 16384, 16384, "alltoall", 8, chunk=8 << 20)

@@ -51,6 +51,7 @@ def _settings(ra, cfg):
     if cfg.M <= 64:
         out.append(dict(mode=1, prio_comm=hi, occ=dict(smem_reserve_bytes=64 * 1024, sm_budget=148)))   # mb-ar winner
         out.append(dict(mode=1, occ=dict(sm_budget=128)))                                # mb-a2a winner
+        out.append(dict(mode=1, prio_comm=hi, occ=dict(sm_budget=140), coll_variant=1))  # mb-ar winner: TMA-ring allreduce
     else:
         out.append(dict(mode=1, occ=dict(smem_reserve_bytes=64 * 1024, sm_budget=128), coll_sm_budget=20))
     return out

@@ -45,6 +45,8 @@ MODES = [
     dict(mode=1, prio_compute=0, prio_comm=-5, use_graph=1),
     dict(mode=1, dependent=0, occ=dict(sm_budget=37), use_graph=1),
     dict(mode=1, coll_variant=2, use_graph=1),                               # copy-engine alltoall = memcpy nodes
+    dict(mode=1, prio_compute=0, prio_comm=-5, coll_variant=1),              # TMA-ring allreduce / LDG alltoall
+    dict(mode=1, coll_variant=1, coll_sm_budget=20, occ=dict(sm_budget=128), use_graph=1),
 ]
 
 

@@ -18,10 +18,13 @@ def ra():
     return m
 
 
-def _run_allreduce(ra, bufs_np, sm_budget=0):
+def _run_allreduce(ra, bufs_np, sm_budget=0, variant=0, smem=0):
     import torch
     dev = [to_dev(b) for b in bufs_np]
-    ra.ra_allreduce_emul(dev, count=bufs_np[0].size, sm_budget=sm_budget)
+    if variant == 0 and smem == 0:
+        ra.ra_allreduce_emul(dev, count=bufs_np[0].size, sm_budget=sm_budget)
+    else:
+        ra.ra_allreduce_emul_ex(dev, count=bufs_np[0].size, sm_budget=sm_budget, smem_bytes_per_cta=smem, variant=variant)
     torch.cuda.synchronize()
     return [to_host(d, np.float32) for d in dev]
 
@@ -39,6 +42,30 @@ def test_allreduce_matches_oracle(ra, P, count):
     got = _run_allreduce(ra, bufs)
     for r in range(P):
         _assert_bits_equal(got[r], ref[r])
+
+
+@pytest.mark.parametrize("P", [1, 2, 3, 8, 16])
+@pytest.mark.parametrize("count", [1, 3, 4, 100, 1000, 65536 + 36, 2 * 148 * 1024 * 3 + 7])
+@pytest.mark.parametrize("smem", [0, 16 * 1024, 200 * 1024])
+def test_allreduce_tma_variant_matches_oracle(ra, P, count, smem):
+    """variant 1 (TMA ring + shared-memory sum): same rank order, so bit-exact too; several slot sizes, ragged tails."""
+    bufs = [ra_inputs.uniform_f32(count, 888 + P, ra_inputs.STREAM_AR + r) for r in range(P)]
+    ref = [b.copy() for b in bufs]
+    oracle.allreduce(ref)
+    got = _run_allreduce(ra, bufs, variant=1, smem=smem)
+    for r in range(P):
+        _assert_bits_equal(got[r], ref[r])
+
+
+def test_allreduce_tma_variant_order_and_denormals(ra):
+    n = 4099
+    bufs = [np.full(n, 2.0 ** 24, np.float32)] + [np.ones(n, np.float32) for _ in range(7)]
+    assert np.all(_run_allreduce(ra, bufs, variant=1)[5] == np.float32(16777216.0))
+    bufs = [np.ones(n, np.float32)] + [np.full(n, 2.0 ** -24, np.float32) for _ in range(7)]
+    assert np.all(_run_allreduce(ra, bufs, variant=1)[0] == np.float32(1.0))
+    tiny = np.float32(2.0 ** -140)
+    bufs = [np.full(n, tiny, np.float32), np.full(n, tiny, np.float32)] + [np.zeros(n, np.float32) for _ in range(2)]
+    assert np.all(_run_allreduce(ra, bufs, variant=1, sm_budget=3)[2] == np.float32(2.0 ** -139))
 
 
 def test_allreduce_order_detectors(ra):

@@ -70,8 +70,9 @@ def test_gemm_writes_stay_inside_c(ra, M, N, K, occ, beta):
     _gemm_with_guards(ra, M, N, K, ldc, occ, beta=beta, alpha=1.0 if beta == 0.0 else 2.0, seed=M + N + K)
 
 
+@pytest.mark.parametrize("variant", [0, 1])
 @pytest.mark.parametrize("P,count", [(1, 5), (3, 4099), (8, 1 << 16), (16, 100003)])
-def test_allreduce_writes_stay_inside_buffers(ra, P, count):
+def test_allreduce_writes_stay_inside_buffers(ra, P, count, variant):
     import torch
     pad = (count + 3) // 4 * 4                                            # keeps every rank buffer 16-byte aligned
     stride = 64 + pad + 64
@@ -83,7 +84,7 @@ def test_allreduce_writes_stay_inside_buffers(ra, P, count):
         b = big[r * stride + 64: r * stride + 64 + count]
         b.copy_(torch.from_numpy(host[r]))
         bufs.append(b)
-    ra.ra_allreduce_emul(bufs, count)
+    ra.ra_allreduce_emul_ex(bufs, count, variant=variant)
     torch.cuda.synchronize()
     oracle.allreduce(host)
     h = to_host(big, np.float32)
