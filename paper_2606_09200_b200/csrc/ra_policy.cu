@@ -113,6 +113,19 @@ ra_status ra_overlap_suggest(const ra_workload* w, const ra_peaks* peaks, ra_sug
         if (w->kind == RA_COLL_ALLREDUCE) s.cfg.coll_variant = (ring_ok && has_gemm && s.gemm_bound == 1) ? 1 : 0;
     }
 
+    // Collective-bound step under a tensor-bound GEMM (the paper's literal cb workloads: 7.5 GB of collective against a
+    // 0.7 ms GEMM).  The GEMM's default plan allocates all 228 KiB of an SM's shared memory, which leaves the co-resident
+    // collective no L1 for its loads in flight (512 threads x P x 16 B = 64 KiB at P = 8): measured, the overlapped step
+    // is then no faster than the serial one (2.02 vs 2.03 ms).  A 32 KiB reserve costs the GEMM a pipeline stage it does
+    // not need here and gives the collective its L1 back: 1.55 ms.  This is the paper's knob doing the paper's job
+    // (PAPER.md:45-47); when the GEMM is the long pole (cb-ar) the stage is worth more than the collective's speed.
+    // The alltoall has a better answer in that regime: the copy engines move it without any SM, L1 or shared memory
+    // (paper-cb-a2a: 1.54-1.63 ms for every GEMM setting against 1.74+ for the SM variants).
+    if (has_gemm && w->kind != RA_COLL_NONE && s.gemm_bound == 0 && t_coll > t_tensor_all) {
+        if (w->kind == RA_COLL_ALLTOALL) s.cfg.coll_variant = 2;
+        else s.cfg.occ.smem_reserve_bytes = 32 * 1024;
+    }
+
     const double t_gemm_alone = has_gemm ? (t_tensor_all > t_gemm_mem ? t_tensor_all : t_gemm_mem) : 0.0;
     const int n = w->n_iters;
     s.t_gemm_ms = t_gemm_alone;

@@ -212,6 +212,14 @@ def test_policy_rooflines_and_choices(ra):
     kw = s["kw"]
     assert kw["occ"]["sm_budget"] == 0 and kw["occ"]["smem_reserve_bytes"] == 0 and kw["prio_comm"] == kw["prio_compute"]
     assert kw["coll_variant"] == 0                              # tensor-bound GEMM: the register allreduce co-resides everywhere
+    # the same GEMM under a collective seven times larger (the paper's literal cb-ar): the collective is the long pole,
+    # so the GEMM gives up a pipeline stage (32 KiB reserve) to leave the co-resident collective its L1
+    wl, keepl = _workload(ra, 8192, 8192, 8192, "allreduce", 4, count=224 << 20, n_iters=10)
+    sl = ra.ra_overlap_suggest(wl, T, H)
+    assert sl["kw"]["occ"]["smem_reserve_bytes"] == 32 * KB and sl["t_coll_ms"] > sl["t_gemm_ms"]
+    wl, keepl = _workload(ra, 8192, 8192, 8192, "alltoall", 4, chunk=224 << 20, n_iters=10)
+    sl = ra.ra_overlap_suggest(wl, T, H)
+    assert sl["kw"]["coll_variant"] == 2 and sl["kw"]["occ"]["smem_reserve_bytes"] == 0     # copy engines: no SM resource at all
     # the same GEMM fills shared memory, so the alltoall must be the shared-memory-free variant
     w, keep = _workload(ra, 8192, 8192, 8192, "alltoall", 8, chunk=8 << 20)
     assert ra.ra_overlap_suggest(w, T, H)["kw"]["coll_variant"] == 1
