@@ -114,10 +114,10 @@ ra_status ra_overlap_suggest(const ra_workload* w, const ra_peaks* peaks, ra_sug
     }
 
     // Collective-bound step under a tensor-bound GEMM (the paper's literal cb workloads: 7.5 GB of collective against a
-    // 0.7 ms GEMM).  The GEMM's default plan allocates all 228 KiB of an SM's shared memory, which leaves the co-resident
-    // collective no L1 for its loads in flight (512 threads x P x 16 B = 64 KiB at P = 8): measured, the overlapped step
+    // 0.7 ms GEMM).  The GEMM's default plan leaves 1.75 KiB of an SM's shared memory: room for ONE collective CTA (each
+    // costs 1 KiB of system-reserved shared memory) and no L1 (carved from the same array): measured, the overlapped step
     // is then no faster than the serial one (2.02 vs 2.03 ms).  A 32 KiB reserve costs the GEMM a pipeline stage it does
-    // not need here and gives the collective its L1 back: 1.55 ms.  This is the paper's knob doing the paper's job
+    // not need here and gives the collective its second CTA and its L1 back: 1.55 ms.  This is the paper's knob doing the paper's job
     // (PAPER.md:45-47); when the GEMM is the long pole (cb-ar) the stage is worth more than the collective's speed.
     // The alltoall has a better answer in that regime: the copy engines move it without any SM, L1 or shared memory
     // (paper-cb-a2a: 1.54-1.63 ms for every GEMM setting against 1.74+ for the SM variants).
