@@ -211,6 +211,11 @@ typedef struct {
     void* a2a_a; void* a2a_b;   /* device; iteration i copies a->b if i is even, b->a if odd */
     size_t chunk_bytes;
     int32_t n_iters;
+    float* const* ar_pristine;  /* optional (NULL = off): HOST array of P device pointers, ar_count floats each, disjoint
+                                   from ar_bufs.  ra_overlap_run / _sweep / _autotune copy ar_pristine[r] -> ar_bufs[r]
+                                   device-to-device before EVERY run, outside the timed window, so that repeated runs of
+                                   the in-place allreduce (magnitudes grow by P per iteration) always reduce the same
+                                   finite data.  Ignored by ra_overlap_run_host (it uploads its inputs every step). */
 } ra_workload;
 
 typedef struct {

@@ -59,7 +59,8 @@ class Workload(Structure):
                 ("A", c_void_p), ("lda", c_int32), ("B", c_void_p), ("ldb", c_int32), ("C", c_void_p), ("ldc", c_int32),
                 ("workspace", c_void_p), ("workspace_bytes", c_size_t),
                 ("kind", c_int32), ("P", c_int32), ("ar_bufs", POINTER(c_void_p)), ("ar_count", c_size_t),
-                ("a2a_a", c_void_p), ("a2a_b", c_void_p), ("chunk_bytes", c_size_t), ("n_iters", c_int32)]
+                ("a2a_a", c_void_p), ("a2a_b", c_void_p), ("chunk_bytes", c_size_t), ("n_iters", c_int32),
+                ("ar_pristine", POINTER(c_void_p))]
 
 
 class OverlapCfg(Structure):
@@ -258,9 +259,10 @@ def ra_set_trace(buf, capacity: int = 0) -> None:
     _check(_L().ra_set_trace(_ptr(buf), int(capacity)), "ra_set_trace")
 
 
-def make_workload(*, gemm=None, allreduce=None, alltoall=None, n_iters=1):
+def make_workload(*, gemm=None, allreduce=None, alltoall=None, n_iters=1, ar_pristine=None):
     """Marshal a workload.  gemm = dict(M,N,K,A,B,C[,alpha,beta,lda,ldb,ldc,transA,transB,workspace]);
-    allreduce = list of P fp32 tensors; alltoall = dict(a, b, P, chunk_bytes).
+    allreduce = list of P fp32 tensors; alltoall = dict(a, b, P, chunk_bytes); ar_pristine = optional list of P
+    fp32 tensors the library copies into the allreduce buffers before every run (outside the timed window).
     Returns (Workload, keepalive) -- keepalive holds the pointer array."""
     w = Workload()
     keep = []
@@ -283,6 +285,11 @@ def make_workload(*, gemm=None, allreduce=None, alltoall=None, n_iters=1):
         w.kind, w.P = RA_COLL_ALLREDUCE, len(allreduce)
         w.ar_bufs = ctypes.cast(arr, POINTER(c_void_p))
         w.ar_count = int(allreduce[0].numel())
+        if ar_pristine is not None:
+            assert len(ar_pristine) == len(allreduce)
+            parr = _ptr_array(ar_pristine)
+            keep.append(parr)
+            w.ar_pristine = ctypes.cast(parr, POINTER(c_void_p))
     elif alltoall is not None:
         w.kind, w.P = RA_COLL_ALLTOALL, int(alltoall["P"])
         w.a2a_a, w.a2a_b = _ptr(alltoall["a"]), _ptr(alltoall["b"])

@@ -197,16 +197,14 @@ static cudaError_t launch_ar(const ArPtrs& ptrs, size_t count, int grid, cudaStr
     return cudaGetLastError();
 }
 
-ra_status allreduce_launch(float* const* bufs, int P, size_t count, int sm_budget, int ctas_per_sm, int smem_bytes_per_cta,
-                           int variant, cudaStream_t stream) {
+// Argument rules of ra_allreduce_emul(_ex); also called by the overlap driver BEFORE it enqueues anything.
+ra_status allreduce_validate(float* const* bufs, int P, size_t count, int sm_budget, int ctas_per_sm, int smem_bytes_per_cta,
+                             int variant) {
     if (bufs == nullptr || P < 1 || P > RA_MAX_RANKS) return RA_ERR_INVALID_ARG;
     if (sm_budget < 0 || ctas_per_sm < 0 || ctas_per_sm > kArCtasPerSm) return RA_ERR_INVALID_ARG;
     if (smem_bytes_per_cta < 0 || (variant != 0 && variant != 1)) return RA_ERR_INVALID_ARG;
-    ArPtrs ptrs{};
-    for (int r = 0; r < P; ++r) {
+    for (int r = 0; r < P; ++r)
         if (bufs[r] == nullptr || (reinterpret_cast<uintptr_t>(bufs[r]) & 15u)) return RA_ERR_INVALID_ARG;
-        ptrs.p[r] = bufs[r];
-    }
     const size_t bytes = count * sizeof(float);
     for (int a = 0; a < P; ++a)
         for (int b = a + 1; b < P; ++b) {
@@ -214,6 +212,18 @@ ra_status allreduce_launch(float* const* bufs, int P, size_t count, int sm_budge
             if (pa < pb + bytes && pb < pa + bytes && bytes > 0) return RA_ERR_INVALID_ARG;
             if (pa == pb) return RA_ERR_INVALID_ARG;
         }
+    if (variant == 1 && count > 0) {          // the TMA ring needs at least one 128-byte slice per rank and slot
+        const int smem = smem_bytes_per_cta ? smem_bytes_per_cta : 64 * 1024;
+        if ((((uint32_t)smem / (uint32_t)(kArTmaSlots * P * 4)) & ~31u) < 32) return RA_ERR_INVALID_ARG;
+    }
+    return RA_OK;
+}
+
+ra_status allreduce_launch(float* const* bufs, int P, size_t count, int sm_budget, int ctas_per_sm, int smem_bytes_per_cta,
+                           int variant, cudaStream_t stream) {
+    RA_TRY(allreduce_validate(bufs, P, count, sm_budget, ctas_per_sm, smem_bytes_per_cta, variant));
+    ArPtrs ptrs{};
+    for (int r = 0; r < P; ++r) ptrs.p[r] = bufs[r];
     if (count == 0) return RA_OK;
 
     DeviceInfo di;

@@ -143,18 +143,27 @@ alltoall_ldg_kernel(const A2aParams p, Trace tr) {
     if (threadIdx.x == 0) trace_end(rec);
 }
 
-ra_status alltoall_launch(const void* send, void* recv, int P, size_t chunk_bytes, int sm_budget,
-                          int smem_bytes_per_cta, int ctas_per_sm, int variant, cudaStream_t stream) {
+// Argument rules of ra_alltoall_emul(_ex); also called by the overlap driver BEFORE it enqueues anything.
+ra_status alltoall_validate(const void* send, const void* recv, int P, size_t chunk_bytes, int sm_budget, int smem_bytes_per_cta,
+                            int ctas_per_sm, int variant) {
     if (send == nullptr || recv == nullptr || P < 1 || P > 256) return RA_ERR_INVALID_ARG;
     if (sm_budget < 0 || smem_bytes_per_cta < 0 || ctas_per_sm < 0 || (variant < 0 || variant > 2))
         return RA_ERR_INVALID_ARG;
     if ((reinterpret_cast<uintptr_t>(send) & 15u) || (reinterpret_cast<uintptr_t>(recv) & 15u)) return RA_ERR_INVALID_ARG;
     if (chunk_bytes % 16 != 0) return RA_ERR_INVALID_ARG;
     const size_t total = (size_t)P * P * chunk_bytes;
-    {
-        const uintptr_t a = reinterpret_cast<uintptr_t>(send), b = reinterpret_cast<uintptr_t>(recv);
-        if (a == b || (total > 0 && a < b + total && b < a + total)) return RA_ERR_INVALID_ARG;
+    const uintptr_t a = reinterpret_cast<uintptr_t>(send), b = reinterpret_cast<uintptr_t>(recv);
+    if (a == b || (total > 0 && a < b + total && b < a + total)) return RA_ERR_INVALID_ARG;
+    if (variant == 0 && chunk_bytes > 0) {    // ring slots of at least 1 KiB
+        const int smem = smem_bytes_per_cta ? smem_bytes_per_cta : kA2aDefaultSmem;
+        if ((((uint32_t)smem / kA2aSlots) & ~127u) < 1024) return RA_ERR_INVALID_ARG;
     }
+    return RA_OK;
+}
+
+ra_status alltoall_launch(const void* send, void* recv, int P, size_t chunk_bytes, int sm_budget,
+                          int smem_bytes_per_cta, int ctas_per_sm, int variant, cudaStream_t stream) {
+    RA_TRY(alltoall_validate(send, recv, P, chunk_bytes, sm_budget, smem_bytes_per_cta, ctas_per_sm, variant));
     if (chunk_bytes == 0) return RA_OK;
 
     DeviceInfo di;

@@ -23,6 +23,10 @@ ra_status allreduce_launch(float* const* bufs, int P, size_t count, int sm_budge
                            int variant, cudaStream_t stream);
 ra_status alltoall_launch(const void* send, void* recv, int P, size_t chunk_bytes, int sm_budget,
                           int smem_bytes_per_cta, int ctas_per_sm, int variant, cudaStream_t stream);
+ra_status allreduce_validate(float* const* bufs, int P, size_t count, int sm_budget, int ctas_per_sm, int smem_bytes_per_cta,
+                             int variant);
+ra_status alltoall_validate(const void* send, const void* recv, int P, size_t chunk_bytes, int sm_budget, int smem_bytes_per_cta,
+                            int ctas_per_sm, int variant);
 
 // ---- cached host objects ----------------------------------------------------------------------
 struct Cache {
@@ -62,6 +66,25 @@ static ra_status validate(const ra_workload* w, const ra_overlap_cfg* cfg, ra_ov
     if (cfg->mode != RA_MODE_SERIAL && cfg->mode != RA_MODE_OVERLAP) return RA_ERR_INVALID_ARG;
     if (w->kind != RA_COLL_ALLREDUCE && w->kind != RA_COLL_ALLTOALL && w->kind != RA_COLL_NONE) return RA_ERR_INVALID_ARG;
     if (w->kind == RA_COLL_NONE && w->M == 0) return RA_ERR_INVALID_ARG;
+    // the collective's argument rules are checked here, before anything is enqueued or any pointer array is read:
+    // a failing call must have no side effects, and K_c^0 is launched only after K_g^0 is already in flight
+    if (w->kind == RA_COLL_ALLREDUCE) {
+        RA_TRY(allreduce_validate(w->ar_bufs, w->P, w->ar_count, cfg->coll_sm_budget, cfg->coll_ctas_per_sm, cfg->coll_smem_bytes,
+                                  cfg->coll_variant == 1 ? 1 : 0));
+        if (w->ar_pristine != nullptr) {
+            for (int r = 0; r < w->P; ++r) {
+                if (w->ar_pristine[r] == nullptr) return RA_ERR_INVALID_ARG;
+                const uintptr_t a = reinterpret_cast<uintptr_t>(w->ar_pristine[r]), bytes = w->ar_count * sizeof(float);
+                for (int q = 0; q < w->P; ++q) {
+                    const uintptr_t b = reinterpret_cast<uintptr_t>(w->ar_bufs[q]);
+                    if (bytes > 0 && a < b + bytes && b < a + bytes) return RA_ERR_INVALID_ARG;
+                }
+            }
+        }
+    } else if (w->kind == RA_COLL_ALLTOALL) {
+        RA_TRY(alltoall_validate(w->a2a_a, w->a2a_b, w->P, w->chunk_bytes, cfg->coll_sm_budget, cfg->coll_smem_bytes,
+                                 cfg->coll_ctas_per_sm, cfg->coll_variant));
+    }
     return RA_OK;
 }
 
@@ -185,16 +208,39 @@ static ra_status run_once(const ra_workload* w, const ra_overlap_cfg* cfg, ra_ov
             g_cache.graphs[key] = gexec;
         }
     }
-    RA_CUDA(cudaEventRecord(ev_start, s_comp));
+    // An in-place allreduce multiplies magnitudes by P every iteration: with `ar_pristine` set the rank buffers are
+    // refilled (device-to-device, on the compute stream, BEFORE ev_start) so that every run reduces the same finite,
+    // full-entropy data -- saturated +-inf / 0 operands would flatter the power-capped clocks and the HBM figures.
+    if (w->kind == RA_COLL_ALLREDUCE && w->ar_pristine != nullptr)
+        for (int r = 0; r < w->P; ++r)
+            RA_CUDA(cudaMemcpyAsync(w->ar_bufs[r], w->ar_pristine[r], w->ar_count * sizeof(float), cudaMemcpyDeviceToDevice, s_comp));
+    // From here on work is in flight on the cached streams: a failure must not return while the caller's buffers are
+    // still being read or written, so every error path drains both streams first.
+    auto drain = [&](ra_status st) {
+        const int saved = g_last_cuda_error;
+        cudaStreamSynchronize(s_comp);
+        if (overlap) cudaStreamSynchronize(s_comm);
+        (void)cudaGetLastError();
+        g_last_cuda_error = saved;
+        return st;
+    };
+#define RA_CUDA_DRAIN(expr)                                              \
+    do {                                                                 \
+        cudaError_t _e = (expr);                                         \
+        if (_e != cudaSuccess) return drain(::ra::cuda_fail(_e));        \
+    } while (0)
+    RA_CUDA_DRAIN(cudaEventRecord(ev_start, s_comp));
     if (gexec) {
-        RA_CUDA(cudaGraphLaunch(gexec, s_comp));
+        RA_CUDA_DRAIN(cudaGraphLaunch(gexec, s_comp));
     } else {
-        if (overlap) RA_CUDA(cudaStreamWaitEvent(s_comm, ev_start, 0));
-        RA_TRY(enqueue_step(w, cfg, s_comp, s_comm, rec, &plan));
+        if (overlap) RA_CUDA_DRAIN(cudaStreamWaitEvent(s_comm, ev_start, 0));
+        const ra_status st = enqueue_step(w, cfg, s_comp, s_comm, rec, &plan);
+        if (st != RA_OK) return drain(st);
     }
-    RA_CUDA(cudaEventRecord(ev_end, s_comp));
-    RA_CUDA(cudaEventSynchronize(ev_end));
-    RA_CUDA(cudaGetLastError());
+    RA_CUDA_DRAIN(cudaEventRecord(ev_end, s_comp));
+    RA_CUDA_DRAIN(cudaEventSynchronize(ev_end));
+    RA_CUDA_DRAIN(cudaGetLastError());
+#undef RA_CUDA_DRAIN
 
     float total = 0.f;
     RA_CUDA(cudaEventElapsedTime(&total, ev_start, ev_end));
@@ -290,7 +336,16 @@ static ra_status run_host(const ra_workload* const* dev, int n_sets, const ra_ho
         }
         RA_CUDA(cudaEventRecord(set_ev(k, 3), s_h2d));
         RA_CUDA(cudaStreamWaitEvent(overlap ? s_comm : s_comp, set_ev(k, 3), 0));
-        RA_TRY(enqueue_step(w, cfg, s_comp, s_comm, false, &plan));
+        {
+            const ra_status st = enqueue_step(w, cfg, s_comp, s_comm, false, &plan);
+            if (st != RA_OK) {                 // copies / kernels of earlier steps are in flight: drain before returning
+                const int saved = g_last_cuda_error;
+                cudaStreamSynchronize(s_h2d); cudaStreamSynchronize(s_comp); cudaStreamSynchronize(s_comm); cudaStreamSynchronize(s_d2h);
+                (void)cudaGetLastError();
+                g_last_cuda_error = saved;
+                return st;
+            }
+        }
         RA_CUDA(cudaEventRecord(set_ev(k, 1), s_comp));
         RA_CUDA(cudaStreamWaitEvent(s_d2h, set_ev(k, 1), 0));
         if (has_gemm && io->C) RA_CUDA(cudaMemcpyAsync(io->C, w->C, c_bytes(w), cudaMemcpyDeviceToHost, s_d2h));

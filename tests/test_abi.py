@@ -40,7 +40,7 @@ def test_struct_layouts_match_header(ra):
     # sizes computed by hand from include/ra.h (LP64)
     assert ctypes.sizeof(ra.Occupancy) == 28
     assert ctypes.sizeof(ra.GemmPlan) == 60
-    assert ctypes.sizeof(ra.Workload) == 152
+    assert ctypes.sizeof(ra.Workload) == 160
     assert ctypes.sizeof(ra.OverlapCfg) == 4 + 28 + 9 * 4
     assert ctypes.sizeof(ra.OverlapResult) == 24 + 60 + 4 + 8
     assert ctypes.sizeof(ra.HostIO) == 7 * 8
@@ -150,6 +150,50 @@ def test_argument_errors_need_no_gpu(ra):
     assert lib.ra_overlap_run(None, None, None) == ra.RA_ERR_INVALID_ARG
 
 
+def test_overlap_driver_validates_the_collective_before_touching_it(ra):
+    """A bad collective description is RA_ERR_INVALID_ARG from ra_overlap_run / _run_host / _sweep: no pointer array is
+    read past P, nothing is enqueued (ra.h: 'a failing call has no side effects').  Needs no device."""
+    lib = ra._L()
+    fake = 0x100000
+    g = dict(M=128, N=128, K=128, A=fake, B=fake + (1 << 20), C=fake + (2 << 20))
+    bufs = [_FakeBuf(1024, fake + (4 << 20) + i * 8192) for i in range(4)]
+    res = ra.OverlapResult()
+
+    def run(w, **kw):
+        return lib.ra_overlap_run(ctypes.byref(w), ctypes.byref(ra.make_cfg(**kw)), ctypes.byref(res))
+
+    w, keep = ra.make_workload(gemm=g, allreduce=bufs, n_iters=2)
+    w.ar_bufs = None
+    assert run(w) == ra.RA_ERR_INVALID_ARG                                    # NULL pointer array (was a host segfault)
+    for bad_p in (0, -3, ra.RA_MAX_RANKS + 1, 1 << 20):
+        w, keep = ra.make_workload(gemm=g, allreduce=bufs, n_iters=2)
+        w.P = bad_p
+        assert run(w) == ra.RA_ERR_INVALID_ARG, bad_p
+        assert run(w, use_graph=1) == ra.RA_ERR_INVALID_ARG, bad_p            # the graph key must not read ar_bufs[0..P)
+    w, keep = ra.make_workload(gemm=g, allreduce=[_FakeBuf(1024, fake), _FakeBuf(1024, fake + 2048)], n_iters=2)
+    assert run(w) == ra.RA_ERR_INVALID_ARG                                    # rank buffers overlap
+    w, keep = ra.make_workload(gemm=g, allreduce=bufs, n_iters=2, ar_pristine=[bufs[1]] * 4)
+    assert run(w) == ra.RA_ERR_INVALID_ARG                                    # pristine copy aliases a rank buffer
+    w, keep = ra.make_workload(gemm=g, allreduce=bufs, n_iters=2)
+    assert run(w, coll_variant=1, coll_smem_bytes=64) == ra.RA_ERR_INVALID_ARG   # ring too small for one slice
+    for a2a in (dict(a=None, b=fake, P=2, chunk_bytes=64), dict(a=fake, b=fake + 64, P=2, chunk_bytes=64),
+                dict(a=fake, b=fake + 4096, P=2, chunk_bytes=24), dict(a=fake, b=fake + 4096, P=0, chunk_bytes=64),
+                dict(a=fake + 8, b=fake + 4096, P=2, chunk_bytes=64)):
+        w, keep = ra.make_workload(gemm=g, alltoall=a2a, n_iters=2)
+        assert run(w) == ra.RA_ERR_INVALID_ARG, a2a
+    w, keep = ra.make_workload(gemm=g, alltoall=dict(a=fake, b=fake + 4096, P=2, chunk_bytes=64), n_iters=2)
+    assert run(w, coll_variant=7) == ra.RA_ERR_INVALID_ARG
+    # host-buffer entry point: P is checked before io->ar_in[0..P) is indexed
+    w, keep = ra.make_workload(gemm=g, allreduce=bufs, n_iters=2)
+    w.P = 1 << 20
+    io, keep_io = ra.make_host_io(A=fake, B=fake, ar_in=[fake] * 4)
+    assert lib.ra_overlap_run_host(ctypes.byref(w), None, ctypes.byref(io), ctypes.byref(ra.make_cfg()), 1,
+                                   ctypes.byref(res)) == ra.RA_ERR_INVALID_ARG
+    cfgs = (ra.OverlapCfg * 1)(ra.make_cfg())
+    best = ctypes.c_int(-1)
+    assert lib.ra_overlap_sweep(ctypes.byref(w), cfgs, 1, 3, (ra.OverlapResult * 1)(), ctypes.byref(best)) == ra.RA_ERR_INVALID_ARG
+
+
 def test_compute_fails_loudly_without_device(ra):
     try:
         import torch
@@ -179,14 +223,15 @@ def test_product_never_imports_oracle():
 
 # ---- S7': the model-based knob policy is host-only, so its logic is tested here ---------------------------------------
 class _FakeBuf:
-    def __init__(self, n):
+    def __init__(self, n, ptr=16):
         self.n = n
+        self.ptr = ptr
 
     def numel(self):
         return self.n
 
     def data_ptr(self):
-        return 16
+        return self.ptr
 
 
 def _workload(ra, M, N, K, coll, P, count=0, chunk=0, n_iters=20):
