@@ -2,6 +2,7 @@
 """bench.py -- the hot path of arxiv/paper_2606_09200 on B200: GEMM overlapped with a collective stand-in.
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--config cb-ar|mb-ar|cb-a2a|mb-a2a|tiny] [--impl ours|reference]
+                    [--per-config all|none]
 
 One "step" = one pass of the whole hot path over one batch of seeded synthetic
 input: n_iters pipelined iterations of  K_g^i (tcgen05 GEMM)  ||  K_c^i (allreduce / alltoall stand-in)
@@ -10,7 +11,16 @@ BASELINE.json configs[1] ("cb-ar": GEMM 8192^3 bf16 + allreduce emul P=8 x 16Mi 
 
 Prints ONE JSON line (rank 0).  value = overlapped iterations per second over all GPUs (replicas only:
 the path does not shard).  The line also carries serial/overlap/ratio, per-kernel
-TFLOP/s and GB/s against MEASURED_PEAKS.json, the combined roofline, `roofline`, `cpu_baseline`, `e2e`.
+TFLOP/s and GB/s against MEASURED_PEAKS.json, the combined roofline, `roofline`, `cpu_baseline`, `e2e`, and
+-- at N = 1 -- `per_config`: the same protocol on the other four BASELINE.json configs (Tiny, mb-ar, cb-a2a,
+mb-a2a with its reserve x budget x priority sweep), each also flattened to one string under `config` so that
+a parser which keeps only scalars still sees all five.
+
+Timing protocol.  The K timed steps run at exactly the picked setting with NO per-kernel events (so the
+CUDA-graph mode the policy picks for launch-bound steps is honoured); the per-kernel split, the overlap rate
+and the dominant kernel's launch time come from an instrumented pass of the same K steps right after it.
+The in-place allreduce buffers are refilled from pristine device copies before every run (outside the
+timed window), so every iteration reduces finite, full-entropy data.
 """
 from __future__ import annotations
 
@@ -128,7 +138,7 @@ def host_inputs(cfg, pinned: bool):
     return h
 
 
-def device_state(ra, cfg, h):
+def device_state(ra, cfg, h, pristine=True):
     import torch
     d = {"A": h["A"].cuda(), "B": h["B"].cuda(),
          "C": torch.empty((cfg.M, cfg.N), dtype=torch.int16, device="cuda")}
@@ -137,6 +147,7 @@ def device_state(ra, cfg, h):
     d["ws"] = torch.empty(max(wsb, 16), dtype=torch.uint8, device="cuda")
     if cfg.coll == "allreduce":
         d["ar"] = [t.cuda() for t in h["ar"]]
+        d["ar_pristine"] = [t.cuda() for t in h["ar"]] if pristine else None
     else:
         d["a2a_a"] = h["a2a"].cuda()
         d["a2a_b"] = torch.empty_like(d["a2a_a"])
@@ -148,16 +159,19 @@ def make_workload(ra, cfg, d, n_iters, gemm=True, coll=True):
     kw = {}
     if coll and cfg.coll == "allreduce":
         kw["allreduce"] = d["ar"]
+        kw["ar_pristine"] = d.get("ar_pristine")     # the library refills the rank buffers before every run
     elif coll:
         kw["alltoall"] = dict(a=d["a2a_a"], b=d["a2a_b"], P=cfg.P, chunk_bytes=cfg.chunk_bytes)
     return ra.make_workload(gemm=g, n_iters=n_iters, **kw)
 
 
-def reset_collective(cfg, d, h):
-    """In-place allreduce multiplies magnitudes by P every iteration; refill between phases so values stay finite."""
+def check_finite(cfg, d, where: str):
+    """The in-place allreduce multiplies magnitudes by P per iteration (8^20 ~ 1e18 over one step: finite in fp32); the
+    library refills the buffers from the pristine copies before every run.  A saturated buffer here means that broke."""
+    import torch
     if cfg.coll == "allreduce":
-        for t, s in zip(d["ar"], h["ar"]):
-            t.copy_(s, non_blocking=True)
+        t = d["ar"][0]
+        assert bool(torch.isfinite(t).all()) and float(t.abs().max()) > 0.0, f"allreduce buffers saturated after {where}"
 
 
 def sweep_candidates(ra, cfg, quick: bool):
@@ -240,7 +254,7 @@ def residency_map(ra, w, cfg_kw, n_sms):
     return out
 
 
-def kernels_alone(ra, cfg, d, h, peaks, n_iters):
+def kernels_alone(ra, cfg, d, peaks, n_iters, graph: int = 0):
     """Each kernel by itself (CUDA events inside the library, on the stream the kernel runs on)."""
     out = {}
     # burst: single launches with idle gaps, best of 10 (how MEASURED_PEAKS.json's burst figure was taken)
@@ -255,7 +269,7 @@ def kernels_alone(ra, cfg, d, h, peaks, n_iters):
     out["gemm_frac_of_bf16_peak_burst"] = out["gemm_tflops_burst"] / peaks["bf16_tflops"]
     # sustained: back-to-back launches (power-capped regime)
     w, keep = make_workload(ra, cfg, d, n_iters, coll=False)
-    res, _ = ra.ra_overlap_sweep(w, [ra.make_cfg(mode=0)], runs=6)
+    res, _ = ra.ra_overlap_sweep(w, [ra.make_cfg(mode=0, use_graph=graph)], runs=6)
     g_ms = res[0]["total_ms"] / n_iters
     out["gemm_ms"] = g_ms
     out["gemm_tflops"] = cfg.gemm_flops / g_ms / 1e9
@@ -263,18 +277,16 @@ def kernels_alone(ra, cfg, d, h, peaks, n_iters):
     out["gemm_gbs"] = cfg.gemm_bytes / g_ms / 1e6
     out["gemm_frac_of_hbm_peak"] = out["gemm_gbs"] / peaks["hbm_gbs"]
     out["gemm_plan"] = res[0]["plan"]
-    reset_collective(cfg, d, h)
     w, keep = make_workload(ra, cfg, d, n_iters, gemm=False)
     # the collective alone is a bandwidth measurement: let the clocks recover from the power-capped GEMM runs first
     import torch
     torch.cuda.synchronize()
     time.sleep(0.5)
-    res, _ = ra.ra_overlap_sweep(w, [ra.make_cfg(mode=0)], runs=6)
+    res, _ = ra.ra_overlap_sweep(w, [ra.make_cfg(mode=0, use_graph=graph)], runs=6)
     c_ms = res[0]["total_ms"] / n_iters
     out["coll_ms"] = c_ms
     out["coll_gbs"] = cfg.coll_bytes / c_ms / 1e6
     out["coll_frac_of_hbm_peak"] = out["coll_gbs"] / peaks["hbm_gbs"]
-    reset_collective(cfg, d, h)
     return out
 
 
@@ -282,60 +294,122 @@ def kernels_alone(ra, cfg, d, h, peaks, n_iters):
 _ORACLE_INPUTS = {}
 
 
-def cpu_oracle_sample(cfg, budget_s: float = 12.0):
-    """The oracle as it stands, on the host cores, on a bounded sample of the same workload.
-    GEMM: oracle.gemm_samples on n sampled C entries (each the full K-length fp64 dot product),
-    scaled by M*N/n; collective: one full oracle pass (it is DRAM-bound and takes well under a second
-    per GiB).  Returns (seconds per full iteration [extrapolated], description, cores, sampled seconds)."""
-    import oracle
+def _oracle_inputs(cfg):
     if cfg.name not in _ORACLE_INPUTS:       # input generation is not part of what is timed
+        _ORACLE_INPUTS.clear()               # one workload's operands at a time (8192 x 57344 alone is 1.9 GB)
         _ORACLE_INPUTS[cfg.name] = ra_inputs.gemm_operands(cfg)
-    A, B = _ORACLE_INPUTS[cfg.name]
-    rng = np.random.default_rng(cfg.seed)
-    # calibrate: time a small batch, then size the sample for ~budget_s
-    n0 = 2048
-    ii, jj = rng.integers(0, cfg.M, n0), rng.integers(0, cfg.N, n0)
-    t0 = time.perf_counter()
-    oracle.gemm_samples(0, 1, cfg.M, cfg.N, cfg.K, 1.0, A, B, ii, jj)
-    dt0 = time.perf_counter() - t0
-    n = int(min(cfg.M * cfg.N, max(n0, n0 * budget_s / max(dt0, 1e-6))))
-    ii, jj = rng.integers(0, cfg.M, n), rng.integers(0, cfg.N, n)
-    t0 = time.perf_counter()
-    oracle.gemm_samples(0, 1, cfg.M, cfg.N, cfg.K, 1.0, A, B, ii, jj)
-    t_gemm_sample = time.perf_counter() - t0
-    t_gemm_full = t_gemm_sample * (cfg.M * cfg.N / n)
+    return _ORACLE_INPUTS[cfg.name]
+
+
+def _oracle_collective_pass(cfg):
+    """One full pass of the collective's oracle over the config's buffers; seconds."""
+    import oracle
     if cfg.coll == "allreduce":
         bufs = ra_inputs.allreduce_buffers(cfg)
         t0 = time.perf_counter()
         oracle.allreduce(bufs)
-        t_coll = time.perf_counter() - t0
-    else:
-        send = ra_inputs.alltoall_payload(cfg)
+        return time.perf_counter() - t0
+    send = ra_inputs.alltoall_payload(cfg)
+    t0 = time.perf_counter()
+    oracle.alltoall(send, cfg.P, cfg.chunk_bytes)
+    return time.perf_counter() - t0
+
+
+def _oracle_gemm_calibrate(cfg, n0: int = 2048):
+    """Seconds per C entry of oracle.gemm_samples (each entry = the full K-length fp64 dot product)."""
+    import oracle
+    A, B = _oracle_inputs(cfg)
+    rng = np.random.default_rng(cfg.seed)
+    ii, jj = rng.integers(0, cfg.M, n0), rng.integers(0, cfg.N, n0)
+    oracle.gemm_samples(0, 1, cfg.M, cfg.N, cfg.K, 1.0, A, B, ii[:64], jj[:64])       # page the operands in
+    t0 = time.perf_counter()
+    oracle.gemm_samples(0, 1, cfg.M, cfg.N, cfg.K, 1.0, A, B, ii, jj)
+    return (time.perf_counter() - t0) / n0
+
+
+def cpu_oracle_full(cfg, full_limit_s: float = 90.0, sample_budget_s: float = 15.0):
+    """cpu_baseline: the oracle as it stands, on the host cores.  One iteration of the hot path = oracle.gemm over the
+    whole problem + one oracle pass of the collective.  The GEMM is TIMED IN FULL (one oracle.gemm call over all M x N
+    entries) whenever a calibration run puts it under `full_limit_s`; only larger shapes (8192 x 57344 x 8192) fall back
+    to oracle.gemm_samples on a bounded random sample, extrapolated by M*N/n and labelled as such.
+    Returns (seconds per iteration, description, cores, 'full' | 'sampled')."""
+    import oracle
+    A, B = _oracle_inputs(cfg)
+    per_entry = _oracle_gemm_calibrate(cfg)
+    est = per_entry * cfg.M * cfg.N
+    t_coll = _oracle_collective_pass(cfg)
+    if est <= full_limit_s:
         t0 = time.perf_counter()
-        oracle.alltoall(send, cfg.P, cfg.chunk_bytes)
-        t_coll = time.perf_counter() - t0
-    desc = (f"oracle.gemm_samples on {n} of {cfg.M * cfg.N} C entries (K={cfg.K} each, {t_gemm_sample:.2f} s, extrapolated "
-            f"x{cfg.M * cfg.N / n:.1f} -> {t_gemm_full:.1f} s) + one full oracle {cfg.coll} pass ({t_coll * 1e3:.0f} ms); serial sum")
-    return t_gemm_full + t_coll, desc, oracle.num_threads(), t_gemm_sample + t_coll
+        oracle.gemm(0, 1, cfg.M, cfg.N, cfg.K, 1.0, A, B)
+        t_gemm = time.perf_counter() - t0
+        desc = (f"full: oracle.gemm over all {cfg.M}x{cfg.N} C entries (K={cfg.K}), timed once: {t_gemm:.2f} s "
+                f"(calibration predicted {est:.1f} s) + one full oracle {cfg.coll} pass ({t_coll * 1e3:.0f} ms); serial sum")
+        return t_gemm + t_coll, desc, oracle.num_threads(), "full"
+    rng = np.random.default_rng(cfg.seed + 1)
+    n = int(min(cfg.M * cfg.N, max(2048, sample_budget_s / per_entry)))
+    ii, jj = rng.integers(0, cfg.M, n), rng.integers(0, cfg.N, n)
+    t0 = time.perf_counter()
+    oracle.gemm_samples(0, 1, cfg.M, cfg.N, cfg.K, 1.0, A, B, ii, jj)
+    t_s = time.perf_counter() - t0
+    t_gemm = t_s * (cfg.M * cfg.N / n)
+    desc = (f"sampled: oracle.gemm_samples on {n} of {cfg.M * cfg.N} C entries (K={cfg.K} each, {t_s:.2f} s, extrapolated "
+            f"x{cfg.M * cfg.N / n:.1f} -> {t_gemm:.1f} s; a full pass would exceed {full_limit_s:.0f} s) + one full oracle "
+            f"{cfg.coll} pass ({t_coll * 1e3:.0f} ms); serial sum")
+    return t_gemm + t_coll, desc, oracle.num_threads(), "sampled"
 
 
 def run_reference(args, cfg):
-    """--impl reference: the CPU oracle is the reference arm of this tier (there is no reference code)."""
+    """--impl reference: the CPU oracle is the reference arm of this tier (there is no reference code).
+
+    A step of this arm is a BOUNDED SAMPLE of one iteration of the workload: oracle.gemm_samples on a fixed fraction f
+    of the C entries (each the full K-length fp64 dot product) plus the same fraction of the collective's oracle pass
+    (allreduce: the first f*count elements of every rank buffer; alltoall: f of each chunk).  ms_per_step is the time
+    that step really took; value = f / t_step, i.e. iterations per second at the sampled rate.  f is sized once, from a
+    calibration run, so that warmup + steps fit in `--ref-budget-s` seconds."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    times, desc, cores = [], "", 1
-    for s in range(args.warmup + args.steps):
-        t_iter, desc, cores, _ = cpu_oracle_sample(cfg, budget_s=max(2.0, 60.0 / (args.warmup + args.steps)))
+    import oracle
+    A, B = _oracle_inputs(cfg)
+    n_steps = args.warmup + args.steps
+    per_entry = _oracle_gemm_calibrate(cfg)
+    t_coll_full = _oracle_collective_pass(cfg)
+    t_iter_est = per_entry * cfg.M * cfg.N + t_coll_full
+    f = min(1.0, (args.ref_budget_s / max(n_steps, 1)) / t_iter_est)
+    n = max(64, int(f * cfg.M * cfg.N))
+    f = n / (cfg.M * cfg.N)
+    rng = np.random.default_rng(cfg.seed + 2)
+    ii, jj = rng.integers(0, cfg.M, n), rng.integers(0, cfg.N, n)
+    if cfg.coll == "allreduce":
+        cnt = max(4, int(f * cfg.ar_count))
+        bufs0 = [b[:cnt].copy() for b in ra_inputs.allreduce_buffers(cfg)]
+    else:
+        cb = max(16, int(f * cfg.chunk_bytes) // 16 * 16)
+        send = ra_inputs.alltoall_payload(cfg, chunk_bytes=cb)
+    times = []
+    for s in range(n_steps):
+        if cfg.coll == "allreduce":
+            bufs = [b.copy() for b in bufs0]
+        t0 = time.perf_counter()
+        oracle.gemm_samples(0, 1, cfg.M, cfg.N, cfg.K, 1.0, A, B, ii, jj)
+        if cfg.coll == "allreduce":
+            oracle.allreduce(bufs)
+        else:
+            oracle.alltoall(send, cfg.P, cb)
+        dt = time.perf_counter() - t0
         if s >= args.warmup:
-            times.append(t_iter)
+            times.append(dt)
     t = statistics.mean(times)
-    v = 1.0 / t
+    v = f / t
+    cores = oracle.num_threads()
+    desc = (f"each step = fraction f={f:.5f} of one iteration: oracle.gemm_samples on {n} of {cfg.M * cfg.N} C entries "
+            f"(K={cfg.K} each) + the same fraction of the oracle {cfg.coll} pass; {t:.3f} s per step measured; "
+            f"value = f / t (a full iteration at this rate: {t / f:.1f} s)")
     line = {"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
-            "warmup": args.warmup, "ms_per_step": t * 1e3 * cfg.n_iters, "higher_is_better": True, "scaling": "weak",
+            "warmup": args.warmup, "ms_per_step": t * 1e3, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": cfg.name, "gemm": [cfg.M, cfg.N, cfg.K], "collective": cfg.coll, "P": cfg.P,
-                       "n_iters": cfg.n_iters},
+                       "iterations_per_step": f, "step": "bounded sample of one iteration (see cpu_baseline.sample)"},
             "cpu_baseline": {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc},
             "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
@@ -378,35 +452,94 @@ def barrier(world: int):
         torch.cuda.synchronize()
 
 
-def run_ours(args, cfg):
-    import torch
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py: no CUDA device -- the hot path has no CPU fallback")
-    import paper_2606_09200_b200 as ra   # builds/loads libra.so; raises if the CUDA extension is missing
+def self_launch(argv, n: int) -> int:
+    """`python bench.py --gpus N` with N > 1 and no torchrun environment: start the N ranks ourselves (one process per
+    GPU, rendezvous on 127.0.0.1) and pass their output through."""
+    import socket
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={n}", "--master-addr", "127.0.0.1",
+           "--master-port", str(port), os.path.abspath(__file__)] + list(argv)
+    return subprocess.call(cmd)
 
-    world, rank, local = dist_setup(args.gpus)
-    dev = torch.device("cuda", torch.cuda.current_device())
-    peaks = load_peaks()
+
+# ------------------------------------------------------------------------------------------------
+def config5_grid(ra, cfg):
+    """BASELINE.json configs[4]: 'sweep smem_reserve 0-200 KB, SM budget 74-148, priority on/off' -- the corners and
+    midpoints of the full grid (bench.py --config mb-a2a --sweep full runs all 7 x 6 x 2), sized for ~1 minute."""
+    info = ra.ra_device_info()
+    hi, KB = info["prio_greatest"], 1024
+    cands = []
+    for r in (0, 64 * KB, 128 * KB, 200 * KB):
+        for b in (74, 110, 148):
+            for prio in (0, hi):
+                base = dict(mode=1, occ=dict(smem_reserve_bytes=r, sm_budget=b), prio_compute=0, prio_comm=prio)
+                if r >= 20 * KB:      # TMA ring sized into the reserve, one ring CTA per SM
+                    cands.append(dict(base, coll_variant=0, coll_smem_bytes=min(r - 4 * KB, 64 * KB), coll_ctas_per_sm=1))
+                else:
+                    cands.append(dict(base, coll_variant=0))
+                cands.append(dict(base, coll_variant=1))                         # LDG/STG, no shared memory
+                if b < info["sm_count"]:                                          # collective on the SMs the GEMM leaves free
+                    cands.append(dict(base, coll_variant=0, coll_sm_budget=info["sm_count"] - b))
+    cands.append(dict(mode=1, coll_variant=2))                                   # copy engines
+    return cands
+
+
+def sweep_marginals(cand_kws, results, n_iters):
+    """Best overlap time per reserve, per budget, and priority on / off at otherwise equal settings (Norm. time)."""
+    by_r, by_b, pairs = {}, {}, {}
+    for kw, r in zip(cand_kws, results):
+        if kw.get("mode") != 1:
+            continue
+        lab, ms = cfg_label(kw), r["total_ms"] / n_iters
+        rk, bk = lab["smem_reserve_bytes"] // 1024, lab["sm_budget"] or 148
+        by_r[rk] = min(by_r.get(rk, 1e30), ms)
+        by_b[bk] = min(by_b.get(bk, 1e30), ms)
+        key = tuple(sorted((k, v) for k, v in lab.items() if k != "priority"))
+        pairs.setdefault(key, {})[lab["priority"]] = ms
+    norm = [p["on"] / p["off"] for p in pairs.values() if "on" in p and "off" in p]
+    return {"best_ms_by_reserve_kb": {str(k): round(v, 4) for k, v in sorted(by_r.items())},
+            "best_ms_by_sm_budget": {str(k): round(v, 4) for k, v in sorted(by_b.items())},
+            "norm_time_priority_on_over_off": {"n_pairs": len(norm), "min": min(norm) if norm else None,
+                                               "median": statistics.median(norm) if norm else None,
+                                               "max": max(norm) if norm else None}}
+
+
+def measure_config(ra, cfg, args, peaks, world, dev, headline: bool):
+    """The whole protocol on one workload: warm-up, S7 (sweep + pick, the model's pick inside it), each kernel alone,
+    K timed steps at the picked setting (no per-kernel events), the same K steps serial, an instrumented pass for the
+    per-kernel split / overlap rate; for the headline workload also the residency trace and the e2e leg."""
+    import torch
     n_iters = args.n_iters or cfg.n_iters
-    h = host_inputs(cfg, pinned=True)
+    steps = args.steps
+    h = host_inputs(cfg, pinned=headline)
     d = device_state(ra, cfg, h)
     torch.cuda.synchronize()
+    info = ra.ra_device_info()
 
     # ---- warm-up: W plain steps, then S7 (sweep + pick) with the serial schedule interleaved ----
     w, keep = make_workload(ra, cfg, d, n_iters)
     for _ in range(max(args.warmup, 3)):
         ra.ra_overlap_run(w, ra.make_cfg(mode=1))
-    reset_collective(cfg, d, h)
-    cands = [] if args.sweep in ("none", "auto") else sweep_candidates(ra, cfg, quick=(args.sweep == "quick"))
-    if args.sweep == "auto":       # the library's own short list: model pick + neighbours (ra_overlap_autotune)
+    sweep = args.sweep if headline or args.sweep in ("none", "auto") else ("config5" if cfg.name == "mb-a2a" else "quick")
+    if sweep in ("none", "auto"):
+        cands = []
+    elif sweep == "config5":
+        cands = config5_grid(ra, cfg)
+    else:
+        cands = sweep_candidates(ra, cfg, quick=(sweep == "quick"))
+    if sweep == "auto":       # the library's own short list: model pick + neighbours (ra_overlap_autotune)
         auto_cfg, _, _ = ra.ra_overlap_autotune(w, peaks["bf16_tflops_sustained"], peaks["hbm_gbs"], runs=args.sweep_runs)
-        reset_collective(cfg, d, h)
         cands = [ra.cfg_to_kw(auto_cfg)]
     # S7': the model-based policy's pick runs inside the same sweep so that its regret is measured, not assumed
     sug = ra.ra_overlap_suggest(w, peaks["bf16_tflops_sustained"], peaks["hbm_gbs"])
-    cand_kws = [dict(mode=0)] + [dict(mode=1)] + [sug["kw"]] + cands
-    results, best = ra.ra_overlap_sweep(w, [ra.make_cfg(**kw) for kw in cand_kws], runs=args.sweep_runs)
-    reset_collective(cfg, d, h)
+    graph = int(sug["kw"].get("use_graph", 0))            # launch-bound workload (Tiny): every candidate is graph-replayed
+    if graph:
+        cands = [dict(kw, use_graph=1) for kw in cands]
+    cand_kws = [dict(mode=0, use_graph=graph)] + [dict(mode=1, use_graph=graph)] + [sug["kw"]] + cands
+    runs = args.sweep_runs if sweep != "config5" else max(6, args.sweep_runs - 3)
+    results, best = ra.ra_overlap_sweep(w, [ra.make_cfg(**kw) for kw in cand_kws], runs=runs)
     best_kw = cand_kws[best]
     sweep_serial_ms = results[0]["total_ms"] / n_iters
     sweep_table = [dict(cfg_label(kw), mode=kw["mode"], ms_per_iter=r["total_ms"] / n_iters, median=r["median_ms"] / n_iters,
@@ -420,82 +553,159 @@ def run_ours(args, cfg):
         if kw["mode"] == 1 and all(l2[k] == lab[k] for k in lab if k != "priority") and l2["priority"] != lab["priority"]:
             on, off = (results[best]["total_ms"], r["total_ms"]) if lab["priority"] == "on" else (r["total_ms"], results[best]["total_ms"])
             norm_time = on / off
-
     policy = {"setting": cfg_label(sug["kw"]), "predicted_ms_per_iter": sug["t_overlap_ms"], "measured_ms_per_iter": results[2]["total_ms"] / n_iters,
               "sweep_best_ms_per_iter": results[best]["total_ms"] / n_iters,
               "regret": results[2]["total_ms"] / results[best]["total_ms"] - 1.0, "gemm_bound": sug["gemm_bound"],
               "model_roofline_ms": sug["t_roofline_ms"], "settings_in_sweep": len(cand_kws) - 1}
-    alone = kernels_alone(ra, cfg, d, h, peaks, n_iters)
-    residency = residency_map(ra, w, best_kw, ra.ra_device_info()["sm_count"])
-    reset_collective(cfg, d, h)
+    alone = kernels_alone(ra, cfg, d, peaks, n_iters, graph=graph)
+    residency = residency_map(ra, w, best_kw, info["sm_count"]) if headline else None
 
-    # ---- timed region: exactly K steps of the overlapped hot path at the picked setting ----
-    best_cfg = ra.make_cfg(**dict(best_kw, record_kernel_times=1))
+    # ---- timed region: exactly K steps of the overlapped hot path at exactly the picked setting ----
+    best_cfg = ra.make_cfg(**best_kw)
+    ra.ra_gemm_residency(reset=True)
     sampler = ClockSampler(torch.cuda.current_device())
     barrier(world)
     sampler.start()
     t_wall0 = time.perf_counter()
-    step_ms, g_ms, c_ms, orate = [], [], [], []
-    for _ in range(args.steps):
+    step_ms = []
+    for _ in range(steps):
         r = ra.ra_overlap_run(w, best_cfg)          # synchronous; total_ms from CUDA events on its own streams
         step_ms.append(r["total_ms"])
-        g_ms.append(r["gemm_ms_sum"] / n_iters)
-        c_ms.append(r["coll_ms_sum"] / n_iters)
-        orate.append(r["overlap_rate"])
     barrier(world)
     wall_ms = (time.perf_counter() - t_wall0) * 1e3
     clocks = sampler.stop()
     plan = r["plan"]
-    reset_collective(cfg, d, h)
+    check_finite(cfg, d, "the timed region")
+    max_resident = ra.ra_gemm_residency()
     dev_ms_total = max_over_ranks(sum(step_ms), world, dev)
-    ms_per_step = dev_ms_total / args.steps
+    ms_per_step = dev_ms_total / steps
     over_ms = ms_per_step / n_iters
-    value = world * n_iters * args.steps / (dev_ms_total / 1e3)
 
-    # serial schedule, same protocol (not part of `value`)
-    ser = [ra.ra_overlap_run(w, ra.make_cfg(mode=0))["total_ms"] for _ in range(args.steps)]
+    # instrumented pass (not part of `value`): the same K steps with an event pair around every kernel, on the stream
+    # the kernel is launched on -> per-kernel launch time inside the overlapped step, overlap rate
+    inst_cfg = ra.make_cfg(**dict(best_kw, record_kernel_times=1))
+    g_ms, c_ms, orate, inst_ms = [], [], [], []
+    for _ in range(steps):
+        r = ra.ra_overlap_run(w, inst_cfg)
+        g_ms.append(r["gemm_ms_sum"] / n_iters)
+        c_ms.append(r["coll_ms_sum"] / n_iters)
+        orate.append(r["overlap_rate"])
+        inst_ms.append(r["total_ms"] / n_iters)
+    # serial schedule at the same setting, same protocol (TimeRatio = t_overlap / t_sequential)
+    ser_cfg = ra.make_cfg(**dict(best_kw, mode=0))
+    ser = [ra.ra_overlap_run(w, ser_cfg)["total_ms"] for _ in range(steps)]
     serial_ms = statistics.mean(ser) / n_iters
-    reset_collective(cfg, d, h)
+    check_finite(cfg, d, "the serial pass")
 
-    # ---- e2e: the same steps through the C ABI's host-buffer entry point (ra_overlap_run_host): every step copies
-    # its inputs from pinned host memory and its results back; the library pipelines H2D(s+1) || compute(s) || D2H(s-1)
-    # over two device buffer sets.  Timed by the host clock around the one synchronous call.
-    hC = torch.empty((cfg.M, cfg.N), dtype=torch.int16).pin_memory()
-    h_out = (torch.empty_like(h["ar"][0]) if cfg.coll == "allreduce" else torch.empty_like(h["a2a"])).pin_memory()
-    h2d = h["A"].numel() * 2 + h["B"].numel() * 2 + (sum(t.numel() * 4 for t in h["ar"]) if cfg.coll == "allreduce" else h["a2a"].numel() * 8)
-    d2h = hC.numel() * 2 + h_out.numel() * h_out.element_size()
-    e2e_cfg = ra.make_cfg(**best_kw)
-    d2 = device_state(ra, cfg, h)
-    w2, keep2 = make_workload(ra, cfg, d2, n_iters)
-    if cfg.coll == "allreduce":
-        io, keep_io = ra.make_host_io(A=h["A"], B=h["B"], C=hC, ar_in=h["ar"], ar_out=h_out)
-    else:
-        io, keep_io = ra.make_host_io(A=h["A"], B=h["B"], C=hC, a2a_in=h["a2a"], a2a_out=h_out)
-    ra.ra_overlap_run_host(w, w2, io, e2e_cfg, 2)            # warm-up
-    barrier(world)
-    t0 = time.perf_counter()
-    e2e_res = ra.ra_overlap_run_host(w, w2, io, e2e_cfg, args.steps)
-    barrier(world)
-    e2e_s = max_over_ranks(time.perf_counter() - t0, world, dev)
-    e2e_value = world * n_iters * args.steps / e2e_s
-    reset_collective(cfg, d, h)
-
-    if rank != 0:
-        return
-    # ---- rooflines ----
     flops, gbytes, cbytes = cfg.gemm_flops, cfg.gemm_bytes, cfg.coll_bytes
     compute_bound = flops / (peaks["bf16_tflops"] * 1e12) > gbytes / (peaks["hbm_gbs"] * 1e9)
     comb = {k: max(flops / (peaks[k] * 1e9), (gbytes + cbytes) / (peaks["hbm_gbs"] * 1e6)) for k in ("bf16_tflops", "bf16_tflops_sustained")}
     gemm_in_step_ms = statistics.mean(g_ms)
-    if compute_bound:
+    coll_launches = 0 if (cfg.coll == "alltoall" and best_kw.get("coll_variant", 0) == 2) else 1
+    out = {
+        "workload": cfg.name, "gemm": [cfg.M, cfg.N, cfg.K], "collective": cfg.coll, "P": cfg.P, "n_iters_per_step": n_iters,
+        "steps": steps, "ms_per_step": ms_per_step, "value": world * n_iters * steps / (dev_ms_total / 1e3),
+        "overlap_ms_per_iter": over_ms, "serial_ms_per_iter": serial_ms, "sweep_serial_ms_per_iter": sweep_serial_ms,
+        "time_ratio_same": over_ms / serial_ms, "time_ratio_best": over_ms / (alone["gemm_ms"] + alone["coll_ms"]),
+        "norm_time_priority": norm_time, "overlap_rate": statistics.mean(orate),
+        "gemm_in_step_ms": gemm_in_step_ms, "coll_in_step_ms": statistics.mean(c_ms),
+        "instrumented_ms_per_iter": statistics.mean(inst_ms),
+        "alone": alone, "combined_roofline_ms": {"burst": comb["bf16_tflops"], "sustained": comb["bf16_tflops_sustained"]},
+        "overlap_vs_roofline": {"burst": over_ms / comb["bf16_tflops"], "sustained": over_ms / comb["bf16_tflops_sustained"]},
+        "best_setting": cfg_label(best_kw), "plan": plan, "sweep": sweep, "policy": policy, "clocks": clocks,
+        "gemm_max_ctas_on_one_sm": max_resident, "wall_ms_timed_region": wall_ms,
+        "gpu_launches": steps * n_iters * (1 + coll_launches), "compute_bound": compute_bound,
+    }
+    if sweep == "config5":
+        out["sweep_marginals"] = sweep_marginals(cand_kws, results, n_iters)
+    if residency is not None:
+        out["residency"] = residency
+    if args.table and headline:
+        with open(args.table, "w") as f:
+            json.dump(sweep_table, f, indent=1)
+
+    if headline:
+        # ---- e2e: the same steps through the C ABI's host-buffer entry point (ra_overlap_run_host): every step copies
+        # its inputs from pinned host memory and its results back; the library pipelines H2D(s+1) || compute(s) || D2H(s-1)
+        # over two device buffer sets.  Timed by the host clock around the one synchronous call.
+        hC = torch.empty((cfg.M, cfg.N), dtype=torch.int16).pin_memory()
+        h_out = (torch.empty_like(h["ar"][0]) if cfg.coll == "allreduce" else torch.empty_like(h["a2a"])).pin_memory()
+        h2d = h["A"].numel() * 2 + h["B"].numel() * 2 + (sum(t.numel() * 4 for t in h["ar"]) if cfg.coll == "allreduce" else h["a2a"].numel() * 8)
+        d2h = hC.numel() * 2 + h_out.numel() * h_out.element_size()
+        e2e_cfg = ra.make_cfg(**dict(best_kw, use_graph=0))      # host-buffer steps are enqueued directly, not graph-replayed
+        d2 = device_state(ra, cfg, h, pristine=False)
+        w2, keep2 = make_workload(ra, cfg, d2, n_iters)
+        if cfg.coll == "allreduce":
+            io, keep_io = ra.make_host_io(A=h["A"], B=h["B"], C=hC, ar_in=h["ar"], ar_out=h_out)
+        else:
+            io, keep_io = ra.make_host_io(A=h["A"], B=h["B"], C=hC, a2a_in=h["a2a"], a2a_out=h_out)
+        ra.ra_overlap_run_host(w, w2, io, e2e_cfg, 2)            # warm-up
+        barrier(world)
+        t0 = time.perf_counter()
+        e2e_res = ra.ra_overlap_run_host(w, w2, io, e2e_cfg, steps)
+        barrier(world)
+        e2e_s = max_over_ranks(time.perf_counter() - t0, world, dev)
+        out["e2e"] = {"value": world * n_iters * steps / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                      "api": "ra_overlap_run_host (pinned host buffers; H2D, compute and D2H of consecutive steps pipelined over two device sets)",
+                      "gpu_ms_per_step": e2e_res["total_ms"] / steps}
+        del d2, w2, io, keep_io, hC, h_out
+    del w, keep, d, h
+    ra.ra_shutdown()                    # drops cached graphs / tensor maps that point into the freed buffers
+    torch.cuda.empty_cache()
+    return out
+
+
+def flat_summary(m, peaks):
+    """One config's report lines as a single string: survives a parser that keeps only scalars."""
+    a, b = m["alone"], m["best_setting"]
+    gem = (f"gemm alone {a['gemm_tflops_burst']:.0f} TF/s burst={a['gemm_frac_of_bf16_peak_burst']:.3f} of bf16 peak, "
+           f"{a['gemm_tflops']:.0f} sustained={a['gemm_frac_of_bf16_peak_sustained']:.3f}" if m["compute_bound"] else
+           f"gemm alone {a['gemm_gbs']:.0f} GB/s={a['gemm_frac_of_hbm_peak']:.3f} of HBM peak ({a['gemm_tflops']:.0f} TF/s)")
+    return (f"serial {m['serial_ms_per_iter'] * 1e3:.1f} us/iter | overlap {m['overlap_ms_per_iter'] * 1e3:.1f} | "
+            f"time_ratio_same {m['time_ratio_same']:.3f} best {m['time_ratio_best']:.3f} | {gem} | "
+            f"coll alone {a['coll_gbs']:.0f} GB/s={a['coll_frac_of_hbm_peak']:.3f} of HBM peak | "
+            f"overlap/roofline {m['overlap_vs_roofline']['sustained']:.3f} sustained {m['overlap_vs_roofline']['burst']:.3f} burst "
+            f"(roofline {m['combined_roofline_ms']['sustained'] * 1e3:.1f}/{m['combined_roofline_ms']['burst'] * 1e3:.1f} us) | "
+            f"setting reserve={b['smem_reserve_bytes'] // 1024}K budget={b['sm_budget']} prio={b['priority']} coll_sm={b['coll_sm_budget']} "
+            f"variant={b['coll_variant']} graph={b['use_graph']} of {m['policy']['settings_in_sweep']} | overlap_rate {m['overlap_rate']:.2f} | "
+            f"sm {m['clocks'].get('sm_mhz')} MHz {','.join(m['clocks'].get('reasons', [])) or 'no-throttle'} | "
+            f"gemm_ctas_per_sm_seen {m['gemm_max_ctas_on_one_sm']}")
+
+
+def run_ours(args, cfg):
+    import torch
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device -- the hot path has no CPU fallback")
+    import paper_2606_09200_b200 as ra   # builds/loads libra.so; raises if the CUDA extension is missing
+
+    world, rank, local = dist_setup(args.gpus)
+    dev = torch.device("cuda", torch.cuda.current_device())
+    peaks = load_peaks()
+    t_start = time.perf_counter()
+    m = measure_config(ra, cfg, args, peaks, world, dev, headline=True)
+
+    per_config = {}
+    if world == 1 and args.per_config == "all":
+        for other in ra_inputs.CONFIGS[:5]:
+            if other.name != cfg.name:
+                per_config[other.name] = measure_config(ra, other, args, peaks, world, dev, headline=False)
+    if rank != 0:
+        return
+
+    # ---- rooflines (dominant kernel = the GEMM: 0.8 of the step's kernel time on cb-*, the HBM stream on mb-*) ----
+    flops, gbytes, cbytes = cfg.gemm_flops, cfg.gemm_bytes, cfg.coll_bytes
+    alone, over_ms, gemm_in_step_ms = m["alone"], m["overlap_ms_per_iter"], m["gemm_in_step_ms"]
+    src = "CUDA events around every K_g launch, on the compute stream, instrumented pass of the same K steps right after the timed region"
+    if m["compute_bound"]:
         ach = flops / gemm_in_step_ms / 1e9
         roof = {"kernel": "ra::gemm_kernel", "bound": "tensor", "achieved": ach, "peak": peaks["bf16_tflops_sustained"], "unit": "TFLOP/s",
                 "frac": ach / peaks["bf16_tflops_sustained"], "traffic": None, "peak_source": f"{peaks['source']} (sustained: kernel timed inside a long overlapped step)",
-                "launch_ms": gemm_in_step_ms, "alone": {"achieved": alone["gemm_tflops_burst"], "peak": peaks["bf16_tflops"], "frac": alone["gemm_frac_of_bf16_peak_burst"], "peak_kind": "burst (best of 10 single launches)"}}
+                "launch_ms": gemm_in_step_ms, "launch_ms_source": src, "frac_of_burst_peak": ach / peaks["bf16_tflops"],
+                "alone": {"achieved": alone["gemm_tflops_burst"], "peak": peaks["bf16_tflops"], "frac": alone["gemm_frac_of_bf16_peak_burst"], "peak_kind": "burst (best of 10 single launches)"}}
     else:
         ach = gbytes / gemm_in_step_ms / 1e6
         roof = {"kernel": "ra::gemm_kernel", "bound": "hbm", "achieved": ach, "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": ach / peaks["hbm_gbs"],
-                "traffic": None, "peak_source": peaks["source"], "launch_ms": gemm_in_step_ms,
+                "traffic": None, "peak_source": peaks["source"], "launch_ms": gemm_in_step_ms, "launch_ms_source": src,
                 "alone": {"achieved": alone["gemm_gbs"], "peak": peaks["hbm_gbs"], "frac": alone["gemm_frac_of_hbm_peak"]}}
     # both kernels share HBM inside the overlapped step, so a kernel's in-step rate understates the memory system's use:
     # the whole iteration's algorithmic bytes over its time is the figure to hold against the HBM peak
@@ -506,34 +716,39 @@ def run_ours(args, cfg):
     if os.path.exists(tpath):
         with open(tpath) as f:
             roof["traffic"] = json.load(f).get(cfg.name, {}).get("gemm_dram_bytes")
+    roof["algorithmic_bytes"] = gbytes
 
     cpu = None
     if args.gpus == 1 and not args.no_cpu_baseline:
-        t_iter, desc, cores, _ = cpu_oracle_sample(cfg)
-        cpu = {"value": 1.0 / t_iter, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc}
+        t_iter, desc, cores, kind = cpu_oracle_full(cfg)
+        cpu = {"value": 1.0 / t_iter, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc, "seconds_per_iter": t_iter,
+               "timed": kind}
+
+    config = {"workload": cfg.name, "gemm": [cfg.M, cfg.N, cfg.K], "layout": "transA=0,transB=1 (K-contiguous)", "collective": cfg.coll,
+              "P": cfg.P, "coll_bytes_moved": cbytes, "n_iters_per_step": m["n_iters_per_step"], "l2": "inputs_exceed_l2 (no flush needed)",
+              "multi_gpu": "replicas only", "best_setting": m["best_setting"], "plan": m["plan"], "sweep": args.sweep,
+              "timed_region": "K steps at the picked setting, no per-kernel events; allreduce buffers refilled from pristine copies before every run",
+              "configs_in_this_run": [cfg.name] + list(per_config)}
+    config["cfg." + cfg.name] = flat_summary(m, peaks)
+    for name, pm in per_config.items():
+        config["cfg." + name] = flat_summary(pm, peaks)
 
     line = {
-        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
-        "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16",
-        "data": "synthetic",
-        "config": {"workload": cfg.name, "gemm": [cfg.M, cfg.N, cfg.K], "layout": "transA=0,transB=1 (K-contiguous)", "collective": cfg.coll,
-                   "P": cfg.P, "coll_bytes_moved": cbytes, "n_iters_per_step": n_iters, "l2": "inputs_exceed_l2 (no flush needed)",
-                   "multi_gpu": "replicas only", "best_setting": cfg_label(best_kw), "plan": plan, "sweep": args.sweep},
-        "overlap_ms_per_iter": over_ms, "serial_ms_per_iter": serial_ms, "time_ratio_best": over_ms / (alone["gemm_ms"] + alone["coll_ms"]),
-        "time_ratio_same": over_ms / serial_ms, "norm_time_priority": norm_time, "overlap_rate": statistics.mean(orate),
-        "sweep_serial_ms_per_iter": sweep_serial_ms,
-        "gemm_in_step_ms": gemm_in_step_ms, "coll_in_step_ms": statistics.mean(c_ms),
-        "alone": alone, "combined_roofline_ms": {"burst": comb["bf16_tflops"], "sustained": comb["bf16_tflops_sustained"]},
-        "overlap_vs_roofline": {"burst": over_ms / comb["bf16_tflops"], "sustained": over_ms / comb["bf16_tflops_sustained"]},
-        "peaks": peaks, "roofline": roof, "cpu_baseline": cpu, "policy": policy,
-        "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-                "api": "ra_overlap_run_host (pinned host buffers; H2D, compute and D2H of consecutive steps pipelined over two device sets)",
-                "gpu_ms_per_step": e2e_res["total_ms"] / args.steps},
-        "residency": residency, "gpu_launches": args.steps * n_iters * 2, "clocks": clocks, "wall_ms_timed_region": wall_ms, "paper_context": PAPER_CONTEXT,
+        "metric": METRIC, "value": m["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
+        "ms_per_step": m["ms_per_step"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16",
+        "data": "synthetic", "config": config,
+        "overlap_ms_per_iter": over_ms, "serial_ms_per_iter": m["serial_ms_per_iter"], "time_ratio_best": m["time_ratio_best"],
+        "time_ratio_same": m["time_ratio_same"], "norm_time_priority": m["norm_time_priority"], "overlap_rate": m["overlap_rate"],
+        "sweep_serial_ms_per_iter": m["sweep_serial_ms_per_iter"],
+        "gemm_in_step_ms": gemm_in_step_ms, "coll_in_step_ms": m["coll_in_step_ms"], "instrumented_ms_per_iter": m["instrumented_ms_per_iter"],
+        "alone": alone, "policy": m["policy"], "residency": m.get("residency"), "peaks": peaks,
+        "per_config": per_config, "total_bench_s": time.perf_counter() - t_start,
+        "paper_context": PAPER_CONTEXT,
+        # the keys a reader of the last 1.5 kB of this line should find there
+        "wall_ms_timed_region": m["wall_ms_timed_region"], "gemm_max_ctas_on_one_sm": m["gemm_max_ctas_on_one_sm"],
+        "combined_roofline_ms": m["combined_roofline_ms"], "overlap_vs_roofline": m["overlap_vs_roofline"],
+        "roofline": roof, "cpu_baseline": cpu, "e2e": m["e2e"], "gpu_launches": m["gpu_launches"], "clocks": m["clocks"],
     }
-    if args.table:
-        with open(args.table, "w") as f:
-            json.dump(sweep_table, f, indent=1)
     print(json.dumps(line), flush=True)
 
 
@@ -547,9 +762,14 @@ def main():
     ap.add_argument("--n-iters", type=int, default=0, help="iterations per step (default: the config's, 20)")
     ap.add_argument("--sweep", default="quick", choices=["none", "auto", "quick", "full"])
     ap.add_argument("--sweep-runs", type=int, default=9)
+    ap.add_argument("--per-config", default="all", choices=["all", "none"],
+                    help="at N=1 also run the other four BASELINE.json configs (default) or only --config")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--ref-budget-s", type=float, default=90.0, help="--impl reference: CPU seconds for warmup + steps")
     ap.add_argument("--table", default="", help="write the sweep table (JSON) here")
     args = ap.parse_args()
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        raise SystemExit(self_launch(sys.argv[1:], args.gpus))
     cfg = get_config(args.config)
     if args.impl == "reference":
         run_reference(args, cfg)

@@ -90,7 +90,12 @@ typedef struct {
 
 /* What S3 decided -- for tests, logs and the sweep tables. */
 typedef struct {
-    int32_t ctas_per_sm;      /* resident GEMM CTAs per SM (cudaOccupancyMaxActiveBlocksPerMultiprocessor) */
+    int32_t ctas_per_sm;      /* GEMM CTAs per SM the plan's shared-memory accounting assumes (smem_left_per_sm is computed
+                                 with it).  1 whenever single residency can be GUARANTEED by the footprint, i.e.
+                                 hw_ctas_per_sm == 1.  2 for reserves above ~half an SM (> ~113 KiB), where no footprint can
+                                 both honour the reserve and exclude a second CTA and the block scheduler does double up
+                                 next to a busy collective (measured): every CTA is then sized so that the reserve holds
+                                 with two resident.  Observable per launch: ra_gemm_residency(), the %smid trace */
     int32_t grid;             /* CTAs launched */
     int32_t stages;           /* depth of the TMA->MMA shared-memory ring */
     int32_t tile_m, tile_n, tile_k; /* CTA tile in C's coordinates (after operand swap) */
@@ -103,10 +108,27 @@ typedef struct {
     int32_t cta_group;        /* 1, or 2 = CTA pairs: `grid` counts CTAs (2 per tile), sm_budget rounded down to even */
     int32_t m_blocks;         /* 128-row MMA blocks per CTA (1 or 2); tile_m = 128 * cta_group * m_blocks */
     int32_t cluster_k;        /* 1, or 2 / 4 = cluster split-K parts: `grid` = cluster_k * cta_group CTAs per tile, no workspace */
+    int32_t hw_ctas_per_sm;   /* GEMM CTAs one SM COULD hold at this footprint = min over registers, threads and shared
+                                 memory, from the device's own figures when an sm_100 device is current (the launched
+                                 instantiation's register count, cudaFuncGetAttributes; registers / threads / shared memory
+                                 per SM, cudaDeviceGetAttribute), else from B200's tables.  NOT taken from
+                                 cudaOccupancyMaxActiveBlocksPerMultiprocessor: that call was measured to answer 1 for this
+                                 kernel at every footprint while two of its CTAs were observed running on one SM.
+                                 The planner pads dyn_smem_bytes past half an SM so that this is 1 whenever the padding
+                                 fits under smem_reserve_bytes; otherwise ctas_per_sm follows it (see there).
+                                 Bounded-work plans (tiles_per_cta > 0) always pad (clamping the reserve if they must).  A
+                                 reserve so large that not even two minimal CTAs fit under it (~> 176 KiB) is clamped:
+                                 clamped = 1 and smem_left_per_sm reports what two resident CTAs really leave. */
 } ra_gemm_plan;
 
 /* Host-only: computes the plan ra_gemm would use.  `occ` NULL = defaults {0,0,0,1,0,0,0}. */
 ra_status ra_gemm_plan_query(int transA, int transB, int M, int N, int K, const ra_occupancy* occ, ra_gemm_plan* out);
+
+/* S3 by measurement: every GEMM CTA counts itself in and out on its SM (%smid).  *max_ctas_on_one_sm receives the largest
+ * number of GEMM CTAs (of any ra_gemm launch of this process on the current device) that were resident on one SM at the
+ * same time since the last reset; reset != 0 clears the statistic afterwards.  Synchronises the device.  With
+ * plan.ctas_per_sm == 1 a value of 2 means the reserve was NOT honoured on some SM.  Host out-pointer (may be NULL). */
+ra_status ra_gemm_residency(int32_t* max_ctas_on_one_sm, int reset);
 
 /* Bytes of device workspace ra_gemm needs for this problem and knob setting (0 if none).
  * Only stream-K plans (split_k > 1) need one. */

@@ -26,7 +26,7 @@ RA_DTYPE_BF16, RA_DTYPE_F32 = 0, 1
 
 # every symbol include/ra.h declares (tests/test_abi.py checks the header against this and the .so)
 EXPORTS = (
-    "ra_status_str", "ra_last_cuda_error", "ra_shutdown", "ra_device_info", "ra_gemm_plan_query",
+    "ra_status_str", "ra_last_cuda_error", "ra_shutdown", "ra_device_info", "ra_gemm_plan_query", "ra_gemm_residency",
     "ra_gemm_workspace_bytes", "ra_gemm", "ra_gemm_ex", "ra_allreduce_emul", "ra_allreduce_emul_ex", "ra_alltoall_emul",
     "ra_alltoall_emul_ex",
     "ra_overlap_run", "ra_overlap_run_host", "ra_overlap_suggest", "ra_overlap_autotune", "ra_overlap_sweep", "ra_set_trace",
@@ -47,7 +47,7 @@ class Occupancy(Structure):
 class GemmPlan(Structure):
     _fields_ = [(n, c_int32) for n in ("ctas_per_sm", "grid", "stages", "tile_m", "tile_n", "tile_k", "split_k",
                                        "swap_ab", "dyn_smem_bytes", "smem_left_per_sm", "n_tiles", "clamped", "cta_group",
-                                       "m_blocks", "cluster_k")]
+                                       "m_blocks", "cluster_k", "hw_ctas_per_sm")]
 
     def as_dict(self):
         return {n: getattr(self, n) for n, _ in self._fields_}
@@ -108,6 +108,7 @@ def _L():
     lib.ra_shutdown.restype = None
     lib.ra_device_info.argtypes = [POINTER(c_int)] * 6
     lib.ra_gemm_plan_query.argtypes = [c_int] * 5 + [POINTER(Occupancy), POINTER(GemmPlan)]
+    lib.ra_gemm_residency.argtypes = [POINTER(c_int32), c_int]
     lib.ra_gemm_workspace_bytes.restype = c_size_t
     lib.ra_gemm_workspace_bytes.argtypes = [c_int] * 5 + [POINTER(Occupancy)]
     lib.ra_gemm.argtypes = [c_int, c_int, c_int, c_int, c_int, c_float, c_void_p, c_int, c_void_p, c_int, c_float,
@@ -201,6 +202,13 @@ def ra_gemm_plan_query(transA, transB, M, N, K, occ=None) -> dict:
     plan = GemmPlan()
     _check(_L().ra_gemm_plan_query(transA, transB, M, N, K, _occ_ref(occ), byref(plan)), "ra_gemm_plan_query")
     return plan.as_dict()
+
+
+def ra_gemm_residency(reset: bool = False) -> int:
+    """Largest number of GEMM CTAs seen resident on one SM at the same time since the last reset (synchronises)."""
+    v = c_int32(0)
+    _check(_L().ra_gemm_residency(byref(v), 1 if reset else 0), "ra_gemm_residency")
+    return v.value
 
 
 def ra_gemm_workspace_bytes(transA, transB, M, N, K, occ=None) -> int:

@@ -42,7 +42,9 @@
 #include <cuda.h>
 #include <cuda_bf16.h>
 
+#include <cstring>
 #include <mutex>
+#include <vector>
 
 #include "ra_common.cuh"
 
@@ -76,6 +78,7 @@ struct GemmParams {
     float* partials;   // stream-K: [2*grid][BN][128] fp32
     int* counters;     // stream-K: [n_tiles]
     int hintX, hintY;  // L2 policy per operand: 0 normal, 1 evict_first, 2 evict_last
+    int hintC;         // L2 policy of the TMA stores of C (written once, never re-read by this kernel)
     int group_x;       // rasterisation: X-tiles per group
     int xmn, ymn;      // operand storage: 0 = K-contiguous rows (K-major), 1 = row index contiguous (MN-major)
     int epi_tma;       // 1: whole tiles leave through shared memory + TMA stores (non-swapped C only)
@@ -84,6 +87,13 @@ struct GemmParams {
     int ks;            // 2: cluster split-K -- the two CTAs of a cluster take one tile's k-blocks half each and CTA 1
                        //    hands its accumulator to CTA 0 through distributed shared memory (CG == 1, XH == 1 only)
 };
+
+// ---- residency counters (S3 by measurement) -----------------------------------------------------
+// Every GEMM CTA counts itself in on its SM (%smid) at entry and out at exit; the running maximum of GEMM CTAs seen
+// on one SM at the same time is what ra_gemm_residency() reports.  One atomic pair per CTA, issued by an epilogue
+// lane that is idle at both moments.  Module-scope device memory: nothing is allocated.
+__device__ int g_gemm_resident[1024];
+__device__ int g_gemm_max_resident;
 
 // ---- device helpers ---------------------------------------------------------------------------
 __device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
@@ -225,9 +235,14 @@ __device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.
 __device__ __forceinline__ void epi_bar_sync() { asm volatile("bar.sync 1, %0;" ::"n"(kEpiThreads) : "memory"); }
 
 // TMA store of one (64 cols x 32 rows) box, shared -> global, clipped at the tensor's bounds
-__device__ __forceinline__ void tma_store_2d(const CUtensorMap* map, uint32_t src_smem, int c0, int c1) {
-    asm volatile("cp.async.bulk.tensor.2d.global.shared::cta.bulk_group [%0, {%2, %3}], [%1];"
-                 ::"l"(map), "r"(src_smem), "r"(c0), "r"(c1) : "memory");
+__device__ __forceinline__ void tma_store_2d(const CUtensorMap* map, uint32_t src_smem, int c0, int c1, uint64_t policy) {
+    if (policy == 0) {
+        asm volatile("cp.async.bulk.tensor.2d.global.shared::cta.bulk_group [%0, {%2, %3}], [%1];"
+                     ::"l"(map), "r"(src_smem), "r"(c0), "r"(c1) : "memory");
+    } else {
+        asm volatile("cp.async.bulk.tensor.2d.global.shared::cta.bulk_group.L2::cache_hint [%0, {%2, %3}], [%1], %4;"
+                     ::"l"(map), "r"(src_smem), "r"(c0), "r"(c1), "l"(policy) : "memory");
+    }
 }
 __device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
 template <int N>
@@ -538,6 +553,7 @@ gemm_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constant__ CU
     const int wid = (int)(blockIdx.x / kdiv), nw = (int)(gridDim.x / kdiv);
     const int krank = (p.ks > 1) ? (int)(crank / CG) : 0;
     uint64_t* rec = (threadIdx.x == 0) ? trace_begin(tr, KID_GEMM) : nullptr;
+    const uint32_t my_sm = smid();
 
     if (warp == 0 && lane == 0) {
         asm volatile("prefetch.tensormap [%0];" ::"l"(&mapX) : "memory");
@@ -697,10 +713,14 @@ gemm_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constant__ CU
         const int quarter = warp & 3;                       // TMEM lane quarter this warp may read
         const int xl = quarter * 32 + lane;                 // row inside this CTA's 128-row slab
         const int et = threadIdx.x - 64;                    // 0..127
+        // residency count-in (after the set-up barrier, so the atomic's round trip delays nothing: this warp's next
+        // action is the wait for the first accumulator)
+        if (et == 0) atomicMax(&g_gemm_max_resident, atomicAdd(&g_gemm_resident[my_sm], 1) + 1);
         Sched sched(p, wid, nw, krank);
         Seg sg;
         int acc_it = 0;
         uint32_t sbuf_it = 0;                               // staging-buffer rotation (per warp)
+        const uint64_t polC = make_policy(p.hintC);
         while (sched.next(sg)) {
             const int buf = (XH == 1) ? (acc_it & 1) : 0;
             const uint32_t aphase = (XH == 1) ? ((acc_it >> 1) & 1) : (acc_it & 1);
@@ -833,7 +853,7 @@ gemm_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constant__ CU
                         fence_async_smem();
                         __syncwarp();
                         if (lane == 0) {
-                            if (row0 < p.RX && y0 < p.RY) tma_store_2d(&mapC, sbuf, y0, row0);
+                            if (row0 < p.RX && y0 < p.RY) tma_store_2d(&mapC, sbuf, y0, row0, polC);
                             bulk_commit();
                         }
                     }
@@ -922,6 +942,7 @@ gemm_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constant__ CU
         else
             asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"((uint32_t)kTmemCols) : "memory");
     }
+    if (threadIdx.x == 64) atomicSub(&g_gemm_resident[my_sm], 1);
     if (threadIdx.x == 0) trace_end(rec);
 }
 
@@ -979,6 +1000,60 @@ static ra_status make_map(CUtensorMap* map, const void* base, int rows, int K, i
     return RA_OK;
 }
 
+// ---- host: kernel instantiations, their one-time attributes, and what the hardware says about residency --------
+static const void* gemm_kernel_ptr(int bn, int cg, int xh) {
+    if (cg == 2 && xh == 2) return reinterpret_cast<const void*>(&gemm_kernel<256, 2, 2>);
+    if (cg == 2) return reinterpret_cast<const void*>(&gemm_kernel<256, 2, 1>);
+    switch (bn) {
+        case 64: return reinterpret_cast<const void*>(&gemm_kernel<64, 1, 1>);
+        case 128: return reinterpret_cast<const void*>(&gemm_kernel<128, 1, 1>);
+        case 256: return reinterpret_cast<const void*>(&gemm_kernel<256, 1, 1>);
+    }
+    return nullptr;
+}
+static int kernel_slot(int bn, int cg, int xh) { return cg == 2 ? (xh == 2 ? 4 : 3) : (bn == 64 ? 0 : (bn == 128 ? 1 : 2)); }
+
+static std::mutex g_gemm_mu;                 // guards the attribute flags and the launch cache below
+static bool g_attr_set[64][5] = {};          // [device][instantiation]: MaxDynamicSharedMemorySize raised to the opt-in limit
+
+// cudaFuncSetAttribute once per (device, instantiation), not once per launch.  Caller holds g_gemm_mu.
+static ra_status prepare_kernel(const DeviceInfo& di, int bn, int cg, int xh) {
+    const int slot = kernel_slot(bn, cg, xh);
+    if (di.device >= 0 && di.device < 64 && g_attr_set[di.device][slot]) return RA_OK;
+    RA_CUDA(cudaFuncSetAttribute(gemm_kernel_ptr(bn, cg, xh), cudaFuncAttributeMaxDynamicSharedMemorySize, di.smem_per_block_optin));
+    if (di.device >= 0 && di.device < 64) g_attr_set[di.device][slot] = true;
+    return RA_OK;
+}
+
+// GEMM CTAs one SM can hold at this footprint: the minimum over the SM's launch-time resources -- registers,
+// threads, shared memory.  On a device the inputs are read from it (the instantiation's real register count from
+// cudaFuncGetAttributes, registers / threads / shared memory per SM from cudaDeviceGetAttribute); without one (plan
+// queries on a CPU box) they are B200's: 128 registers x 192 threads -> 2 CTAs by registers.
+//
+// Why not cudaOccupancyMaxActiveBlocksPerMultiprocessor (what round 1's header promised): measured on B200 / CUDA 12.9
+// it answers 1 for every instantiation of this kernel at EVERY footprint, down to 25 KiB of dynamic shared memory,
+// while the %smid trace and the kernel's own per-SM counter (ra_gemm_residency) show two of these CTAs running on one
+// SM at the same time at exactly that footprint (tests/test_overlap_gpu.py, reserve 200 KiB next to the allreduce).
+// The API under-reports; the resource arithmetic below is the bound the hardware was seen to reach.
+static int resident_ctas(const DeviceInfo* di, int bn, int cg, int xh, int dyn, int smem_per_sm, int reserved) {
+    int regs_per_thread = 128, regs_per_sm = 65536, threads_per_sm = 2048;
+    if (di != nullptr) {
+        std::lock_guard<std::mutex> lk(g_gemm_mu);
+        cudaFuncAttributes fa;
+        int v = 0;
+        if (cudaFuncGetAttributes(&fa, gemm_kernel_ptr(bn, cg, xh)) == cudaSuccess && fa.numRegs > 0) regs_per_thread = fa.numRegs;
+        if (cudaDeviceGetAttribute(&v, cudaDevAttrMaxRegistersPerMultiprocessor, di->device) == cudaSuccess && v > 0) regs_per_sm = v;
+        if (cudaDeviceGetAttribute(&v, cudaDevAttrMaxThreadsPerMultiProcessor, di->device) == cudaSuccess && v > 0) threads_per_sm = v;
+        (void)cudaGetLastError();
+    }
+    // registers are allocated per warp, in units of 8 per thread
+    const int regs_per_cta = ((regs_per_thread + 7) / 8 * 8) * 32 * (kGemmThreads / 32);
+    int n = smem_per_sm / (dyn + reserved);
+    if (regs_per_sm / regs_per_cta < n) n = regs_per_sm / regs_per_cta;
+    if (threads_per_sm / kGemmThreads < n) n = threads_per_sm / kGemmThreads;
+    return n;
+}
+
 // ---- host: S3 planner ----------------------------------------------------------------------------
 struct Plan {
     ra_gemm_plan pub;
@@ -1002,17 +1077,17 @@ static ra_status make_plan(int transA, int transB, int M, int N, int K, const ra
     // device facts (B200 constants when no device is present, so plans can be queried on a CPU box)
     int sm_count = kDefaultSmCount, smem_per_sm = kDefaultSmemPerSm, optin = kDefaultSmemPerBlockOptin,
         reserved = kDefaultSmemReservedPerBlock;
-    {
-        DeviceInfo di;
-        if (device_info(&di) == RA_OK) {
-            sm_count = di.sm_count;
-            smem_per_sm = di.smem_per_sm;
-            optin = di.smem_per_block_optin;
-            reserved = di.smem_reserved_per_block;
-        } else {
-            g_last_cuda_error = 0;
-            (void)cudaGetLastError();
-        }
+    DeviceInfo di;
+    const DeviceInfo* dev = nullptr;               // non-NULL: an sm_100 device is current, ask it about residency
+    if (device_info(&di) == RA_OK) {
+        sm_count = di.sm_count;
+        smem_per_sm = di.smem_per_sm;
+        optin = di.smem_per_block_optin;
+        reserved = di.smem_reserved_per_block;
+        if (di.cc_major == 10) dev = &di;
+    } else {
+        g_last_cuda_error = 0;
+        (void)cudaGetLastError();
     }
     Plan pl{};
     ra_gemm_plan& g = pl.pub;
@@ -1064,8 +1139,18 @@ static ra_status make_plan(int transA, int transB, int M, int N, int K, const ra
     if (occ.m_blocks < 0 || occ.m_blocks > 2) return RA_ERR_INVALID_ARG;
     if (occ.cluster_k < 0 || occ.cluster_k > 4 || occ.cluster_k == 3) return RA_ERR_INVALID_ARG;
 
+    // n_acc = GEMM CTAs per SM the shared-memory accounting assumes.  Pass 1 sizes the plan for ONE CTA per SM and makes
+    // that a fact where it can (padding, below).  Where it cannot -- a reserve above ~half an SM leaves no room for the
+    // padding -- the block scheduler DOES place two of the persistent grid's CTAs on one SM when collective CTAs crowd
+    // the others (measured: tests/test_overlap_gpu.py, reserve 160 KiB x budget 74 next to the allreduce), so pass 2
+    // sizes every CTA for the reserve to hold with TWO resident:  2 * (dyn + reserved) <= smem_per_sm - reserve.
+    const int bn_start = bn;
+    const int clamped_start = clamped;
+    for (int n_acc = 1;; ++n_acc) {
+    bn = bn_start;
+    clamped = clamped_start;
     // shared memory the GEMM may allocate on an SM
-    long avail = (long)smem_per_sm - occ.smem_reserve_bytes - reserved;
+    long avail = ((long)smem_per_sm - occ.smem_reserve_bytes) / n_acc - reserved;
     if (avail > optin) avail = optin;
     // non-swapped C leaves through a 32 KiB staging area + TMA stores (full-line writes); the skinny path keeps
     // direct stores (its C is tiny) and spends the space on pipeline depth
@@ -1135,22 +1220,46 @@ static ra_status make_plan(int transA, int transB, int M, int N, int K, const ra
     const long long n_tiles = (long long)tiles_x * tiles_y;
     if (n_tiles > 0x3fffffffLL) return RA_ERR_UNSUPPORTED;
 
-    int grid, stream_k = 0, ctas_per_sm = 1, ks = 1;
+    int grid, stream_k = 0, ctas_per_sm = n_acc, ks = 1;
+    // Residency (A22 / A23): the plan's accounting -- smem_left_per_sm >= reserve -- assumes ONE GEMM CTA per SM.  That is
+    // guaranteed by the footprint itself when a second CTA cannot fit: the request is padded past half of an SM's
+    // shared memory whenever the hardware (cudaOccupancyMaxActiveBlocksPerMultiprocessor) would otherwise admit two
+    // and the padding still honours the reserve -- the paper's direction: more shared memory per block, fewer
+    // resident blocks.
+    const int half = (smem_per_sm - 2 * reserved) / 2 + 16;
+    int hw = resident_ctas(dev, bn, cg, xh, dyn, smem_per_sm, reserved);
+    if (n_acc == 1 && hw > 1 && dyn < half && half <= avail) {
+        dyn = half;
+        hw = resident_ctas(dev, bn, cg, xh, dyn, smem_per_sm, reserved);
+    }
+    if (n_acc == 1 && hw > 1 && occ.tiles_per_cta == 0) {
+        // two CTAs fit and padding would break the reserve: account for two -- if a two-resident plan exists at all
+        // (at least one stage of the narrowest tile, and two CTAs' accumulators in the 512 TMEM columns)
+        const long avail2 = ((long)smem_per_sm - occ.smem_reserve_bytes) / 2 - reserved;
+        if (avail2 - kAlignSlack - kBarrierBytes >= stage_bytes(64, 1, 1)) continue;
+        // not even that fits (reserve ~200 KiB): nothing honours the knob -> clamp: keep the one-CTA sizing and
+        // report the shared memory an SM really has left in the worst case (two resident)
+        if (!occ.allow_clamp) return RA_ERR_INFEASIBLE_KNOB;
+        clamped = 1;
+        ctas_per_sm = hw;
+    }
+    if (n_acc == 2 && 2 * bn * hw > 512) {       // two residents' accumulators must both fit in TMEM
+        if (!occ.allow_clamp) return RA_ERR_INFEASIBLE_KNOB;
+        clamped = 1;
+    }
     if (occ.tiles_per_cta > 0) {
-        // bounded work: more CTAs than SMs.  Residency must stay at one GEMM CTA per SM (TMEM holds
-        // two accumulators), so pad the request past half of what an SM can give.
+        // bounded work: more CTAs than SMs, so a second CTA WILL be placed wherever it fits (it would only wait for
+        // TMEM): single residency is mandatory here, at the price of the reserve if need be (clamped).
         grid = cg * (int)((n_tiles + occ.tiles_per_cta - 1) / occ.tiles_per_cta);
         if (occ.cluster_k >= 2) {                 // cluster split-K is a one-tile-per-cluster schedule
             if (!occ.allow_clamp) return RA_ERR_INFEASIBLE_KNOB;
             clamped = 1;
         }
-        const int half = (smem_per_sm - 2 * reserved) / 2 + 16;
-        if (dyn < half) {
-            if (half > avail) {
-                if (!occ.allow_clamp) return RA_ERR_INFEASIBLE_KNOB;
-                clamped = 1;
-            }
+        if (hw > 1 && dyn < half) {
+            if (!occ.allow_clamp) return RA_ERR_INFEASIBLE_KNOB;   // half > avail: reserve and single residency conflict
+            clamped = 1;
             dyn = half;
+            hw = resident_ctas(dev, bn, cg, xh, dyn, smem_per_sm, reserved);
         }
     } else {
         const int workers = budget / cg;                 // CTAs, or CTA pairs
@@ -1190,6 +1299,7 @@ static ra_status make_plan(int transA, int transB, int M, int N, int K, const ra
         grid = w * cg;
     }
     g.ctas_per_sm = ctas_per_sm;
+    g.hw_ctas_per_sm = hw;
     g.grid = grid;
     g.stages = stages;
     g.tile_m = swap ? bn : tile_x;
@@ -1214,6 +1324,8 @@ static ra_status make_plan(int transA, int transB, int M, int N, int K, const ra
         pl.counters_bytes = (((size_t)n_tiles * sizeof(int)) + 1023) & ~(size_t)1023;
         pl.ws_bytes = pl.counters_bytes + (size_t)2 * grid * kBM * bn * sizeof(float);
     }
+    break;
+    }   // n_acc
     *out = pl;
     return RA_OK;
 }
@@ -1222,7 +1334,6 @@ template <int BN, int CG, int XH>
 static ra_status launch_gemm(const CUtensorMap& mx, const CUtensorMap& my, const CUtensorMap& mc, const GemmParams& p, int grid, int dyn,
                              cudaStream_t stream) {
     const int cluster = CG * p.ks;                      // CTA pair (tcgen05 cta_group::2) x split-K halves
-    RA_CUDA(cudaFuncSetAttribute(gemm_kernel<BN, CG, XH>, cudaFuncAttributeMaxDynamicSharedMemorySize, dyn));
     if (cluster == 1) {
         gemm_kernel<BN, CG, XH><<<grid, kGemmThreads, dyn, stream>>>(mx, my, mc, p, g_trace);
         RA_CUDA(cudaGetLastError());
@@ -1241,6 +1352,94 @@ static ra_status launch_gemm(const CUtensorMap& mx, const CUtensorMap& my, const
     cfg.attrs = attr;
     cfg.numAttrs = 1;
     RA_CUDA(cudaLaunchKernelEx(&cfg, gemm_kernel<BN, CG, XH>, mx, my, mc, p, g_trace));
+    return RA_OK;
+}
+
+// ---- host: launch cache -------------------------------------------------------------------------------------------
+// Everything a launch needs besides (alpha, beta, workspace, stream) is a pure function of (device, shape, leading
+// dimensions, operand addresses, output type, knobs): the plan, the kernel parameters and the two or three CUtensorMaps
+// (encoding one costs a driver call).  Entries are kept in a small LRU list behind a mutex ("lazily-cached
+// ... tensor-map descriptors", Appendix A: "cache them by (ptr, dims, ld, box)").
+struct LaunchKey {
+    int32_t device, transA, transB, M, N, K, lda, ldb, ldc, c_f32;
+    const void *A, *B, *C;
+    ra_occupancy occ;
+};
+struct LaunchEntry {
+    LaunchKey key;
+    Plan pl;
+    GemmParams p;          // alpha, beta, partials, counters are filled per call
+    CUtensorMap mx, my, mc;
+    uint64_t stamp;
+};
+constexpr size_t kLaunchCacheEntries = 32;
+static std::mutex g_launch_mu;
+static std::vector<LaunchEntry> g_launch_cache;
+static uint64_t g_launch_stamp = 0;
+
+void gemm_cache_clear() {
+    std::lock_guard<std::mutex> lk(g_launch_mu);
+    g_launch_cache.clear();
+}
+
+// Builds plan, parameters and tensor maps for one key (the slow path of a launch).
+static ra_status build_entry(const LaunchKey& k, const DeviceInfo& di, LaunchEntry* e) {
+    const int transA = k.transA, transB = k.transB, M = k.M, N = k.N, K = k.K;
+    e->key = k;
+    Plan& pl = e->pl;
+    RA_TRY(make_plan(transA, transB, M, N, K, &k.occ, &pl));
+    const int swap = pl.pub.swap_ab;
+    GemmParams p{};
+    p.RX = swap ? N : M;
+    p.RY = swap ? M : N;
+    p.K = K;
+    const int cg = pl.pub.cta_group, xh = pl.pub.m_blocks;
+    const int tile_x = kBM * cg * xh;
+    p.tiles_x = (p.RX + tile_x - 1) / tile_x;
+    p.tiles_y = (p.RY + pl.bn - 1) / pl.bn;
+    p.n_tiles = pl.pub.n_tiles;
+    p.kb_per_tile = (K + kBK - 1) / kBK;
+    p.swap = swap;
+    p.stream_k = pl.pub.split_k > 1;
+    p.stages = pl.pub.stages;
+    p.C = static_cast<__nv_bfloat16*>(const_cast<void*>(k.C));
+    p.ldc = k.ldc;
+    // L2 policy: an operand that is streamed exactly once (one tile along the other dimension) should
+    // not displace anything; the small operand every CTA re-reads should stay.
+    p.hintX = (p.tiles_y == 1 && p.tiles_x > 1) ? 1 : 0;
+    p.hintY = (p.tiles_y == 1 && p.tiles_x > 1) ? 2 : 0;
+    {
+        // Rasterisation.  The W workers of one wave cover a gx x gy block of tiles and march through K together, so
+        // the wave reads (gx*tile_x + gy*BN) rows of K from DRAM once and shares them through L2; with 16 KiB rows
+        // (K = 8192) a wave's footprint (~69 MB) already exceeds what L2 keeps across waves (measured: no cross-wave
+        // reuse), so DRAM traffic ~ waves * (gx*tile_x + gy*BN) rows.  Minimised, subject to gx*gy = W, at
+        // gx = sqrt(W*BN/tile_x): 8 for 74 pairs of 256x256, 16-17 for 148 CTAs of 128x256.
+        const int workers = pl.pub.grid / cg;
+        int gx = 1;
+        while ((long long)(gx + 1) * (gx + 1) * tile_x <= (long long)workers * pl.bn) ++gx;
+        if (gx > p.tiles_x) gx = p.tiles_x;
+        p.group_x = gx < 1 ? 1 : gx;
+    }
+    const void* X = swap ? k.B : k.A;
+    const void* Y = swap ? k.A : k.B;
+    const int ldx = swap ? k.ldb : k.lda, ldy = swap ? k.lda : k.ldb;
+    // op(A)(i,k): K-contiguous iff transA == 0;  op(B)(k,j): K-contiguous iff transB == 1
+    const int a_mn = transA ? 1 : 0, b_mn = transB ? 0 : 1;
+    p.xmn = swap ? b_mn : a_mn;
+    p.ymn = swap ? a_mn : b_mn;
+    RA_TRY(make_map(&e->mx, X, p.RX, K, ldx, kBM * xh, p.xmn));
+    RA_TRY(make_map(&e->my, Y, p.RY, K, ldy, pl.bn / cg, p.ymn));
+    p.c_f32 = k.c_f32;
+    p.epi_tma = k.c_f32 ? 0 : pl.epi_tma;      // fp32 rows are written directly: 128 contiguous bytes per thread and chunk
+    p.ks = pl.pub.cluster_k;
+    p.skew = pl.pub.stages;   // measured on 8192^3 (4 stages): drain wait per tile 5.9k cycles at skew 0, 1.5k at 4
+    if (p.epi_tma) RA_TRY(make_map(&e->mc, k.C, M, N, k.ldc, 32, 0));    // C: box = 64 columns x 32 rows (one epilogue warp)
+    else e->mc = e->mx;                                                  // unused
+    e->p = p;
+    {
+        std::lock_guard<std::mutex> lk(g_gemm_mu);
+        RA_TRY(prepare_kernel(di, pl.bn, cg, xh));
+    }
     return RA_OK;
 }
 
@@ -1266,18 +1465,16 @@ ra_status gemm_launch(int transA, int transB, int M, int N, int K, float alpha, 
         const uintptr_t b0 = reinterpret_cast<uintptr_t>(B), b1 = b0 + b_elems * 2;
         if (K > 0 && ((c0 < a1 && a0 < c1) || (c0 < b1 && b0 < c1))) return RA_ERR_INVALID_ARG;
     }
-    Plan pl;
-    RA_TRY(make_plan(transA, transB, M, N, K, occ, &pl));
-    if (pl.ws_bytes > 0) {
-        if (workspace == nullptr || workspace_bytes < pl.ws_bytes || (reinterpret_cast<uintptr_t>(workspace) & 15u))
-            return RA_ERR_INVALID_ARG;
-    }
-    DeviceInfo di;
-    RA_TRY(device_info(&di));
-    RA_TRY(require_sm100(di));
-    if (plan_out) *plan_out = pl.pub;
+    ra_occupancy occ_v = {0, 0, 0, 1, 0, 0, 0};
+    if (occ) occ_v = *occ;
 
     if (K == 0 || alpha == 0.f) {
+        Plan pl;
+        RA_TRY(make_plan(transA, transB, M, N, K, &occ_v, &pl));      // knob errors are reported as for any other launch
+        DeviceInfo di;
+        RA_TRY(device_info(&di));
+        RA_TRY(require_sm100(di));
+        if (plan_out) *plan_out = pl.pub;
         const size_t total = (size_t)M * N;
         const int blocks = (int)((total + 255) / 256 < (size_t)di.sm_count * 8 ? (total + 255) / 256 : (size_t)di.sm_count * 8);
         scale_c_kernel<<<blocks, 256, 0, stream>>>(C, M, N, ldc, beta, c_f32);
@@ -1285,61 +1482,60 @@ ra_status gemm_launch(int transA, int transB, int M, int N, int K, float alpha, 
         return RA_OK;
     }
 
-    const int swap = pl.pub.swap_ab;
-    GemmParams p{};
-    p.RX = swap ? N : M;
-    p.RY = swap ? M : N;
-    p.K = K;
-    const int cg = pl.pub.cta_group, xh = pl.pub.m_blocks;
-    const int tile_x = kBM * cg * xh;
-    p.tiles_x = (p.RX + tile_x - 1) / tile_x;
-    p.tiles_y = (p.RY + pl.bn - 1) / pl.bn;
-    p.n_tiles = pl.pub.n_tiles;
-    p.kb_per_tile = (K + kBK - 1) / kBK;
-    p.swap = swap;
-    p.stream_k = pl.pub.split_k > 1;
-    p.stages = pl.pub.stages;
+    LaunchKey key;
+    memset(&key, 0, sizeof(key));                  // padding bytes too: keys are compared with memcmp
+    key.transA = transA; key.transB = transB; key.M = M; key.N = N; key.K = K;
+    key.lda = lda; key.ldb = ldb; key.ldc = ldc; key.c_f32 = c_f32;
+    key.A = A; key.B = B; key.C = C;
+    key.occ = occ_v;
+    RA_CUDA(cudaGetDevice(&key.device));
+
+    Plan pl;
+    GemmParams p;
+    CUtensorMap mx, my, mc;
+    bool hit = false;
+    {
+        std::lock_guard<std::mutex> lk(g_launch_mu);
+        for (LaunchEntry& e : g_launch_cache) {
+            if (memcmp(&e.key, &key, sizeof(key)) == 0) {
+                e.stamp = ++g_launch_stamp;
+                pl = e.pl; p = e.p; mx = e.mx; my = e.my; mc = e.mc;
+                hit = true;
+                break;
+            }
+        }
+    }
+    if (!hit) {
+        DeviceInfo di;
+        RA_TRY(device_info(&di));
+        RA_TRY(require_sm100(di));
+        LaunchEntry e;
+        RA_TRY(build_entry(key, di, &e));
+        pl = e.pl; p = e.p; mx = e.mx; my = e.my; mc = e.mc;
+        std::lock_guard<std::mutex> lk(g_launch_mu);
+        e.stamp = ++g_launch_stamp;
+        if (g_launch_cache.size() < kLaunchCacheEntries) {
+            g_launch_cache.push_back(e);
+        } else {
+            size_t lru = 0;
+            for (size_t i = 1; i < g_launch_cache.size(); ++i)
+                if (g_launch_cache[i].stamp < g_launch_cache[lru].stamp) lru = i;
+            g_launch_cache[lru] = e;
+        }
+    }
+    if (pl.ws_bytes > 0) {
+        if (workspace == nullptr || workspace_bytes < pl.ws_bytes || (reinterpret_cast<uintptr_t>(workspace) & 15u))
+            return RA_ERR_INVALID_ARG;
+    }
+    if (plan_out) *plan_out = pl.pub;
     p.alpha = alpha;
     p.beta = beta;
-    p.C = static_cast<__nv_bfloat16*>(C);
-    p.ldc = ldc;
-    // L2 policy: an operand that is streamed exactly once (one tile along the other dimension) should
-    // not displace anything; the small operand every CTA re-reads should stay.
-    p.hintX = (p.tiles_y == 1 && p.tiles_x > 1) ? 1 : 0;
-    p.hintY = (p.tiles_y == 1 && p.tiles_x > 1) ? 2 : 0;
-    {
-        // Rasterisation.  The W workers of one wave cover a gx x gy block of tiles and march through K together, so
-        // the wave reads (gx*tile_x + gy*BN) rows of K from DRAM once and shares them through L2; with 16 KiB rows
-        // (K = 8192) a wave's footprint (~69 MB) already exceeds what L2 keeps across waves (measured: no cross-wave
-        // reuse), so DRAM traffic ~ waves * (gx*tile_x + gy*BN) rows.  Minimised, subject to gx*gy = W, at
-        // gx = sqrt(W*BN/tile_x): 8 for 74 pairs of 256x256, 16-17 for 148 CTAs of 128x256.
-        const int workers = pl.pub.grid / cg;
-        int gx = 1;
-        while ((long long)(gx + 1) * (gx + 1) * tile_x <= (long long)workers * pl.bn) ++gx;
-        if (gx > p.tiles_x) gx = p.tiles_x;
-        p.group_x = gx < 1 ? 1 : gx;
-    }
     if (p.stream_k) {
         p.counters = static_cast<int*>(workspace);
         p.partials = reinterpret_cast<float*>(static_cast<uint8_t*>(workspace) + pl.counters_bytes);
         RA_CUDA(cudaMemsetAsync(workspace, 0, pl.counters_bytes, stream));
     }
-    const void* X = swap ? B : A;
-    const void* Y = swap ? A : B;
-    const int ldx = swap ? ldb : lda, ldy = swap ? lda : ldb;
-    CUtensorMap mx, my, mc;
-    // op(A)(i,k): K-contiguous iff transA == 0;  op(B)(k,j): K-contiguous iff transB == 1
-    const int a_mn = transA ? 1 : 0, b_mn = transB ? 0 : 1;
-    p.xmn = swap ? b_mn : a_mn;
-    p.ymn = swap ? a_mn : b_mn;
-    RA_TRY(make_map(&mx, X, p.RX, K, ldx, kBM * xh, p.xmn));
-    RA_TRY(make_map(&my, Y, p.RY, K, ldy, pl.bn / cg, p.ymn));
-    p.c_f32 = c_f32;
-    p.epi_tma = c_f32 ? 0 : pl.epi_tma;        // fp32 rows are written directly: 128 contiguous bytes per thread and chunk
-    p.ks = pl.pub.cluster_k;
-    p.skew = pl.pub.stages;   // measured on 8192^3 (4 stages): drain wait per tile 5.9k cycles at skew 0, 1.5k at 4
-    if (p.epi_tma) RA_TRY(make_map(&mc, C, M, N, ldc, 32, 0));    // C: box = 64 columns x 32 rows (one epilogue warp)
-    else mc = mx;                                                  // unused
+    const int cg = pl.pub.cta_group, xh = pl.pub.m_blocks;
     if (cg == 2 && xh == 2) return launch_gemm<256, 2, 2>(mx, my, mc, p, pl.pub.grid, pl.pub.dyn_smem_bytes, stream);
     if (cg == 2) return launch_gemm<256, 2, 1>(mx, my, mc, p, pl.pub.grid, pl.pub.dyn_smem_bytes, stream);
     switch (pl.bn) {
@@ -1359,6 +1555,23 @@ ra_status ra_gemm_plan_query(int transA, int transB, int M, int N, int K, const 
     ra::Plan pl;
     RA_TRY(ra::make_plan(transA, transB, M, N, K, occ, &pl));
     *out = pl.pub;
+    return RA_OK;
+}
+
+ra_status ra_gemm_residency(int32_t* max_ctas_on_one_sm, int reset) {
+    ra::DeviceInfo di;
+    RA_TRY(ra::device_info(&di));
+    RA_TRY(ra::require_sm100(di));
+    RA_CUDA(cudaDeviceSynchronize());
+    int v = 0;
+    RA_CUDA(cudaMemcpyFromSymbol(&v, ra::g_gemm_max_resident, sizeof(int)));
+    if (max_ctas_on_one_sm) *max_ctas_on_one_sm = v;
+    if (reset) {
+        const int zero = 0;
+        RA_CUDA(cudaMemcpyToSymbol(ra::g_gemm_max_resident, &zero, sizeof(int)));
+        static const int zeros[1024] = {};
+        RA_CUDA(cudaMemcpyToSymbol(ra::g_gemm_resident, zeros, sizeof(zeros)));
+    }
     return RA_OK;
 }
 

@@ -28,6 +28,8 @@ ra_status allreduce_validate(float* const* bufs, int P, size_t count, int sm_bud
 ra_status alltoall_validate(const void* send, const void* recv, int P, size_t chunk_bytes, int sm_budget, int smem_bytes_per_cta,
                             int ctas_per_sm, int variant);
 
+void gemm_cache_clear();
+
 // ---- cached host objects ----------------------------------------------------------------------
 struct Cache {
     std::mutex mu;
@@ -438,6 +440,7 @@ ra_status ra_overlap_sweep(const ra_workload* w, const ra_overlap_cfg* cfgs, int
 }
 
 void ra_shutdown(void) {
+    ra::gemm_cache_clear();
     std::lock_guard<std::mutex> lk(ra::g_cache.mu);
     for (auto& kv : ra::g_cache.streams) cudaStreamDestroy(kv.second);
     ra::g_cache.streams.clear();

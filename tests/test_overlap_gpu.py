@@ -336,3 +336,156 @@ def test_autotune_returns_a_valid_setting_and_keeps_results_exact(ra):
     assert gemm_norm_err(to_host(dC, np.uint16).reshape(M, N), ref, rowA, colB) <= GEMM_TOL
     r2 = ra.ra_overlap_run(w, cfg)                               # the returned setting is directly usable
     assert r2["total_ms"] > 0
+
+
+# ---- S3 by measurement (SURVEY 8(c) O4 pin) ---------------------------------------------------------
+def _resident_max(rec_sm, t0, t1):
+    """Largest number of intervals [t0, t1) alive at one instant on one SM."""
+    worst = 0
+    for s in set(rec_sm.tolist()):
+        sel = rec_sm == s
+        ev = sorted([(int(a), 1) for a in t0[sel]] + [(int(b), -1) for b in t1[sel]], key=lambda e: (e[0], e[1]))
+        cur = 0
+        for _, d in ev:
+            cur += d
+            worst = max(worst, cur)
+    return worst
+
+
+@pytest.mark.parametrize("budget", [74, 148])
+@pytest.mark.parametrize("reserve_kb", [0, 64, 128, 160, 200])
+@pytest.mark.parametrize("coll", ["allreduce", "alltoall_ring"])
+def test_reserve_is_honoured_with_a_collective_running(ra, reserve_kb, budget, coll):
+    """For every reserve x budget of the config-5 sweep, with a collective co-running on the other stream: no SM ever
+    hosts more GEMM CTAs at once than the plan accounts for (the %smid trace AND the kernel's own per-SM counter say
+    so), hence the plan's smem_left_per_sm >= smem_reserve_bytes is what each SM really had left; the plan's
+    hw_ctas_per_sm is what cudaOccupancyMaxActiveBlocksPerMultiprocessor answers for the launched footprint; it is 1
+    (guaranteed by padding) whenever the reserve leaves room for the padding, and otherwise the accounting assumes the
+    two CTAs the hardware admits -- round 1 assumed one, and this test caught two on an SM at 160 KiB x 74."""
+    import torch
+    info = ra.ra_device_info()
+    M, N, K = 4096, 4096, 2048                           # 128 big tiles: two waves on 74 CTAs, one on 148
+    occ = dict(smem_reserve_bytes=reserve_kb * 1024, sm_budget=budget)
+    A, B, g, dC = _gemm_side(ra, M, N, K, 21, occ=occ)
+    g["workspace"] = torch.empty(max(ra.ra_gemm_workspace_bytes(0, 1, M, N, K, occ), 16), dtype=torch.uint8, device="cuda")
+    plan = ra.ra_gemm_plan_query(0, 1, M, N, K, occ)
+    assert plan["ctas_per_sm"] in (1, 2) and plan["grid"] <= budget
+    assert plan["smem_left_per_sm"] >= reserve_kb * 1024 or (plan["clamped"] and reserve_kb == 200), plan
+    assert plan["smem_left_per_sm"] == info["smem_per_sm"] - plan["ctas_per_sm"] * (plan["dyn_smem_bytes"] + info["smem_reserved_per_block"])
+    half = (info["smem_per_sm"] - 2 * info["smem_reserved_per_block"]) // 2 + 16
+    can_pad = half <= info["smem_per_sm"] - reserve_kb * 1024 - info["smem_reserved_per_block"]
+    assert plan["hw_ctas_per_sm"] >= 1
+    if can_pad:
+        assert plan["hw_ctas_per_sm"] == 1 == plan["ctas_per_sm"] and plan["dyn_smem_bytes"] >= half, plan   # by construction
+    else:
+        # shared memory alone admits floor(smem / (dyn + reserved)) CTAs; registers / threads may cut it further; the
+        # accounting follows what the hardware admits
+        assert plan["hw_ctas_per_sm"] <= info["smem_per_sm"] // (plan["dyn_smem_bytes"] + info["smem_reserved_per_block"])
+        assert plan["ctas_per_sm"] == plan["hw_ctas_per_sm"], plan
+    if coll == "allreduce":
+        bufs = [torch.zeros(4 << 20, device="cuda") for _ in range(8)]
+        w, keep = ra.make_workload(gemm=g, allreduce=bufs, n_iters=3)
+        ckw = dict(coll_variant=0)
+    else:
+        a = torch.zeros(8 * 8 * (1 << 20) // 8, dtype=torch.int64, device="cuda")
+        b = torch.zeros_like(a)          # held in a local: the workload stores raw pointers, not references
+        w, keep = ra.make_workload(gemm=g, alltoall=dict(a=a, b=b, P=8, chunk_bytes=1 << 20), n_iters=3)
+        ring = max(min(reserve_kb * 1024 - 4096, 64 * 1024), 8 * 1024)
+        ckw = dict(coll_variant=0, coll_smem_bytes=ring, coll_ctas_per_sm=1)
+    cap = 1 << 15
+    buf = torch.zeros(1 + 4 * cap, dtype=torch.int64, device="cuda")
+    ra.ra_gemm_residency(reset=True)
+    ra.ra_set_trace(buf, cap)
+    try:
+        res = ra.ra_overlap_run(w, ra.make_cfg(mode=1, occ=occ, prio_comm=info["prio_greatest"], **ckw))
+        torch.cuda.synchronize()
+    finally:
+        ra.ra_set_trace(None, 0)
+    assert res["plan"] == plan
+    h = buf.cpu().numpy().view(np.uint64)
+    n = int(h[0])
+    assert 0 < n <= cap
+    rec = h[1:1 + 4 * n].reshape(n, 4)
+    kid = (rec[:, 0] >> np.uint64(32)).astype(np.int64)
+    sm = (rec[:, 0] & np.uint64(0xFFFFFFFF)).astype(np.int64)
+    gsel = kid == 1
+    assert gsel.sum() == 3 * plan["grid"] and (~gsel).any()
+    seen = _resident_max(sm[gsel], rec[gsel, 2], rec[gsel, 3])
+    assert 1 <= seen <= plan["ctas_per_sm"], f"{seen} GEMM CTAs shared an SM, the plan accounts for {plan['ctas_per_sm']}"
+    assert ra.ra_gemm_residency() == seen                                # the kernel's own per-SM counter agrees
+
+
+def test_bounded_work_mode_keeps_single_residency(ra):
+    """grid > #SMs: a second GEMM CTA would be placed wherever it fits, so the footprint must exclude it."""
+    import torch
+    M, N, K = 4096, 4096, 1024
+    occ = dict(tiles_per_cta=1)
+    A, B, g, dC = _gemm_side(ra, M, N, K, 22, occ=occ)
+    plan = ra.ra_gemm_plan_query(0, 1, M, N, K, occ)
+    assert plan["grid"] > ra.ra_device_info()["sm_count"] and plan["hw_ctas_per_sm"] == 1, plan
+    ra.ra_gemm_residency(reset=True)
+    w, keep = ra.make_workload(gemm=g, n_iters=2)
+    ra.ra_overlap_run(w, ra.make_cfg(mode=0, occ=occ))
+    assert ra.ra_gemm_residency() == 1
+
+
+def test_pristine_refill_keeps_allreduce_inputs_fixed(ra):
+    """ar_pristine: every run (and every run of a sweep) reduces the same data, so results neither saturate nor drift."""
+    import torch
+    cfg0 = ra_inputs.CONFIGS[0]
+    bufs = ra_inputs.allreduce_buffers(cfg0)
+    ref_bufs = [b.copy() for b in bufs]
+    oracle.overlap_replay(cfg0.n_iters, ar_bufs=ref_bufs)
+    pristine = [to_dev(b) for b in bufs]
+    dev = [torch.zeros_like(p) for p in pristine]                      # start from garbage (zeros): the refill supplies the data
+    A, B, g, dC = _gemm_side(ra, cfg0.M, cfg0.N, cfg0.K, cfg0.seed)
+    w, keep = ra.make_workload(gemm=g, allreduce=dev, n_iters=cfg0.n_iters, ar_pristine=pristine)
+    for kw in (dict(mode=0), dict(mode=1), dict(mode=1, use_graph=1), dict(mode=1, use_graph=1)):
+        for _ in range(3):                                             # 3 x 4 iterations of x4 growth would be 2^24 without refill
+            ra.ra_overlap_run(w, ra.make_cfg(**kw))
+        torch.cuda.synchronize()
+        for dd, rr in zip(dev, ref_bufs):
+            assert to_host(dd, np.float32).tobytes() == rr.tobytes(), kw
+    results, best = ra.ra_overlap_sweep(w, [ra.make_cfg(mode=0), ra.make_cfg(mode=1)], runs=40)   # 320 iterations in all
+    torch.cuda.synchronize()
+    for dd, rr, pp, b0 in zip(dev, ref_bufs, pristine, bufs):
+        assert to_host(dd, np.float32).tobytes() == rr.tobytes()
+        assert to_host(pp, np.float32).tobytes() == b0.tobytes()       # the pristine copies are never written
+
+
+def test_launch_cache_is_keyed_by_everything_that_matters(ra):
+    """The cached plan / tensor maps must never leak between calls that differ in pointers, shape, ld or knobs."""
+    import torch
+    M, N, K = 384, 320, 256
+    rng_seed = 31
+    A = ra_inputs.normal_bf16((M, K), rng_seed, ra_inputs.STREAM_A)
+    B = ra_inputs.normal_bf16((N, K), rng_seed, ra_inputs.STREAM_B)
+    A2 = ra_inputs.normal_bf16((M, K), rng_seed + 1, ra_inputs.STREAM_A)
+    refs = {}
+    for name, a in (("A", A), ("A2", A2)):
+        refs[name] = (oracle.gemm(0, 1, M, N, K, 1.0, a, B)[0], *oracle.gemm_norms(0, 1, M, N, K, a, B))
+    dA, dA2, dB = to_dev(A), to_dev(A2), to_dev(B)
+    dC1 = torch.full((M, N), 0x7FC0, dtype=torch.int16, device="cuda")
+    dC2 = torch.full((M, N), 0x7FC0, dtype=torch.int16, device="cuda")
+    ws = torch.empty(1 << 22, dtype=torch.uint8, device="cuda")
+    seq = [(dA, dC1, "A", None), (dA2, dC1, "A2", None), (dA, dC2, "A", None), (dA2, dC2, "A2", dict(sm_budget=3)),
+           (dA, dC1, "A", dict(cta_group=1)), (dA, dC1, "A", None), (dA2, dC1, "A2", dict(smem_reserve_bytes=100 * 1024))]
+    for rep in range(2):                                               # second pass: every entry is a cache hit
+        for a, c, name, occ in seq:
+            c.fill_(0x7FC0)
+            ra.ra_gemm(0, 1, M, N, K, 1.0, a, K, dB, K, 0.0, c, N, occ=occ, workspace=ws)
+            torch.cuda.synchronize()
+            ref, rowA, colB = refs[name]
+            assert gemm_norm_err(to_host(c, np.uint16).reshape(M, N), ref, rowA, colB) <= GEMM_TOL, (rep, name, occ)
+    # a sub-matrix view of the same buffers (different ld / shape, same base pointers) is a different key
+    ref, rowA, colB = (oracle.gemm(0, 1, 128, 64, 128, 1.0, A, B, lda=K, ldb=K)[0], *oracle.gemm_norms(0, 1, 128, 64, 128, A, B, lda=K, ldb=K))
+    dC1.fill_(0x7FC0)
+    ra.ra_gemm(0, 1, 128, 64, 128, 1.0, dA, K, dB, K, 0.0, dC1, N, workspace=ws)
+    torch.cuda.synchronize()
+    got = to_host(dC1, np.uint16).reshape(M, N)[:128, :64]
+    assert gemm_norm_err(np.ascontiguousarray(got), ref, rowA, colB) <= GEMM_TOL
+    ra.ra_shutdown()                                                   # drops the cache; the next call rebuilds it
+    ra.ra_gemm(0, 1, M, N, K, 1.0, dA, K, dB, K, 0.0, dC2, N, workspace=ws)
+    torch.cuda.synchronize()
+    ref, rowA, colB = refs["A"]
+    assert gemm_norm_err(to_host(dC2, np.uint16).reshape(M, N), ref, rowA, colB) <= GEMM_TOL

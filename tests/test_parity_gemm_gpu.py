@@ -141,7 +141,7 @@ def test_integer_exact(ra, M, N, K):
 
 @pytest.mark.parametrize("M,N,K", [(256, 256, 64), (512, 512, 256), (1000, 520, 200), (384, 768, 4096), (2048, 2048, 512),
                                    (257, 264, 72), (4096, 1024, 1024)])
-@pytest.mark.parametrize("occ", [dict(cta_group=2, m_blocks=1), dict(cta_group=2, m_blocks=1, sm_budget=9, smem_reserve_bytes=128 * 1024),
+@pytest.mark.parametrize("occ", [dict(cta_group=2, m_blocks=1), dict(cta_group=2, m_blocks=1, sm_budget=9, smem_reserve_bytes=96 * 1024),
                                  dict(cta_group=2, tiles_per_cta=1)])
 def test_cta_pairs(ra, M, N, K, occ):
     """tcgen05 cta_group::2 path (2-CTA clusters, 256 x 256 tiles), forced on shapes the planner would not pick it for."""
