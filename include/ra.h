@@ -86,6 +86,20 @@ typedef struct {
                                  2 parts only) and reduced through distributed shared memory in ascending-k order;
                                  needs parts * tiles <= #SMs (pairs: 4 * tiles) and room for the parts' accumulators
                                  in part 0's stage ring */
+    int32_t l2_persist_bytes; /* 0 = off (default).  > 0: the GEMM claims this much of L2 as a persisting carve-out
+                                 (cudaLimitPersistingL2CacheSize, clamped to the device maximum: 79 MiB on B200) and keeps
+                                 the X-operand panel of one raster group resident in it (TMA loads with the evict_last
+                                 policy, the group widened to what the carve-out holds), so X is read from DRAM once
+                                 and Y once per group instead of both once per wave: 8192^3 moves 635 MB instead of 957 MB
+                                 (profiles/r02_l2_persist.md).  The carve-out is DEVICE-WIDE and is taken from every
+                                 other kernel's L2 -- the streaming collectives slow down next to it (measured: -10 % at
+                                 24 MiB, 2.3x at 64 MiB and above) -- which makes it a resource traded between K_g and K_c
+                                 like the shared-memory reserve.  ra_gemm sets the carve-out when it
+                                 differs from what the library last set (one driver call, not inside a stream capture)
+                                 and leaves it set; ra_overlap_run / _sweep / _autotune / _run_host set it for the run and
+                                 take it back before returning; ra_l2_persist(0) and ra_shutdown take it back too.
+                                 Ignored (reported as 0 in the plan) by swapped, stream-K, cluster split-K and
+                                 single-wave plans.  Does not change results (same per-element k order). */
 } ra_occupancy;
 
 /* What S3 decided -- for tests, logs and the sweep tables. */
@@ -119,9 +133,12 @@ typedef struct {
                                  Bounded-work plans (tiles_per_cta > 0) always pad (clamping the reserve if they must).  A
                                  reserve so large that not even two minimal CTAs fit under it (~> 176 KiB) is clamped:
                                  clamped = 1 and smem_left_per_sm reports what two resident CTAs really leave. */
+    int32_t group_x;          /* rasterisation: tile rows (of tile_m, or tile_n when swap_ab) per raster group; inside a
+                                 group tiles are numbered row-fastest */
+    int32_t l2_persist_bytes; /* the occupancy knob if this plan uses it, else 0 */
 } ra_gemm_plan;
 
-/* Host-only: computes the plan ra_gemm would use.  `occ` NULL = defaults {0,0,0,1,0,0,0}. */
+/* Host-only: computes the plan ra_gemm would use.  `occ` NULL = defaults {0,0,0,1,0,0,0,0}. */
 ra_status ra_gemm_plan_query(int transA, int transB, int M, int N, int K, const ra_occupancy* occ, ra_gemm_plan* out);
 
 /* S3 by measurement: every GEMM CTA counts itself in and out on its SM (%smid).  *max_ctas_on_one_sm receives the largest
@@ -340,6 +357,13 @@ ra_status ra_overlap_autotune(const ra_workload* w, const ra_peaks* peaks, int r
  * settings with mode == RA_MODE_OVERLAP (or over all if none).  Host pointers all. */
 ra_status ra_overlap_sweep(const ra_workload* w, const ra_overlap_cfg* cfgs, int n, int runs,
                            ra_overlap_result* results, int* best);
+
+/* Sets the current device's persisting-L2 carve-out to min(bytes, device maximum) and reports what was granted (host
+ * out-pointer, may be NULL; the driver rounds up to eighths of the L2, 15.8 MiB steps on B200); bytes = 0 takes it back and turns the lines it held into normal ones.  This is the state
+ * ra_occupancy.l2_persist_bytes manages for the GEMM (see there); the call exists so that a caller who ran ra_gemm with
+ * the knob can give the L2 back before launching something else.  One driver call when the value changes, none
+ * otherwise; not to be called while a stream of the device is being captured.  RA_ERR_INVALID_ARG for bytes < 0. */
+ra_status ra_l2_persist(int64_t bytes, int64_t* granted);
 
 /* ---------------------------------------------------------------------------------------------
  * Residency trace (evidence for "per-SM residency during overlap").  When a trace buffer is set,

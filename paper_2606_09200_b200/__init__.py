@@ -30,6 +30,7 @@ EXPORTS = (
     "ra_gemm_workspace_bytes", "ra_gemm", "ra_gemm_ex", "ra_allreduce_emul", "ra_allreduce_emul_ex", "ra_alltoall_emul",
     "ra_alltoall_emul_ex",
     "ra_overlap_run", "ra_overlap_run_host", "ra_overlap_suggest", "ra_overlap_autotune", "ra_overlap_sweep", "ra_set_trace",
+    "ra_l2_persist",
 )
 
 
@@ -41,13 +42,14 @@ class RaError(RuntimeError):
 
 class Occupancy(Structure):
     _fields_ = [("smem_reserve_bytes", c_int32), ("sm_budget", c_int32), ("tiles_per_cta", c_int32),
-                ("allow_clamp", c_int32), ("cta_group", c_int32), ("m_blocks", c_int32), ("cluster_k", c_int32)]
+                ("allow_clamp", c_int32), ("cta_group", c_int32), ("m_blocks", c_int32), ("cluster_k", c_int32),
+                ("l2_persist_bytes", c_int32)]
 
 
 class GemmPlan(Structure):
     _fields_ = [(n, c_int32) for n in ("ctas_per_sm", "grid", "stages", "tile_m", "tile_n", "tile_k", "split_k",
                                        "swap_ab", "dyn_smem_bytes", "smem_left_per_sm", "n_tiles", "clamped", "cta_group",
-                                       "m_blocks", "cluster_k", "hw_ctas_per_sm")]
+                                       "m_blocks", "cluster_k", "hw_ctas_per_sm", "group_x", "l2_persist_bytes")]
 
     def as_dict(self):
         return {n: getattr(self, n) for n, _ in self._fields_}
@@ -178,7 +180,7 @@ def _occ(occ) -> Occupancy | None:
         return occ
     return Occupancy(int(occ.get("smem_reserve_bytes", 0)), int(occ.get("sm_budget", 0)),
                      int(occ.get("tiles_per_cta", 0)), int(occ.get("allow_clamp", 1)), int(occ.get("cta_group", 0)),
-                     int(occ.get("m_blocks", 0)), int(occ.get("cluster_k", 0)))
+                     int(occ.get("m_blocks", 0)), int(occ.get("cluster_k", 0)), int(occ.get("l2_persist_bytes", 0)))
 
 
 def _occ_ref(occ):
@@ -352,6 +354,14 @@ def make_host_io(*, A=None, B=None, C=None, ar_in=None, ar_out=None, a2a_in=None
     return io, keep
 
 
+def ra_l2_persist(nbytes: int) -> int:
+    """Sets the device's persisting-L2 carve-out (0 = give it back); returns the bytes granted."""
+    from ctypes import c_int64
+    g = c_int64(0)
+    _check(_L().ra_l2_persist(c_int64(int(nbytes)), byref(g)), "ra_l2_persist")
+    return int(g.value)
+
+
 def ra_overlap_run_host(dev0: Workload, dev1, io: HostIO, cfg: OverlapCfg, n_steps: int = 1) -> dict:
     """n_steps steps from host buffers, copies pipelined against compute over the device sets dev0 / dev1 (or None)."""
     res = OverlapResult()
@@ -364,7 +374,7 @@ def cfg_to_kw(c: OverlapCfg) -> dict:
     """OverlapCfg -> the keyword form make_cfg takes (for logging / re-creating a setting)."""
     return dict(mode=c.mode, occ=dict(smem_reserve_bytes=c.occ.smem_reserve_bytes, sm_budget=c.occ.sm_budget,
                                       tiles_per_cta=c.occ.tiles_per_cta, cta_group=c.occ.cta_group, m_blocks=c.occ.m_blocks,
-                                      cluster_k=c.occ.cluster_k),
+                                      cluster_k=c.occ.cluster_k, l2_persist_bytes=c.occ.l2_persist_bytes),
                 coll_sm_budget=c.coll_sm_budget, coll_smem_bytes=c.coll_smem_bytes, coll_ctas_per_sm=c.coll_ctas_per_sm,
                 coll_variant=c.coll_variant, prio_compute=c.prio_compute, prio_comm=c.prio_comm, dependent=c.dependent,
                 use_graph=c.use_graph)

@@ -39,6 +39,45 @@ ra_status device_info(DeviceInfo* out) {
 
 ra_status require_sm100(const DeviceInfo& di) { return di.cc_major == 10 ? RA_OK : RA_ERR_ARCH; }
 
+// ---- persisting-L2 carve-out (cudaLimitPersistingL2CacheSize) -------------------------------------------------------
+// evict_last TMA loads only stick when the device has a persisting carve-out (measured: without it the policy changes
+// nothing), and the carve-out is taken away from every other kernel's L2 (measured: the streaming collectives lose
+// 10 % at 24 MiB, 35 % at 32-56 MiB, 2.3x at 64+ MiB).  It is therefore a per-setting resource like the shared-memory
+// reserve: the library tracks what it last set per device and only calls the driver on a change.
+static std::mutex g_l2_mutex;
+static long long g_l2_state[64];     // what was asked for (after clamping to the device maximum)
+static long long g_l2_granted[64];   // what the driver made of it (it rounds up to eighths of the L2: 15.8 MiB steps on B200)
+static bool g_l2_known[64] = {};
+
+ra_status l2_persist_ensure(long long bytes, long long* granted) {
+    if (bytes < 0) return RA_ERR_INVALID_ARG;
+    int dev = -1;
+    RA_CUDA(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= 64) return RA_ERR_UNSUPPORTED;
+    std::lock_guard<std::mutex> lk(g_l2_mutex);
+    if (!g_l2_known[dev]) {
+        if (bytes == 0) {                       // never touched and nothing wanted: leave the device alone
+            if (granted) *granted = 0;
+            return RA_OK;
+        }
+        g_l2_state[dev] = g_l2_granted[dev] = 0;
+        g_l2_known[dev] = true;
+    }
+    int max_bytes = 0;
+    RA_CUDA(cudaDeviceGetAttribute(&max_bytes, cudaDevAttrMaxPersistingL2CacheSize, dev));
+    const long long want = bytes < (long long)max_bytes ? bytes : (long long)max_bytes;
+    if (want != g_l2_state[dev]) {
+        RA_CUDA(cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, (size_t)want));
+        if (want == 0) RA_CUDA(cudaCtxResetPersistingL2Cache());   // lines left in the carve-out become normal lines again
+        size_t got = 0;
+        RA_CUDA(cudaDeviceGetLimit(&got, cudaLimitPersistingL2CacheSize));
+        g_l2_state[dev] = want;
+        g_l2_granted[dev] = (long long)got;
+    }
+    if (granted) *granted = g_l2_granted[dev];
+    return RA_OK;
+}
+
 }  // namespace ra
 
 extern "C" {
@@ -67,6 +106,13 @@ ra_status ra_device_info(int* sm_count, int* smem_per_sm, int* smem_per_block_op
     if (smem_reserved_per_block) *smem_reserved_per_block = di.smem_reserved_per_block;
     if (prio_least) *prio_least = di.prio_least;
     if (prio_greatest) *prio_greatest = di.prio_greatest;
+    return RA_OK;
+}
+
+ra_status ra_l2_persist(int64_t bytes, int64_t* granted) {
+    long long g = 0;
+    RA_TRY(ra::l2_persist_ensure((long long)bytes, &g));
+    if (granted) *granted = (int64_t)g;
     return RA_OK;
 }
 

@@ -38,6 +38,10 @@ struct DeviceInfo {
 ra_status device_info(DeviceInfo* out);
 // RA_ERR_ARCH unless the current device is sm_100-family.
 ra_status require_sm100(const DeviceInfo& di);
+// Sets the current device's persisting-L2 carve-out to min(bytes, device maximum) unless that is what this library
+// last set (then no driver call is made); bytes = 0 also resets the persisting lines.  Must not be called while a
+// stream of the device is being captured unless it is a no-op.
+ra_status l2_persist_ensure(long long bytes, long long* granted = nullptr);
 
 // Planner constants used when no device is present (plan queries on a CPU-only box): B200 values.
 constexpr int kDefaultSmCount = 148;

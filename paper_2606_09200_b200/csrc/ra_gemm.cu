@@ -1059,6 +1059,7 @@ struct Plan {
     ra_gemm_plan pub;
     int bn;
     int epi_tma;       // whole tiles leave through the shared-memory staging area + TMA stores
+    int hint_x;        // L2 policy of the X loads when an X panel is kept resident (2 = evict_last), else 0
     size_t counters_bytes, ws_bytes;
 };
 
@@ -1070,7 +1071,7 @@ static ra_status validate_shape(int transA, int transB, int M, int N, int K) {
 
 static ra_status make_plan(int transA, int transB, int M, int N, int K, const ra_occupancy* occ_in, Plan* out) {
     RA_TRY(validate_shape(transA, transB, M, N, K));
-    ra_occupancy occ = {0, 0, 0, 1, 0, 0, 0};
+    ra_occupancy occ = {0, 0, 0, 1, 0, 0, 0, 0};
     if (occ_in) occ = *occ_in;
     if (occ.smem_reserve_bytes < 0 || occ.sm_budget < 0 || occ.tiles_per_cta < 0) return RA_ERR_INVALID_ARG;
 
@@ -1138,6 +1139,7 @@ static ra_status make_plan(int transA, int transB, int M, int N, int K, const ra
     if (occ.cta_group < 0 || occ.cta_group > 2) return RA_ERR_INVALID_ARG;
     if (occ.m_blocks < 0 || occ.m_blocks > 2) return RA_ERR_INVALID_ARG;
     if (occ.cluster_k < 0 || occ.cluster_k > 4 || occ.cluster_k == 3) return RA_ERR_INVALID_ARG;
+    if (occ.l2_persist_bytes < 0) return RA_ERR_INVALID_ARG;
 
     // n_acc = GEMM CTAs per SM the shared-memory accounting assumes.  Pass 1 sizes the plan for ONE CTA per SM and makes
     // that a fact where it can (padding, below).  Where it cannot -- a reserve above ~half an SM leaves no room for the
@@ -1316,6 +1318,35 @@ static ra_status make_plan(int transA, int transB, int M, int N, int K, const ra
     g.cluster_k = ks;
     pl.bn = bn;
     pl.epi_tma = epi_bytes > 0;
+    {
+        // Rasterisation.  The W workers of one wave cover a gx x gy block of tiles and march through K together, so
+        // the wave reads (gx*tile_x + gy*BN) rows of K from DRAM once and shares them through L2 in time.  Nothing
+        // survives from one wave to the next under the default L2 policy once a wave's footprint passes ~50 MB
+        // (measured, profiles/r02_l2_persist.md: 8192^3 reads waves x footprint), so DRAM traffic ~ waves *
+        // (gx*tile_x + gy*BN) rows, minimised subject to gx*gy = W at gx = sqrt(W*BN/tile_x): 6 for 74 pairs of 512 x 256.
+        const int workers = grid / (cg * ks);
+        int gx = 1;
+        while ((long long)(gx + 1) * (gx + 1) * tile_x <= (long long)workers * bn) ++gx;
+        pl.hint_x = 0;
+        g.l2_persist_bytes = 0;
+        // l2_persist_bytes: the X panel of a group (gx*tile_x rows x K) is loaded with the evict_last policy and stays in
+        // the persisting carve-out of L2 while the group's Y tiles stream past it, so X is read from DRAM once and Y once
+        // per group.  The group is widened to what the carve-out holds; a carve-out smaller than the default group's
+        // panel still keeps part of it.
+        const long long xtile_bytes = (long long)tile_x * K * 2;
+        if (occ.l2_persist_bytes > 0 && !swap && !stream_k && ks == 1 && tiles_x * tiles_y > workers && xtile_bytes > 0) {
+            const int fit = (int)(occ.l2_persist_bytes / xtile_bytes);
+            if (fit > gx) {
+                gx = fit < tiles_x ? fit : tiles_x;
+                const int groups = (tiles_x + gx - 1) / gx;
+                gx = (tiles_x + groups - 1) / groups;         // equal groups: 16 tile rows at 9 that fit -> 8 + 8, not 9 + 7
+            }
+            pl.hint_x = 2;
+            g.l2_persist_bytes = occ.l2_persist_bytes;
+        }
+        if (gx > tiles_x) gx = (int)tiles_x;
+        g.group_x = gx < 1 ? 1 : gx;
+    }
     if (stream_k) {
         const long long U = n_tiles * kb;
         // max number of CTA ranges one tile can span
@@ -1408,18 +1439,8 @@ static ra_status build_entry(const LaunchKey& k, const DeviceInfo& di, LaunchEnt
     // not displace anything; the small operand every CTA re-reads should stay.
     p.hintX = (p.tiles_y == 1 && p.tiles_x > 1) ? 1 : 0;
     p.hintY = (p.tiles_y == 1 && p.tiles_x > 1) ? 2 : 0;
-    {
-        // Rasterisation.  The W workers of one wave cover a gx x gy block of tiles and march through K together, so
-        // the wave reads (gx*tile_x + gy*BN) rows of K from DRAM once and shares them through L2; with 16 KiB rows
-        // (K = 8192) a wave's footprint (~69 MB) already exceeds what L2 keeps across waves (measured: no cross-wave
-        // reuse), so DRAM traffic ~ waves * (gx*tile_x + gy*BN) rows.  Minimised, subject to gx*gy = W, at
-        // gx = sqrt(W*BN/tile_x): 8 for 74 pairs of 256x256, 16-17 for 148 CTAs of 128x256.
-        const int workers = pl.pub.grid / cg;
-        int gx = 1;
-        while ((long long)(gx + 1) * (gx + 1) * tile_x <= (long long)workers * pl.bn) ++gx;
-        if (gx > p.tiles_x) gx = p.tiles_x;
-        p.group_x = gx < 1 ? 1 : gx;
-    }
+    p.group_x = pl.pub.group_x;
+    if (pl.hint_x) p.hintX = pl.hint_x;
     const void* X = swap ? k.B : k.A;
     const void* Y = swap ? k.A : k.B;
     const int ldx = swap ? k.ldb : k.lda, ldy = swap ? k.lda : k.ldb;
@@ -1465,7 +1486,7 @@ ra_status gemm_launch(int transA, int transB, int M, int N, int K, float alpha, 
         const uintptr_t b0 = reinterpret_cast<uintptr_t>(B), b1 = b0 + b_elems * 2;
         if (K > 0 && ((c0 < a1 && a0 < c1) || (c0 < b1 && b0 < c1))) return RA_ERR_INVALID_ARG;
     }
-    ra_occupancy occ_v = {0, 0, 0, 1, 0, 0, 0};
+    ra_occupancy occ_v = {0, 0, 0, 1, 0, 0, 0, 0};
     if (occ) occ_v = *occ;
 
     if (K == 0 || alpha == 0.f) {
@@ -1481,6 +1502,8 @@ ra_status gemm_launch(int transA, int transB, int M, int N, int K, float alpha, 
         RA_CUDA(cudaGetLastError());
         return RA_OK;
     }
+
+    RA_TRY(l2_persist_ensure(occ_v.l2_persist_bytes));   // no driver call unless the carve-out has to change
 
     LaunchKey key;
     memset(&key, 0, sizeof(key));                  // padding bytes too: keys are compared with memcmp

@@ -146,8 +146,7 @@ static ra_status check_priorities(const ra_overlap_cfg* cfg) {
     return RA_OK;
 }
 
-static ra_status run_once(const ra_workload* w, const ra_overlap_cfg* cfg, ra_overlap_result* res) {
-    std::lock_guard<std::mutex> lk(g_cache.mu);
+static ra_status run_once_locked(const ra_workload* w, const ra_overlap_cfg* cfg, ra_overlap_result* res) {
     const int n = w->n_iters;
     const bool has_gemm = w->M > 0 && w->N > 0;
     const bool has_coll = w->kind != RA_COLL_NONE;
@@ -282,6 +281,21 @@ static ra_status run_once(const ra_workload* w, const ra_overlap_cfg* cfg, ra_ov
     return RA_OK;
 }
 
+// The GEMM's L2 carve-out (occ.l2_persist_bytes) is set for the duration of one run and taken back afterwards: it is
+// device-wide, and a collective launched later on its own must not inherit it.
+static ra_status run_once(const ra_workload* w, const ra_overlap_cfg* cfg, ra_overlap_result* res) {
+    std::lock_guard<std::mutex> lk(g_cache.mu);
+    const long long want = (w->M > 0 && w->N > 0) ? cfg->occ.l2_persist_bytes : 0;
+    if (want < 0) return RA_ERR_INVALID_ARG;
+    if (want > 0) RA_TRY(l2_persist_ensure(want));
+    ra_status st = run_once_locked(w, cfg, res);
+    if (want > 0) {
+        const ra_status r = l2_persist_ensure(0);
+        if (st == RA_OK) st = r;
+    }
+    return st;
+}
+
 // ---- host-buffer pipeline: H2D(step s+1)  ||  compute(step s)  ||  D2H(step s-1) ---------------------------
 static size_t a_bytes(const ra_workload* w) { return (size_t)(w->transA ? w->K : w->M) * (size_t)w->lda * 2; }
 static size_t b_bytes(const ra_workload* w) { return (size_t)(w->transB ? w->N : w->K) * (size_t)w->ldb * 2; }
@@ -392,7 +406,14 @@ ra_status ra_overlap_run_host(const ra_workload* dev0, const ra_workload* dev1, 
     }
     if (dev0->kind == RA_COLL_ALLTOALL && io->a2a_in == nullptr) return RA_ERR_INVALID_ARG;
     const ra_workload* sets[2] = {dev0, dev1};
-    return ra::run_host(sets, dev1 ? 2 : 1, io, cfg, n_steps, res);
+    const long long want = has_gemm ? cfg->occ.l2_persist_bytes : 0;
+    if (want > 0) RA_TRY(ra::l2_persist_ensure(want));
+    ra_status st = ra::run_host(sets, dev1 ? 2 : 1, io, cfg, n_steps, res);
+    if (want > 0) {
+        const ra_status r = ra::l2_persist_ensure(0);
+        if (st == RA_OK) st = r;
+    }
+    return st;
 }
 
 ra_status ra_overlap_run(const ra_workload* w, const ra_overlap_cfg* cfg, ra_overlap_result* res) {
@@ -441,6 +462,7 @@ ra_status ra_overlap_sweep(const ra_workload* w, const ra_overlap_cfg* cfgs, int
 
 void ra_shutdown(void) {
     ra::gemm_cache_clear();
+    (void)ra::l2_persist_ensure(0);
     std::lock_guard<std::mutex> lk(ra::g_cache.mu);
     for (auto& kv : ra::g_cache.streams) cudaStreamDestroy(kv.second);
     ra::g_cache.streams.clear();

@@ -38,11 +38,11 @@ def test_status_strings(ra):
 
 def test_struct_layouts_match_header(ra):
     # sizes computed by hand from include/ra.h (LP64)
-    assert ctypes.sizeof(ra.Occupancy) == 28
-    assert ctypes.sizeof(ra.GemmPlan) == 64
+    assert ctypes.sizeof(ra.Occupancy) == 32
+    assert ctypes.sizeof(ra.GemmPlan) == 72
     assert ctypes.sizeof(ra.Workload) == 160
-    assert ctypes.sizeof(ra.OverlapCfg) == 4 + 28 + 9 * 4
-    assert ctypes.sizeof(ra.OverlapResult) == 24 + 64 + 8
+    assert ctypes.sizeof(ra.OverlapCfg) == 4 + 32 + 9 * 4
+    assert ctypes.sizeof(ra.OverlapResult) == 24 + 72 + 8
     assert ctypes.sizeof(ra.HostIO) == 7 * 8
 
 
@@ -325,7 +325,7 @@ def test_header_is_plain_c_and_links_from_c(ra, tmp_path):
     src.write_text(
         '#include "ra.h"\n#include <stdio.h>\n'
         "int main(void) {\n"
-        "  ra_gemm_plan p; ra_occupancy o = {0, 0, 0, 1, 0, 0, 0};\n"
+        "  ra_gemm_plan p; ra_occupancy o = {0, 0, 0, 1, 0, 0, 0, 0};\n"
         "  if (ra_gemm_plan_query(0, 1, 8192, 8192, 8192, &o, &p) != RA_OK) return 1;\n"
         '  printf("%d %d %d %s\\n", p.tile_m, p.tile_n, p.grid, ra_status_str(RA_ERR_ARCH));\n'
         "  return ra_gemm_plan_query(0, 1, 8, 8, 8, &o, (ra_gemm_plan*)0) == RA_ERR_INVALID_ARG ? 0 : 2;\n"
@@ -375,3 +375,22 @@ def test_planner_invariants_random(ra):
             assert p["cluster_k"] == 1
 
     prop()
+
+
+def test_l2_persist_plan(ra):
+    """occ.l2_persist_bytes: the raster group is widened to the X panel the carve-out holds (equal groups), the plan
+    reports the knob only where it is used, and everything else about the plan is unchanged (a
+    resource knob, not a different algorithm)."""
+    base = ra.ra_gemm_plan_query(0, 1, 8192, 8192, 8192)
+    assert base["group_x"] == 6 and base["l2_persist_bytes"] == 0
+    p = ra.ra_gemm_plan_query(0, 1, 8192, 8192, 8192, dict(l2_persist_bytes=79 << 20))
+    assert p["group_x"] == 8 and p["l2_persist_bytes"] == 79 << 20            # 9 panels of 8 MiB fit: 16 rows -> 8 + 8
+    assert {k: v for k, v in p.items() if k not in ("group_x", "l2_persist_bytes")} == \
+           {k: v for k, v in base.items() if k not in ("group_x", "l2_persist_bytes")}
+    q = ra.ra_gemm_plan_query(0, 1, 8192, 8192, 8192, dict(l2_persist_bytes=32 << 20))
+    assert q["group_x"] == 6 and q["l2_persist_bytes"] == 32 << 20            # smaller than the default group: keeps part of it
+    # swapped (skinny), single-wave and stream-K plans ignore the knob
+    assert ra.ra_gemm_plan_query(0, 1, 64, 16384, 16384, dict(l2_persist_bytes=79 << 20))["l2_persist_bytes"] == 0
+    assert ra.ra_gemm_plan_query(0, 1, 2048, 2048, 2048, dict(l2_persist_bytes=79 << 20))["l2_persist_bytes"] == 0
+    with pytest.raises(ra.RaError):
+        ra.ra_gemm_plan_query(0, 1, 8192, 8192, 8192, dict(l2_persist_bytes=-1))

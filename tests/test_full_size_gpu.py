@@ -96,6 +96,9 @@ def test_full_size_integer_exact(ra, index):
     if full:
         settings.append(dict(mode=1, occ=dict(sm_budget=128, smem_reserve_bytes=64 * 1024), coll_sm_budget=20))
         settings.append(dict(mode=0, occ=dict(tiles_per_cta=1)))          # bounded-work grid (CTAs retire per tile)
+        settings.append(dict(mode=1, prio_comm=hi, occ=dict(l2_persist_bytes=79 << 20)))   # X panel resident in L2, groups of 8
+    else:
+        settings.append(dict(mode=1, occ=dict(l2_persist_bytes=64 << 20)))
     for kw in settings:
         dC = torch.full((M, N), 0x7FC0, dtype=torch.int16, device="cuda")
         occ = kw.get("occ")

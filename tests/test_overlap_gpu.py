@@ -489,3 +489,31 @@ def test_launch_cache_is_keyed_by_everything_that_matters(ra):
     torch.cuda.synchronize()
     ref, rowA, colB = refs["A"]
     assert gemm_norm_err(to_host(dC2, np.uint16).reshape(M, N), ref, rowA, colB) <= GEMM_TOL
+
+
+@pytest.mark.parametrize("use_graph", [0, 1])
+def test_l2_persist_is_set_for_the_run_and_taken_back(ra, use_graph):
+    """occ.l2_persist_bytes inside the overlap driver (ra.h): the carve-out is device-wide, so ra_overlap_run sets it for
+    the run and gives it back -- a collective launched afterwards must not inherit it.  Results: the allreduce equals the
+    oracle's replay bit for bit, C equals the knob-free run bit for bit ("without modifying kernel logic")."""
+    import torch
+    cudart = pytest.importorskip("cuda.bindings.runtime")
+    M, N, K = 4096, 4096, 2048
+    A, B, g, dC = _gemm_side(ra, M, N, K, 9)
+    host = [ra_inputs.uniform_f32(1 << 18, 9, ra_inputs.STREAM_AR + r) for r in range(4)]
+    outs = []
+    for occ in (None, dict(l2_persist_bytes=24 << 20)):
+        bufs = [to_dev(h) for h in host]
+        dC.fill_(0x7FC0)
+        w, keep = ra.make_workload(gemm=g, allreduce=bufs, n_iters=3)
+        res = ra.ra_overlap_run(w, ra.make_cfg(mode=1, occ=occ, use_graph=use_graph))
+        torch.cuda.synchronize()
+        err, lim = cudart.cudaDeviceGetLimit(cudart.cudaLimit.cudaLimitPersistingL2CacheSize)
+        assert int(err) == 0 and int(lim) == 0, (err, lim)
+        assert res["plan"]["l2_persist_bytes"] == (occ or {}).get("l2_persist_bytes", 0)
+        ref = [h.copy() for h in host]
+        oracle.overlap_replay(3, ar_bufs=ref)
+        for dd, rr in zip(bufs, ref):
+            assert to_host(dd, np.float32).tobytes() == rr.tobytes()
+        outs.append(to_host(dC, np.uint16).copy())
+    assert np.array_equal(outs[0], outs[1])

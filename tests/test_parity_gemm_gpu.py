@@ -439,3 +439,42 @@ def test_cluster_split_k_four_parts(ra, M, N, K):
     assert np.array_equal(got, ref16)                          # integer inputs: exact whatever the association
     again, _ = run_gemm(ra, M, N, K, A, B, occ=occ, ldc=(N + 7) // 8 * 8)
     assert np.array_equal(got, again)
+
+
+def _persisting_l2_limit():
+    """The device's current cudaLimitPersistingL2CacheSize, read through cuda-python (independent of the library)."""
+    cudart = pytest.importorskip("cuda.bindings.runtime")
+    err, val = cudart.cudaDeviceGetLimit(cudart.cudaLimit.cudaLimitPersistingL2CacheSize)
+    assert int(err) == 0, err
+    return int(val)
+
+
+def test_l2_persist_same_bits_and_state(ra):
+    """occ.l2_persist_bytes (ra.h): a resource knob -- raster group + evict_last loads -- that must not change one bit of
+    C (per-element k order is untouched), sets the device carve-out for ra_gemm and leaves it, and ra_l2_persist(0) /
+    ra_overlap_run take it back."""
+    M, N, K = 4096, 4096, 2048                      # 128 tiles of 512 x 256 over 74 CTA pairs: two waves, groups matter
+    A = ra_inputs.normal_bf16((M, K), 71, ra_inputs.STREAM_A)
+    B = ra_inputs.normal_bf16((N, K), 71, ra_inputs.STREAM_B)
+    base, _ = run_gemm(ra, M, N, K, A, B)
+    occ = dict(l2_persist_bytes=24 << 20)
+    plan = ra.ra_gemm_plan_query(0, 1, M, N, K, occ)
+    assert plan["l2_persist_bytes"] == 24 << 20 and plan["group_x"] == 8, plan     # 2 MiB per tile row: all 8 rows of X stay resident
+    got, _ = run_gemm(ra, M, N, K, A, B, occ=occ)
+    assert got.tobytes() == base.tobytes()
+    set_to = _persisting_l2_limit()                 # ra_gemm leaves the carve-out set (the next GEMM wants it too);
+    assert 24 << 20 <= set_to < 40 << 20            # the driver rounds up to eighths of the L2 (15.8 MiB on B200)
+    assert ra.ra_l2_persist(0) == 0
+    assert _persisting_l2_limit() == 0
+    # a knob-free GEMM after a persisting one takes the carve-out back by itself
+    run_gemm(ra, M, N, K, A, B, occ=occ)
+    assert _persisting_l2_limit() == set_to
+    again, _ = run_gemm(ra, M, N, K, A, B)
+    assert _persisting_l2_limit() == 0 and again.tobytes() == base.tobytes()
+    # more than the device has: clamped, reported
+    granted = ra.ra_l2_persist(1 << 40)
+    assert 0 < granted <= 126 << 20 and _persisting_l2_limit() == granted
+    assert ra.ra_l2_persist(0) == 0
+    ref, _ = oracle.gemm(0, 1, M, N, K, 1.0, A, B)
+    rowA, colB = oracle.gemm_norms(0, 1, M, N, K, A, B)
+    assert gemm_norm_err(got, ref, rowA, colB) <= GEMM_TOL
