@@ -358,6 +358,47 @@ ra_status ra_overlap_autotune(const ra_workload* w, const ra_peaks* peaks, int r
 ra_status ra_overlap_sweep(const ra_workload* w, const ra_overlap_cfg* cfgs, int n, int runs,
                            ra_overlap_result* results, int* best);
 
+/* ---------------------------------------------------------------------------------------------
+ * N4: the stand-ins as real exchanges over peer memory ("aggregated across all GPUs using allreduce ...
+ * alltoall to route tokens between devices"; 4 / 8 GPUs per node).  One process per GPU; every rank owns one
+ * buffer and reaches the others' through CUDA IPC mappings (NVLink / NVSwitch peer memory).  K2 and K3 are unchanged:
+ * they only ever take P device pointers.  No call here waits on another rank: the caller orders the ranks (a barrier of
+ * its process group before -- inputs ready -- and after -- every slice / chunk written).  Unmeasured on NVLink
+ * (one GPU at hand): exercised by P sequential ranks on one device and by two processes sharing one device through
+ * real IPC handles (tests/test_peer_gpu.py).
+ *
+ * ra_ipc_handle   what a rank publishes for one device pointer: the CUDA IPC handle of the allocation that holds it,
+ *                 the pointer's offset inside that allocation (so sub-allocated pointers, e.g. a caching allocator's,
+ *                 can be shared) and the bytes that follow it.  Plain bytes: ship it over any transport.
+ * ra_ipc_export   HOST out-pointer; dev_ptr a DEVICE pointer of this process (not itself an IPC mapping).
+ * ra_ipc_open     maps a peer's handle into this process (peer access is enabled lazily by the driver) and returns the
+ *                 DEVICE pointer that corresponds to the exported one.  Open each handle once per process.
+ * ra_ipc_close    unmaps a pointer ra_ipc_open returned (RA_ERR_INVALID_ARG for any other pointer).
+ * ra_peer_slice   host-only: the floats [begin, end) of a count-float buffer that rank `rank` of P reduces; the slices
+ *                 partition [0, count), boundaries are multiples of 4 floats (16-byte vectors).
+ * ra_allreduce_peer  bufs: HOST array of the P DEVICE pointers IN RANK ORDER (own buffer at index rank, the rest opened
+ *                 from the peers' handles), count floats each.  Launches K2 on this rank's slice: sum in the fixed order
+ *                 0..P-1, one RNE binary32 add per rank, written back to the slice of ALL P buffers.  After every rank
+ *                 has run, every buffer equals the oracle's allreduce bit for bit.  variant as ra_allreduce_emul_ex.
+ * ra_alltoall_peer   send: this rank's P chunks (DEVICE); recv: HOST array of the P ranks' receive buffers (DEVICE
+ *                 pointers in rank order, P chunks each).  Pushes chunk j into slot `rank` of recv[j]:
+ *                 recv_j[rank] = send_rank[j].  variant as ra_alltoall_emul_ex (2 = copy engines, peer-to-peer).
+ * Errors as the emulation calls; 1 <= P <= RA_MAX_RANKS, 0 <= rank < P.
+ * ------------------------------------------------------------------------------------------- */
+typedef struct {
+    uint8_t opaque[64];   /* cudaIpcMemHandle_t */
+    uint64_t offset;      /* of the exported pointer inside its allocation */
+    uint64_t bytes;       /* from the exported pointer to the end of its allocation */
+} ra_ipc_handle;
+
+ra_status ra_ipc_export(const void* dev_ptr, ra_ipc_handle* out);
+ra_status ra_ipc_open(const ra_ipc_handle* h, void** dev_ptr);
+ra_status ra_ipc_close(void* dev_ptr);
+ra_status ra_peer_slice(size_t count, int P, int rank, size_t* begin, size_t* end);
+ra_status ra_allreduce_peer(float* const* bufs, int P, int rank, size_t count, int sm_budget, int variant, void* stream);
+ra_status ra_alltoall_peer(const void* send, void* const* recv, int P, int rank, size_t chunk_bytes, int sm_budget, int variant,
+                           void* stream);
+
 /* Sets the current device's persisting-L2 carve-out to min(bytes, device maximum) and reports what was granted (host
  * out-pointer, may be NULL; the driver rounds up to eighths of the L2, 15.8 MiB steps on B200); bytes = 0 takes it back and turns the lines it held into normal ones.  This is the state
  * ra_occupancy.l2_persist_bytes manages for the GEMM (see there); the call exists so that a caller who ran ra_gemm with

@@ -30,7 +30,7 @@ EXPORTS = (
     "ra_gemm_workspace_bytes", "ra_gemm", "ra_gemm_ex", "ra_allreduce_emul", "ra_allreduce_emul_ex", "ra_alltoall_emul",
     "ra_alltoall_emul_ex",
     "ra_overlap_run", "ra_overlap_run_host", "ra_overlap_suggest", "ra_overlap_autotune", "ra_overlap_sweep", "ra_set_trace",
-    "ra_l2_persist",
+    "ra_l2_persist", "ra_ipc_export", "ra_ipc_open", "ra_ipc_close", "ra_peer_slice", "ra_allreduce_peer", "ra_alltoall_peer",
 )
 
 
@@ -44,6 +44,11 @@ class Occupancy(Structure):
     _fields_ = [("smem_reserve_bytes", c_int32), ("sm_budget", c_int32), ("tiles_per_cta", c_int32),
                 ("allow_clamp", c_int32), ("cta_group", c_int32), ("m_blocks", c_int32), ("cluster_k", c_int32),
                 ("l2_persist_bytes", c_int32)]
+
+
+class IpcHandle(Structure):
+    """ra_ipc_handle: plain bytes (bytes(handle) / IpcHandle.from_buffer_copy(b)) -- ship it over any transport."""
+    _fields_ = [("opaque", ctypes.c_uint8 * 64), ("offset", ctypes.c_uint64), ("bytes", ctypes.c_uint64)]
 
 
 class GemmPlan(Structure):
@@ -130,6 +135,13 @@ def _L():
     lib.ra_overlap_sweep.argtypes = [POINTER(Workload), POINTER(OverlapCfg), c_int, c_int, POINTER(OverlapResult),
                                      POINTER(c_int)]
     lib.ra_set_trace.argtypes = [c_void_p, c_size_t]
+    lib.ra_l2_persist.argtypes = [ctypes.c_int64, POINTER(ctypes.c_int64)]
+    lib.ra_ipc_export.argtypes = [c_void_p, POINTER(IpcHandle)]
+    lib.ra_ipc_open.argtypes = [POINTER(IpcHandle), POINTER(c_void_p)]
+    lib.ra_ipc_close.argtypes = [c_void_p]
+    lib.ra_peer_slice.argtypes = [c_size_t, c_int, c_int, POINTER(c_size_t), POINTER(c_size_t)]
+    lib.ra_allreduce_peer.argtypes = [POINTER(c_void_p), c_int, c_int, c_size_t, c_int, c_int, c_void_p]
+    lib.ra_alltoall_peer.argtypes = [c_void_p, POINTER(c_void_p), c_int, c_int, c_size_t, c_int, c_int, c_void_p]
     for name in EXPORTS:
         fn = getattr(lib, name)
         if name not in ("ra_status_str", "ra_last_cuda_error", "ra_shutdown", "ra_gemm_workspace_bytes"):
@@ -263,6 +275,46 @@ def ra_alltoall_emul_ex(send, recv, P, chunk_bytes, sm_budget=0, smem_bytes_per_
     _check(_L().ra_alltoall_emul_ex(_ptr(send), _ptr(recv), int(P), int(chunk_bytes), int(sm_budget),
                                     int(smem_bytes_per_cta), int(ctas_per_sm), int(variant), _stream(stream)),
            "ra_alltoall_emul_ex")
+
+
+# ---- N4: peer-memory collectives (one process per GPU; see paper_2606_09200_b200/peer.py for the handle exchange) ----
+def ra_ipc_export(dev) -> bytes:
+    """Handle bytes for a device tensor / pointer of this process."""
+    h = IpcHandle()
+    _check(_L().ra_ipc_export(_ptr(dev), byref(h)), "ra_ipc_export")
+    return bytes(h)
+
+
+def ra_ipc_open(handle: bytes) -> int:
+    """Maps a peer's handle; returns the device pointer (int)."""
+    h = IpcHandle.from_buffer_copy(handle)
+    p = c_void_p(0)
+    _check(_L().ra_ipc_open(byref(h), byref(p)), "ra_ipc_open")
+    return int(p.value)
+
+
+def ra_ipc_close(ptr: int) -> None:
+    _check(_L().ra_ipc_close(c_void_p(int(ptr))), "ra_ipc_close")
+
+
+def ra_peer_slice(count: int, P: int, rank: int) -> tuple:
+    b, e = c_size_t(0), c_size_t(0)
+    _check(_L().ra_peer_slice(int(count), int(P), int(rank), byref(b), byref(e)), "ra_peer_slice")
+    return int(b.value), int(e.value)
+
+
+def ra_allreduce_peer(bufs, rank, count, sm_budget=0, variant=0, stream=None) -> None:
+    """bufs: the P device pointers (tensors or ints) in rank order."""
+    arr = _ptr_array(bufs)
+    _check(_L().ra_allreduce_peer(arr, len(bufs), int(rank), int(count), int(sm_budget), int(variant), _stream(stream)),
+           "ra_allreduce_peer")
+
+
+def ra_alltoall_peer(send, recv, rank, chunk_bytes, sm_budget=0, variant=0, stream=None) -> None:
+    """send: this rank's P chunks; recv: the P ranks' receive buffers (tensors or ints) in rank order."""
+    arr = _ptr_array(recv)
+    _check(_L().ra_alltoall_peer(_ptr(send), arr, len(recv), int(rank), int(chunk_bytes), int(sm_budget), int(variant),
+                                 _stream(stream)), "ra_alltoall_peer")
 
 
 def ra_set_trace(buf, capacity: int = 0) -> None:

@@ -14,7 +14,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(_HERE)
 CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "libra.so")
-SOURCES = ["ra_api.cu", "ra_allreduce.cu", "ra_alltoall.cu", "ra_gemm.cu", "ra_overlap.cu", "ra_policy.cu"]
+SOURCES = ["ra_api.cu", "ra_allreduce.cu", "ra_alltoall.cu", "ra_gemm.cu", "ra_overlap.cu", "ra_policy.cu", "ra_peer.cu"]
 HEADERS = [os.path.join(CSRC, "ra_common.cuh"), os.path.join(ROOT, "include", "ra.h")]
 
 NVCC_FLAGS = [

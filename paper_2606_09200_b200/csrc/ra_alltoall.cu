@@ -46,6 +46,8 @@ __device__ __forceinline__ void bulk_wait_all() {
 struct A2aParams {
     const uint8_t* send;
     uint8_t* recv;
+    uint8_t* peer_recv[RA_MAX_RANKS];   // peer mode (ra_alltoall_peer): rank j's receive buffer; `send` is this rank's row
+    int32_t peer_rank;                  // -1: single-device emulation (send / recv hold all P x P chunks)
     uint32_t P;
     uint32_t slice_bytes;        // S: bytes per ring slot
     uint64_t chunk_bytes;
@@ -57,10 +59,15 @@ __device__ __forceinline__ void a2a_unit(const A2aParams& p, uint64_t u, const u
                                          uint32_t& bytes) {
     const uint64_t c = u / p.slices_per_chunk;
     const uint32_t s = (uint32_t)(u - c * p.slices_per_chunk);
-    const uint32_t i = (uint32_t)(c / p.P), j = (uint32_t)(c - (uint64_t)i * p.P);
     const uint64_t off = (uint64_t)s * p.slice_bytes;
     const uint64_t left = p.chunk_bytes - off;
     bytes = left < p.slice_bytes ? (uint32_t)left : p.slice_bytes;
+    if (p.peer_rank >= 0) {                   // chunk c of this rank's row goes to slot `rank` of rank c's buffer
+        src = p.send + c * p.chunk_bytes + off;
+        dst = p.peer_recv[c] + (uint64_t)p.peer_rank * p.chunk_bytes + off;
+        return;
+    }
+    const uint32_t i = (uint32_t)(c / p.P), j = (uint32_t)(c - (uint64_t)i * p.P);
     src = p.send + ((uint64_t)i * p.P + j) * p.chunk_bytes + off;
     dst = p.recv + ((uint64_t)j * p.P + i) * p.chunk_bytes + off;
 }
@@ -161,6 +168,9 @@ ra_status alltoall_validate(const void* send, const void* recv, int P, size_t ch
     return RA_OK;
 }
 
+static ra_status launch_kernels(A2aParams p, uint64_t n_chunks, const DeviceInfo& di, int sm_budget, int smem_bytes_per_cta,
+                                int ctas_per_sm, int variant, cudaStream_t stream);
+
 ra_status alltoall_launch(const void* send, void* recv, int P, size_t chunk_bytes, int sm_budget,
                           int smem_bytes_per_cta, int ctas_per_sm, int variant, cudaStream_t stream) {
     RA_TRY(alltoall_validate(send, recv, P, chunk_bytes, sm_budget, smem_bytes_per_cta, ctas_per_sm, variant));
@@ -182,13 +192,55 @@ ra_status alltoall_launch(const void* send, void* recv, int P, size_t chunk_byte
         }
         return RA_OK;
     }
-    const int sms = (sm_budget == 0 || sm_budget > di.sm_count) ? di.sm_count : sm_budget;
-
     A2aParams p{};
     p.send = static_cast<const uint8_t*>(send);
     p.recv = static_cast<uint8_t*>(recv);
+    p.peer_rank = -1;
     p.P = (uint32_t)P;
     p.chunk_bytes = chunk_bytes;
+    return launch_kernels(p, (uint64_t)P * P, di, sm_budget, smem_bytes_per_cta, ctas_per_sm, variant, stream);
+}
+
+// N4 (ra_peer.cu): rank `rank` pushes its P chunks into slot `rank` of the P receive buffers (its own included).
+ra_status alltoall_peer_launch(const void* send, void* const* recv, int P, int rank, size_t chunk_bytes, int sm_budget,
+                               int smem_bytes_per_cta, int ctas_per_sm, int variant, cudaStream_t stream) {
+    if (send == nullptr || recv == nullptr || P < 1 || P > RA_MAX_RANKS || rank < 0 || rank >= P) return RA_ERR_INVALID_ARG;
+    if (sm_budget < 0 || smem_bytes_per_cta < 0 || ctas_per_sm < 0 || variant < 0 || variant > 2) return RA_ERR_INVALID_ARG;
+    if ((reinterpret_cast<uintptr_t>(send) & 15u) || chunk_bytes % 16 != 0) return RA_ERR_INVALID_ARG;
+    const uintptr_t s0 = reinterpret_cast<uintptr_t>(send), s1 = s0 + (size_t)P * chunk_bytes;
+    for (int j = 0; j < P; ++j) {
+        if (recv[j] == nullptr || (reinterpret_cast<uintptr_t>(recv[j]) & 15u)) return RA_ERR_INVALID_ARG;
+        const uintptr_t r0 = reinterpret_cast<uintptr_t>(recv[j]), r1 = r0 + (size_t)P * chunk_bytes;
+        if (chunk_bytes > 0 && s0 < r1 && r0 < s1) return RA_ERR_INVALID_ARG;            // send must not alias a receive buffer
+    }
+    if (variant == 0 && chunk_bytes > 0) {
+        const int smem = smem_bytes_per_cta ? smem_bytes_per_cta : kA2aDefaultSmem;
+        if ((((uint32_t)smem / kA2aSlots) & ~127u) < 1024) return RA_ERR_INVALID_ARG;
+    }
+    if (chunk_bytes == 0) return RA_OK;
+    DeviceInfo di;
+    RA_TRY(device_info(&di));
+    RA_TRY(require_sm100(di));
+    if (variant == 2) {                       // copy engines: one peer-to-peer cudaMemcpyAsync per destination
+        for (int j = 0; j < P; ++j)
+            RA_CUDA(cudaMemcpyAsync(static_cast<char*>(recv[j]) + (size_t)rank * chunk_bytes,
+                                    static_cast<const char*>(send) + (size_t)j * chunk_bytes, chunk_bytes, cudaMemcpyDefault, stream));
+        return RA_OK;
+    }
+    A2aParams p{};
+    p.send = static_cast<const uint8_t*>(send);
+    p.recv = nullptr;
+    for (int j = 0; j < P; ++j) p.peer_recv[j] = static_cast<uint8_t*>(recv[j]);
+    p.peer_rank = rank;
+    p.P = (uint32_t)P;
+    p.chunk_bytes = chunk_bytes;
+    return launch_kernels(p, (uint64_t)P, di, sm_budget, smem_bytes_per_cta, ctas_per_sm, variant, stream);
+}
+
+static ra_status launch_kernels(A2aParams p, uint64_t n_chunks, const DeviceInfo& di, int sm_budget, int smem_bytes_per_cta,
+                                int ctas_per_sm, int variant, cudaStream_t stream) {
+    const size_t chunk_bytes = p.chunk_bytes;
+    const int sms = (sm_budget == 0 || sm_budget > di.sm_count) ? di.sm_count : sm_budget;
 
     if (variant == 0) {
         int smem = smem_bytes_per_cta ? smem_bytes_per_cta : kA2aDefaultSmem;
@@ -199,7 +251,7 @@ ra_status alltoall_launch(const void* send, void* recv, int P, size_t chunk_byte
         if (slice > chunk_bytes) slice = (uint32_t)((chunk_bytes + 127) & ~(size_t)127);
         p.slice_bytes = slice;
         p.slices_per_chunk = (uint32_t)((chunk_bytes + slice - 1) / slice);
-        p.n_units = (uint64_t)P * P * p.slices_per_chunk;
+        p.n_units = n_chunks * p.slices_per_chunk;
         const int dyn = (int)(slice * kA2aSlots);
         int cps = ctas_per_sm ? ctas_per_sm : kA2aDefaultCtasPerSm;
         uint64_t grid = (uint64_t)sms * cps;
@@ -210,7 +262,7 @@ ra_status alltoall_launch(const void* send, void* recv, int P, size_t chunk_byte
     } else {
         p.slice_bytes = 64 * 1024;
         p.slices_per_chunk = (uint32_t)((chunk_bytes + p.slice_bytes - 1) / p.slice_bytes);
-        p.n_units = (uint64_t)P * P * p.slices_per_chunk;
+        p.n_units = n_chunks * p.slices_per_chunk;
         int cps = ctas_per_sm ? ctas_per_sm : kCopyCtasPerSm;
         uint64_t grid = (uint64_t)sms * cps;
         if (grid > p.n_units) grid = p.n_units;
