@@ -201,8 +201,8 @@ def sweep_candidates(ra, cfg, quick: bool):
                     elif b < info["sm_count"] or cfg.M <= 128:
                         cands.append(dict(base, coll_variant=tma))
                     cands.append(dict(base, coll_variant=ldg))
-                    if cfg.coll == "alltoall" and csb == 0:
-                        cands.append(dict(base, coll_variant=2))
+                    if csb == 0 and (cfg.coll == "alltoall" or (r == 0 and b == info["sm_count"])):
+                        cands.append(dict(base, coll_variant=2))       # copy engines: all of the alltoall / the allreduce's fan-out
     if cfg.M > 128:
         # L2 as the traded resource: the GEMM keeps an X panel in a persisting carve-out of 1/8 .. 5/8 of the L2 (less DRAM
         # traffic, less energy) and the collective streams through what is left (slower alone, but it is the hidden kernel)
@@ -815,7 +815,7 @@ def run_power_table(args, cfg):
     w_both, k0 = make_workload(ra, cfg, d, n_iters)
     w_gemm, k1 = make_workload(ra, cfg, d, n_iters, coll=False)
     w_coll, k2 = make_workload(ra, cfg, d, n_iters, gemm=False)
-    variants = (0, 1) if cfg.coll == "allreduce" else (0, 1, 2)
+    variants = (0, 1, 2)
     rows = [("K_g alone", w_gemm, dict(mode=0)),
             ("K_g alone, X panel in L2 (79 MiB carve-out)", w_gemm, dict(mode=0, occ=dict(l2_persist_bytes=79 * MiB)))]
     for v in variants:

@@ -200,7 +200,10 @@ ra_status ra_allreduce_emul(float* const* bufs, int P, size_t count, int sm_budg
  * each) per budgeted SM, 1..4 (0 = default 2).  variant 1: TMA ring -- a thread bulk-copies the P rank slices of a unit
  * into a shared-memory slot, 128 threads sum them there in the same rank order (bit-identical result), the first slice is
  * bulk-stored to all P buffers; smem_bytes_per_cta = two slots of P slices (0 = 64 KiB), ctas_per_sm 0 = 2.  This is
- * the variant whose co-residency with the GEMM depends on smem_reserve_bytes.  (Same argument order as
+ * the variant whose co-residency with the GEMM depends on smem_reserve_bytes.  variant 2: the all-gather half on the
+ * copy engines (the mechanism of ConCCL's DMA offload): variant 0's kernel writes the sum to bufs[0] only
+ * (4P + 4 bytes per element through the SMs instead of 8P) and P-1 device-to-device cudaMemcpyAsync on the same stream
+ * fan it out; same bits, 12P - 4 bytes of HBM traffic per element instead of 8P.  (Same argument order as
  * ra_alltoall_emul_ex.) */
 ra_status ra_allreduce_emul_ex(float* const* bufs, int P, size_t count, int sm_budget, int smem_bytes_per_cta, int ctas_per_sm,
                                int variant, void* stream);
@@ -263,7 +266,8 @@ typedef struct {
     int32_t coll_sm_budget;     /* 0 = all SMs */
     int32_t coll_smem_bytes;    /* TMA-ring variants: ring bytes per CTA (0 = default 64 KiB) */
     int32_t coll_ctas_per_sm;   /* collective CTAs per budgeted SM; 0 = default */
-    int32_t coll_variant;       /* alltoall: 0 = TMA ring, 1 = LDG/STG, 2 = copy engines;  allreduce: 0 = LDG/STG, 1 = TMA ring */
+    int32_t coll_variant;       /* alltoall: 0 = TMA ring, 1 = LDG/STG, 2 = copy engines;  allreduce: 0 = LDG/STG, 1 = TMA ring,
+                                   2 = LDG/STG reduce into rank 0 + copy-engine fan-out */
     int32_t prio_compute, prio_comm; /* cudaStreamCreateWithPriority values; equal = "priority off" */
     int32_t dependent;          /* 1: K_c^i waits for K_g^i (the paper's schedule); 0: free-running streams */
     int32_t record_kernel_times;/* 1: per-kernel event pairs (perturbs the schedule slightly) */

@@ -39,7 +39,7 @@ __device__ __forceinline__ void st_stream(float4* p, float4 v) {
 
 template <int P>
 __global__ void __launch_bounds__(kArThreads, kArCtasPerSm)
-allreduce_kernel(const __grid_constant__ ArPtrs ptrs, size_t count, Trace tr) {
+allreduce_kernel(const __grid_constant__ ArPtrs ptrs, size_t count, int n_write, Trace tr) {
     uint64_t* rec = (threadIdx.x == 0) ? trace_begin(tr, KID_ALLREDUCE) : nullptr;
 
     const size_t nvec = count >> 2;
@@ -68,8 +68,11 @@ allreduce_kernel(const __grid_constant__ ArPtrs ptrs, size_t count, Trace tr) {
                 }
             }
         }
+        // n_write = P: the sum goes back to every rank buffer; n_write = 1 (variant 2): to buffer 0 only, the copy
+        // engines fan it out afterwards
 #pragma unroll
-        for (int r = 0; r < P; ++r) st_stream(reinterpret_cast<float4*>(ptrs.p[r]) + v, s);
+        for (int r = 0; r < P; ++r)
+            if (r < n_write) st_stream(reinterpret_cast<float4*>(ptrs.p[r]) + v, s);
     }
     // ragged tail: count % 4 scalars
     if (blockIdx.x == 0) {
@@ -79,7 +82,8 @@ allreduce_kernel(const __grid_constant__ ArPtrs ptrs, size_t count, Trace tr) {
 #pragma unroll
             for (int r = 1; r < P; ++r) s = __fadd_rn(s, ptrs.p[r][e]);
 #pragma unroll
-            for (int r = 0; r < P; ++r) ptrs.p[r][e] = s;
+            for (int r = 0; r < P; ++r)
+                if (r < n_write) ptrs.p[r][e] = s;
         }
     }
     if (threadIdx.x == 0) trace_end(rec);
@@ -192,8 +196,8 @@ allreduce_tma_kernel(const __grid_constant__ ArTmaParams p, Trace tr) {
 }
 
 template <int P>
-static cudaError_t launch_ar(const ArPtrs& ptrs, size_t count, int grid, cudaStream_t stream) {
-    allreduce_kernel<P><<<grid, kArThreads, 0, stream>>>(ptrs, count, g_trace);
+static cudaError_t launch_ar(const ArPtrs& ptrs, size_t count, int n_write, int grid, cudaStream_t stream) {
+    allreduce_kernel<P><<<grid, kArThreads, 0, stream>>>(ptrs, count, n_write, g_trace);
     return cudaGetLastError();
 }
 
@@ -202,7 +206,7 @@ ra_status allreduce_validate(float* const* bufs, int P, size_t count, int sm_bud
                              int variant) {
     if (bufs == nullptr || P < 1 || P > RA_MAX_RANKS) return RA_ERR_INVALID_ARG;
     if (sm_budget < 0 || ctas_per_sm < 0 || ctas_per_sm > kArCtasPerSm) return RA_ERR_INVALID_ARG;
-    if (smem_bytes_per_cta < 0 || (variant != 0 && variant != 1)) return RA_ERR_INVALID_ARG;
+    if (smem_bytes_per_cta < 0 || variant < 0 || variant > 2) return RA_ERR_INVALID_ARG;
     for (int r = 0; r < P; ++r)
         if (bufs[r] == nullptr || (reinterpret_cast<uintptr_t>(bufs[r]) & 15u)) return RA_ERR_INVALID_ARG;
     const size_t bytes = count * sizeof(float);
@@ -229,6 +233,7 @@ ra_status allreduce_launch(float* const* bufs, int P, size_t count, int sm_budge
     DeviceInfo di;
     RA_TRY(device_info(&di));
     RA_TRY(require_sm100(di));
+    RA_TRY(l2_persist_first_use(stream));
     int sms = (sm_budget == 0 || sm_budget > di.sm_count) ? di.sm_count : sm_budget;
     if (variant == 1) {
         int smem = smem_bytes_per_cta ? smem_bytes_per_cta : 64 * 1024;
@@ -264,7 +269,7 @@ ra_status allreduce_launch(float* const* bufs, int P, size_t count, int sm_budge
 
     cudaError_t e;
     switch (P) {
-#define RA_AR_CASE(n) case n: e = launch_ar<n>(ptrs, count, (int)grid, stream); break;
+#define RA_AR_CASE(n) case n: e = launch_ar<n>(ptrs, count, variant == 2 ? 1 : n, (int)grid, stream); break;
         RA_AR_CASE(1) RA_AR_CASE(2) RA_AR_CASE(3) RA_AR_CASE(4) RA_AR_CASE(5) RA_AR_CASE(6) RA_AR_CASE(7) RA_AR_CASE(8)
         RA_AR_CASE(9) RA_AR_CASE(10) RA_AR_CASE(11) RA_AR_CASE(12) RA_AR_CASE(13) RA_AR_CASE(14) RA_AR_CASE(15)
         RA_AR_CASE(16)
@@ -272,6 +277,14 @@ ra_status allreduce_launch(float* const* bufs, int P, size_t count, int sm_budge
         default: return RA_ERR_INVALID_ARG;
     }
     RA_CUDA(e);
+    if (variant == 2) {
+        // the all-gather half on the copy engines (the mechanism of ConCCL's DMA offload): the kernel above
+        // wrote the sum to buffer 0 only -- 4P + 4 bytes per element through the SMs instead of 8P -- and P-1
+        // device-to-device copies, ordered after it on the same stream, put it into the other rank buffers without a
+        // resident CTA.  Same bits; 12P - 4 bytes of HBM traffic per element instead of 8P.
+        for (int r = 1; r < P; ++r)
+            RA_CUDA(cudaMemcpyAsync(bufs[r], bufs[0], count * sizeof(float), cudaMemcpyDeviceToDevice, stream));
+    }
     return RA_OK;
 }
 

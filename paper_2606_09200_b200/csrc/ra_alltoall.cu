@@ -179,6 +179,7 @@ ra_status alltoall_launch(const void* send, void* recv, int P, size_t chunk_byte
     DeviceInfo di;
     RA_TRY(device_info(&di));
     RA_TRY(require_sm100(di));
+    RA_TRY(l2_persist_first_use(stream));
     if (variant == 2) {
         // SM-free variant (the mechanism of ConCCL): the device's copy engines move the chunks;
         // no CTA is ever resident, so the GEMM's occupancy knobs are irrelevant to it.  One plain
@@ -221,6 +222,7 @@ ra_status alltoall_peer_launch(const void* send, void* const* recv, int P, int r
     DeviceInfo di;
     RA_TRY(device_info(&di));
     RA_TRY(require_sm100(di));
+    RA_TRY(l2_persist_first_use(stream));
     if (variant == 2) {                       // copy engines: one peer-to-peer cudaMemcpyAsync per destination
         for (int j = 0; j < P; ++j)
             RA_CUDA(cudaMemcpyAsync(static_cast<char*>(recv[j]) + (size_t)rank * chunk_bytes,

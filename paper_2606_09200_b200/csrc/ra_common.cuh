@@ -42,6 +42,8 @@ ra_status require_sm100(const DeviceInfo& di);
 // last set (then no driver call is made); bytes = 0 also resets the persisting lines.  Must not be called while a
 // stream of the device is being captured unless it is a no-op.
 ra_status l2_persist_ensure(long long bytes, long long* granted = nullptr);
+// Collectives call this before their first launch on a device: takes back a carve-out the context came up with.
+ra_status l2_persist_first_use(cudaStream_t stream);
 
 // Planner constants used when no device is present (plan queries on a CPU-only box): B200 values.
 constexpr int kDefaultSmCount = 148;

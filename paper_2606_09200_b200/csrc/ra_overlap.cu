@@ -72,7 +72,7 @@ static ra_status validate(const ra_workload* w, const ra_overlap_cfg* cfg, ra_ov
     // a failing call must have no side effects, and K_c^0 is launched only after K_g^0 is already in flight
     if (w->kind == RA_COLL_ALLREDUCE) {
         RA_TRY(allreduce_validate(w->ar_bufs, w->P, w->ar_count, cfg->coll_sm_budget, cfg->coll_ctas_per_sm, cfg->coll_smem_bytes,
-                                  cfg->coll_variant == 1 ? 1 : 0));
+                                  cfg->coll_variant));
         if (w->ar_pristine != nullptr) {
             for (int r = 0; r < w->P; ++r) {
                 if (w->ar_pristine[r] == nullptr) return RA_ERR_INVALID_ARG;
@@ -93,7 +93,7 @@ static ra_status validate(const ra_workload* w, const ra_overlap_cfg* cfg, ra_ov
 static ra_status launch_coll(const ra_workload* w, const ra_overlap_cfg* cfg, int iter, cudaStream_t s) {
     if (w->kind == RA_COLL_ALLREDUCE)
         return allreduce_launch(w->ar_bufs, w->P, w->ar_count, cfg->coll_sm_budget, cfg->coll_ctas_per_sm, cfg->coll_smem_bytes,
-                                cfg->coll_variant == 1 ? 1 : 0, s);
+                                cfg->coll_variant, s);
     if (w->kind == RA_COLL_ALLTOALL) {
         const void* src = (iter & 1) ? w->a2a_b : w->a2a_a;
         void* dst = (iter & 1) ? w->a2a_a : w->a2a_b;
@@ -287,7 +287,7 @@ static ra_status run_once(const ra_workload* w, const ra_overlap_cfg* cfg, ra_ov
     std::lock_guard<std::mutex> lk(g_cache.mu);
     const long long want = (w->M > 0 && w->N > 0) ? cfg->occ.l2_persist_bytes : 0;
     if (want < 0) return RA_ERR_INVALID_ARG;
-    if (want > 0) RA_TRY(l2_persist_ensure(want));
+    RA_TRY(l2_persist_ensure(want));          // want = 0 too: a carve-out found on the device is the collective's loss
     ra_status st = run_once_locked(w, cfg, res);
     if (want > 0) {
         const ra_status r = l2_persist_ensure(0);
@@ -407,7 +407,8 @@ ra_status ra_overlap_run_host(const ra_workload* dev0, const ra_workload* dev1, 
     if (dev0->kind == RA_COLL_ALLTOALL && io->a2a_in == nullptr) return RA_ERR_INVALID_ARG;
     const ra_workload* sets[2] = {dev0, dev1};
     const long long want = has_gemm ? cfg->occ.l2_persist_bytes : 0;
-    if (want > 0) RA_TRY(ra::l2_persist_ensure(want));
+    if (want < 0) return RA_ERR_INVALID_ARG;
+    RA_TRY(ra::l2_persist_ensure(want));
     ra_status st = ra::run_host(sets, dev1 ? 2 : 1, io, cfg, n_steps, res);
     if (want > 0) {
         const ra_status r = ra::l2_persist_ensure(0);

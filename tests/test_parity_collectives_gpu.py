@@ -170,3 +170,23 @@ def test_alltoall_errors(ra):
     with pytest.raises(ra.RaError):
         ra.ra_alltoall_emul(a, b, 0, 64)
     ra.ra_alltoall_emul(a, b, 2, 0)             # empty
+
+
+@pytest.mark.parametrize("P", [1, 2, 3, 8, 16])
+@pytest.mark.parametrize("count", [1, 3, 4, 1000, 65536 + 36, 2 * 148 * 512 * 4 + 7])
+def test_allreduce_copy_engine_fanout_matches_oracle(ra, P, count):
+    """variant 2 (ra.h, the DMA-offload mechanism): the kernel reduces into rank 0's buffer only and the copy
+    engines put the sum into the others -- every buffer must still equal the oracle bit for bit."""
+    bufs = [ra_inputs.uniform_f32(count, 555 + P, ra_inputs.STREAM_AR + r) for r in range(P)]
+    ref = [b.copy() for b in bufs]
+    oracle.allreduce(ref)
+    got = _run_allreduce(ra, bufs, variant=2)
+    for r in range(P):
+        _assert_bits_equal(got[r], ref[r])
+
+
+def test_allreduce_copy_engine_fanout_order_and_denormals(ra):
+    bufs = [np.full(4099, 16777216.0 if r == 0 else 1.0, dtype=np.float32) for r in range(8)]
+    assert np.all(_run_allreduce(ra, bufs, variant=2)[7] == np.float32(16777216.0))   # left to right: 2^24 + 1 stays 2^24
+    bufs = [np.full(4099, 2.0 ** -140, dtype=np.float32) for _ in range(2)]
+    assert np.all(_run_allreduce(ra, bufs, variant=2, sm_budget=3)[1] == np.float32(2.0 ** -139))
