@@ -773,6 +773,8 @@ def _occ_from_args(args):
         occ["sm_budget"] = args.sm_budget
     if args.smem_reserve_kib:
         occ["smem_reserve_bytes"] = args.smem_reserve_kib << 10
+    if args.tile_k:
+        occ["tile_k"] = args.tile_k
     return occ
 
 
@@ -800,6 +802,47 @@ def run_gemm_only(args, cfg):
                       "gemm_ms_sustained": g_ms, "gemm_tflops_sustained": cfg.gemm_flops / g_ms / 1e9,
                       "frac_of_bf16_peak_burst": cfg.gemm_flops / gb_ms / 1e9 / peaks["bf16_tflops"],
                       "algorithmic_bytes": cfg.gemm_bytes}))
+
+
+def run_tile_k_table(args):
+    """N3, the paper's tile-size study (Figs. 5-6: execution time of the larger-TILE_K configuration
+    opt2 normalised to opt1, with priority-aware overlap) restated for this GEMM: occ.tile_k = 64 (opt2) against 32 (opt1)
+    on the four full-size configs -- K_g alone, serial, overlapped without and with priority.  Settings interleaved
+    round-robin by ra_overlap_sweep (first third of the runs warm-up).  One JSON line; --table writes markdown."""
+    import torch
+    import paper_2606_09200_b200 as ra
+    hi = ra.ra_device_info()["prio_greatest"]
+    out = []
+    for cfg in ra_inputs.CONFIGS[1:5]:
+        d = device_state(ra, cfg, host_inputs(cfg, pinned=False))
+        n_iters = args.n_iters or cfg.n_iters
+        w_both, k0 = make_workload(ra, cfg, d, n_iters)
+        w_gemm, k1 = make_workload(ra, cfg, d, n_iters, coll=False)
+        variant = 1 if cfg.coll == "alltoall" and cfg.M > 128 else 0
+        row = {"workload": cfg.name}
+        for label, w, kw in (("gemm_alone", w_gemm, dict(mode=0)), ("serial", w_both, dict(mode=0, coll_variant=variant)),
+                             ("overlap", w_both, dict(mode=1, coll_variant=variant)),
+                             ("overlap_priority", w_both, dict(mode=1, coll_variant=variant, prio_comm=hi))):
+            cfgs = [ra.make_cfg(**dict(kw, occ=dict(tile_k=tk))) for tk in (64, 32)]
+            res, _ = ra.ra_overlap_sweep(w, cfgs, runs=max(args.sweep_runs, 9))
+            t64, t32 = res[0]["total_ms"] / n_iters, res[1]["total_ms"] / n_iters
+            row[label] = {"tile_k_64_ms": t64, "tile_k_32_ms": t32, "norm_64_over_32": t64 / t32,
+                          "stages": [res[0]["plan"]["stages"], res[1]["plan"]["stages"]],
+                          "dyn_smem_bytes": [res[0]["plan"]["dyn_smem_bytes"], res[1]["plan"]["dyn_smem_bytes"]]}
+        out.append(row)
+        del d, w_both, w_gemm
+        torch.cuda.empty_cache()
+    print(json.dumps({"mode": "tile-k-table", "rows": out}))
+    if args.table:
+        with open(args.table, "w") as f:
+            f.write("| workload | stages x stage bytes (64 / 32) | K_g alone ms (64 / 32) | norm | serial ms | norm | overlap ms | norm | overlap + priority ms | norm |\n")
+            f.write("|---|---|---|---|---|---|---|---|---|---|\n")
+            for r in out:
+                g = r["gemm_alone"]
+                cells = [r["workload"], f"{g['stages'][0]} / {g['stages'][1]} stages, dyn smem {g['dyn_smem_bytes'][0]} / {g['dyn_smem_bytes'][1]} B"]
+                for k in ("gemm_alone", "serial", "overlap", "overlap_priority"):
+                    cells += [f"{r[k]['tile_k_64_ms']:.4f} / {r[k]['tile_k_32_ms']:.4f}", f"{r[k]['norm_64_over_32']:.3f}"]
+                f.write("| " + " | ".join(cells) + " |\n")
 
 
 def run_power_table(args, cfg):
@@ -882,7 +925,8 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--ref-budget-s", type=float, default=90.0, help="--impl reference: CPU seconds for warmup + steps")
     ap.add_argument("--table", default="", help="write the sweep table (JSON; --mode power-table: markdown) here")
-    ap.add_argument("--mode", default="bench", choices=["bench", "gemm-only", "power-table"],
+    ap.add_argument("--tile-k", type=int, default=0, help="--mode gemm-only: occ.tile_k (32 or 64)")
+    ap.add_argument("--mode", default="bench", choices=["bench", "gemm-only", "power-table", "tile-k-table"],
                     help="gemm-only / power-table: diagnostics behind profiles/ (one GPU, not the bench contract)")
     ap.add_argument("--l2-persist-mib", type=int, default=0, help="--mode gemm-only: occ.l2_persist_bytes in MiB")
     ap.add_argument("--sm-budget", type=int, default=0, help="--mode gemm-only: occ.sm_budget")
@@ -896,6 +940,8 @@ def main():
         return run_gemm_only(args, cfg)
     if args.mode == "power-table":
         return run_power_table(args, cfg)
+    if args.mode == "tile-k-table":
+        return run_tile_k_table(args)
     if args.impl == "reference":
         run_reference(args, cfg)
     else:

@@ -100,6 +100,13 @@ typedef struct {
                                  take it back before returning; ra_l2_persist(0) and ra_shutdown take it back too.
                                  Ignored (reported as 0 in the plan) by swapped, stream-K, cluster split-K and
                                  single-wave plans.  Does not change results (same per-element k order). */
+    int32_t tile_k;           /* 0 / 64 = default: 64 bf16 of K per pipeline stage (128-byte swizzle rows).  32: half-size
+                                 stages (64-byte rows, two UMMA_K steps each) -- the tile-k axis of the paper's opt1 /
+                                 opt2 study (a larger TILE_K gives every block a longer compute window
+                                 and a larger shared-memory footprint).  K-contiguous operands only (transA = 0,
+                                 transB = 1) and no cluster split-K: otherwise clamped to 64 / RA_ERR_INFEASIBLE_KNOB.
+                                 Same per-element k order, so results are bit-identical to tile_k = 64.  Reported in
+                                 ra_gemm_plan.tile_k. */
 } ra_occupancy;
 
 /* What S3 decided -- for tests, logs and the sweep tables. */
@@ -138,7 +145,7 @@ typedef struct {
     int32_t l2_persist_bytes; /* the occupancy knob if this plan uses it, else 0 */
 } ra_gemm_plan;
 
-/* Host-only: computes the plan ra_gemm would use.  `occ` NULL = defaults {0,0,0,1,0,0,0,0}. */
+/* Host-only: computes the plan ra_gemm would use.  `occ` NULL = defaults {0,0,0,1,0,0,0,0,0}. */
 ra_status ra_gemm_plan_query(int transA, int transB, int M, int N, int K, const ra_occupancy* occ, ra_gemm_plan* out);
 
 /* S3 by measurement: every GEMM CTA counts itself in and out on its SM (%smid).  *max_ctas_on_one_sm receives the largest

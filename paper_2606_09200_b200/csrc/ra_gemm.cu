@@ -72,6 +72,7 @@ struct GemmParams {
     int swap;          // 0: C[x*ldc + y]   1: C[y*ldc + x]
     int stream_k;
     int stages;
+    int bk;            // k extent of one pipeline stage: 64 (128-byte swizzle rows) or 32 (64-byte rows; K-major operands only)
     float alpha, beta;
     __nv_bfloat16* C;
     int ldc;
@@ -169,6 +170,16 @@ __device__ __forceinline__ uint64_t umma_desc_sw128(uint32_t smem_addr) {
     d |= (uint64_t)(1024 >> 4) << 32;
     d |= (uint64_t)1 << 46;
     d |= (uint64_t)2 << 61;
+    return d;
+}
+// K-major, 64-byte swizzle (tile_k = 32): rows of 64 B, 8-row groups 512 B apart (SBO), layout type 4 = SWIZZLE_64B.
+__device__ __forceinline__ uint64_t umma_desc_sw64(uint32_t smem_addr) {
+    uint64_t d = 0;
+    d |= (uint64_t)((smem_addr & 0x3FFFFu) >> 4);
+    d |= (uint64_t)1 << 16;
+    d |= (uint64_t)(512 >> 4) << 32;
+    d |= (uint64_t)1 << 46;
+    d |= (uint64_t)4 << 61;
     return d;
 }
 // MN-major, 128-byte swizzle.  The stage holds one 8 KiB box per 64 rows (TMA box = 64 rows x 64 k, the 64 rows
@@ -525,12 +536,16 @@ gemm_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constant__ CU
     static_assert(CG == 1 || CG == 2, "CG");
     static_assert(XH == 1 || XH == 2, "XH");
     static_assert(kStageBytes == stage_bytes(BN, CG, XH), "stage size");
+    // tile_k = 32 halves every piece of a stage (the constants above are the tile_k = 64 sizes)
+    const int bk_shift = (p.bk == 32) ? 1 : 0;
+    const uint32_t xhalf_bytes = (uint32_t)kXHalfBytes >> bk_shift, xbytes = (uint32_t)kXBytes >> bk_shift;
+    const uint32_t stage_sz = (uint32_t)kStageBytes >> bk_shift;
 
     extern __shared__ uint8_t smem_raw[];
     // 1024-byte alignment for the 128B swizzle; the barrier block sits after the stages.  Both CTAs of a pair
     // compute identical offsets (same kernel, same dynamic-smem base), which cta_group::2 relies on.
     const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
-    const uint32_t epi_base = smem_base + p.stages * kStageBytes;     // staging for TMA stores (epi_tma only)
+    const uint32_t epi_base = smem_base + p.stages * stage_sz;     // staging for TMA stores (epi_tma only)
     const uint32_t bar_base = epi_base + (p.epi_tma ? kEpiStageBytes : 0);
     auto full_bar = [&](int s) { return bar_base + 8u * s; };
     auto empty_bar = [&](int s) { return bar_base + 8u * (kMaxStages + s); };
@@ -602,28 +617,28 @@ gemm_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constant__ CU
                 const int y0 = ty * BN + (int)rank * kYRows;
                 for (int kb = sg.kb0; kb < sg.kb1; ++kb) {
                     mbar_wait(empty_bar(stage), phase ^ 1u);           // local: MMAs reading this stage retired
-                    const uint32_t sx = smem_base + stage * kStageBytes;
+                    const uint32_t sx = smem_base + stage * stage_sz;
                     uint32_t bar;
                     if constexpr (CG == 1) {
                         bar = full_bar(stage);
-                        mbar_expect_tx(bar, kStageBytes);
+                        mbar_expect_tx(bar, stage_sz);
                     } else {
                         bar = mapa(full_bar(stage), lead);            // the leader's barrier collects both halves
-                        mbar_expect_tx_cluster(bar, kStageBytes);
+                        mbar_expect_tx_cluster(bar, stage_sz);
                     }
                     // K-major operand: one box (64 k x rows).  MN-major operand: one box (64 rows x 64 k) per 64 rows.
                     if (!p.xmn) {
-                        tma_load_2d<CG>(sx, &mapX, kb * kBK, x0, bar, polX);
+                        tma_load_2d<CG>(sx, &mapX, kb * p.bk, x0, bar, polX);
                     } else {
 #pragma unroll
                         for (int b = 0; b < kBM * XH / 64; ++b) tma_load_2d<CG>(sx + b * 8192, &mapX, x0 + 64 * b, kb * kBK, bar, polX);
                     }
                     if (!p.ymn) {
-                        tma_load_2d<CG>(sx + kXBytes, &mapY, kb * kBK, y0, bar, polY);
+                        tma_load_2d<CG>(sx + xbytes, &mapY, kb * p.bk, y0, bar, polY);
                     } else {
 #pragma unroll
                         for (int b = 0; b < kYRows / 64; ++b)
-                            tma_load_2d<CG>(sx + kXBytes + b * 8192, &mapY, y0 + 64 * b, kb * kBK, bar, polY);
+                            tma_load_2d<CG>(sx + xbytes + b * 8192, &mapY, y0 + 64 * b, kb * kBK, bar, polY);
                     }
                     if (++stage == p.stages) { stage = 0; phase ^= 1u; }
                 }
@@ -641,10 +656,17 @@ gemm_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constant__ CU
             const int kx_step = p.xmn ? (2048 >> 4) : (32 >> 4), ky_step = p.ymn ? (2048 >> 4) : (32 >> 4);
             // the four UMMA_K steps of X block h against the Y rows of one stage, into accumulator column acc_col
             auto issue_block = [&](int st, int h, uint32_t acc_col, bool first) {
-                const uint32_t sx = smem_base + st * kStageBytes;
-                const uint32_t sxh = sx + h * kXHalfBytes;
+                const uint32_t sx = smem_base + st * stage_sz;
+                const uint32_t sxh = sx + h * xhalf_bytes;
+                if (bk_shift) {                    // tile_k = 32: two UMMA_K steps per stage, 64-byte swizzle (K-major operands only)
+                    const uint64_t dx = umma_desc_sw64(sxh), dy = umma_desc_sw64(sx + xbytes);
+#pragma unroll
+                    for (int k = 0; k < 2; ++k)
+                        umma_bf16<CG>(tmem_base + acc_col, dx + (uint64_t)(2 * k), dy + (uint64_t)(2 * k), idesc, (!first || k > 0) ? 1u : 0u);
+                    return;
+                }
                 const uint64_t dx = p.xmn ? umma_desc_sw128_mn(sxh) : umma_desc_sw128(sxh);
-                const uint64_t dy = p.ymn ? umma_desc_sw128_mn(sx + kXBytes) : umma_desc_sw128(sx + kXBytes);
+                const uint64_t dy = p.ymn ? umma_desc_sw128_mn(sx + xbytes) : umma_desc_sw128(sx + xbytes);
 #pragma unroll
                 for (int k = 0; k < kBK / kUmmaK; ++k) {
                     // per UMMA_K step: K-major +32 B inside the swizzle atom, MN-major +2 k-groups of 1024 B
@@ -983,15 +1005,16 @@ static ra_status get_encode(EncodeTiledFn* fn) {
 
 // K-major operand: rows x K bf16, row pitch ld; box = 64 (k) x box_rows.  MN-major operand: K x rows bf16 (rows
 // contiguous), pitch ld; box = 64 (rows) x 64 (k).  128-byte swizzle, OOB -> zeros.
-static ra_status make_map(CUtensorMap* map, const void* base, int rows, int K, int ld, int box_rows, int mn_major) {
+static ra_status make_map(CUtensorMap* map, const void* base, int rows, int K, int ld, int box_rows, int mn_major, int bk = kBK) {
     EncodeTiledFn enc;
     RA_TRY(get_encode(&enc));
     const cuuint64_t dims[2] = {(cuuint64_t)(mn_major ? rows : K), (cuuint64_t)(mn_major ? K : rows)};
     const cuuint64_t strides[1] = {(cuuint64_t)ld * 2};
-    const cuuint32_t box[2] = {(cuuint32_t)(mn_major ? 64 : kBK), (cuuint32_t)(mn_major ? kBK : box_rows)};
+    const cuuint32_t box[2] = {(cuuint32_t)(mn_major ? 64 : bk), (cuuint32_t)(mn_major ? kBK : box_rows)};
     const cuuint32_t estr[2] = {1, 1};
     const CUresult r = enc(map, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(base), dims, strides, box, estr,
-                           CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                           CU_TENSOR_MAP_INTERLEAVE_NONE, (!mn_major && bk == 32) ? CU_TENSOR_MAP_SWIZZLE_64B : CU_TENSOR_MAP_SWIZZLE_128B,
+                           CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
                            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) {
         g_last_cuda_error = (int)cudaErrorInvalidValue;
@@ -1071,7 +1094,7 @@ static ra_status validate_shape(int transA, int transB, int M, int N, int K) {
 
 static ra_status make_plan(int transA, int transB, int M, int N, int K, const ra_occupancy* occ_in, Plan* out) {
     RA_TRY(validate_shape(transA, transB, M, N, K));
-    ra_occupancy occ = {0, 0, 0, 1, 0, 0, 0, 0};
+    ra_occupancy occ = {0, 0, 0, 1, 0, 0, 0, 0, 0};
     if (occ_in) occ = *occ_in;
     if (occ.smem_reserve_bytes < 0 || occ.sm_budget < 0 || occ.tiles_per_cta < 0) return RA_ERR_INVALID_ARG;
 
@@ -1106,7 +1129,20 @@ static ra_status make_plan(int transA, int transB, int M, int N, int K, const ra
     const int swap = ((M <= 64 && N >= 128) || (M <= 128 && N >= 1024)) ? 1 : 0;
     const int RX = swap ? N : M, RY = swap ? M : N;
     int bn = RY > 128 ? 256 : (RY > 64 ? 128 : 64);
-    const int kb = (K + kBK - 1) / kBK;
+    // tile_k (N3: the paper's opt1 / opt2 differ in TILE_K): 32 halves every pipeline stage (64-byte
+    // swizzle rows, two UMMA_K steps per stage).  K-contiguous operands only; cluster split-K keeps 64.
+    if (occ.tile_k != 0 && occ.tile_k != 32 && occ.tile_k != 64) return RA_ERR_INVALID_ARG;
+    int bk = kBK;
+    if (occ.tile_k == 32) {
+        if (transA == 0 && transB == 1 && occ.cluster_k < 2) {
+            bk = 32;
+        } else {
+            if (!occ.allow_clamp) return RA_ERR_INFEASIBLE_KNOB;
+            clamped = 1;
+        }
+    }
+    const int kb = (K + bk - 1) / bk;
+    auto stage_bytes = [bk](int bn_, int cg_, int xh_) { return ra::stage_bytes(bn_, cg_, xh_) * bk / kBK; };
     // Small problems: when narrower tiles still fit in ONE wave, take them -- more CTAs share the work and each CTA's
     // serial tail (TMEM drain + stores, ~0.45 us per 64-column box per warp) shrinks with the tile; operand re-use per
     // byte is worse but nothing is bandwidth-bound at this size (1024^3: 13 us with 256 x 256 pair tiles on 32 CTAs).
@@ -1279,9 +1315,9 @@ static ra_status make_plan(int transA, int transB, int M, int N, int K, const ra
         // that stream-K's finer split wins) and the receiving stage ring can hold a 128 x BN fp32 accumulator.
         const long ring = (long)stages * stage_bytes(bn, cg, 1), slot = (long)kBM * bn * 4;
         // 4-CTA clusters (four single-CTA parts, or two CTA pairs) must also fit the chip's cluster capacity
-        const bool ks2_fits = xh == 1 && n_tiles > 0 && 2 * n_tiles <= workers && kb >= 2 && ring >= slot &&
+        const bool ks2_fits = bk == kBK && xh == 1 && n_tiles > 0 && 2 * n_tiles <= workers && kb >= 2 && ring >= slot &&
                               (cg == 1 || n_tiles <= max_clusters4);
-        const bool ks4_fits = xh == 1 && cg == 1 && n_tiles > 0 && 4 * n_tiles <= workers && kb >= 4 && ring >= 3 * slot &&
+        const bool ks4_fits = bk == kBK && xh == 1 && cg == 1 && n_tiles > 0 && 4 * n_tiles <= workers && kb >= 4 && ring >= 3 * slot &&
                               n_tiles <= max_clusters4;
         if (ks4_fits && occ.cluster_k != 1 && occ.cluster_k != 2 && (kb >= 32 || occ.cluster_k == 4)) {
             ks = 4;                                   // four single-CTA parts per tile, three slots in part 0's ring
@@ -1306,7 +1342,7 @@ static ra_status make_plan(int transA, int transB, int M, int N, int K, const ra
     g.stages = stages;
     g.tile_m = swap ? bn : tile_x;
     g.tile_n = swap ? kBM : bn;
-    g.tile_k = kBK;
+    g.tile_k = bk;
     g.swap_ab = swap;
     g.dyn_smem_bytes = dyn;
     g.smem_left_per_sm = smem_per_sm - ctas_per_sm * (dyn + reserved);
@@ -1429,7 +1465,8 @@ static ra_status build_entry(const LaunchKey& k, const DeviceInfo& di, LaunchEnt
     p.tiles_x = (p.RX + tile_x - 1) / tile_x;
     p.tiles_y = (p.RY + pl.bn - 1) / pl.bn;
     p.n_tiles = pl.pub.n_tiles;
-    p.kb_per_tile = (K + kBK - 1) / kBK;
+    p.bk = pl.pub.tile_k;
+    p.kb_per_tile = (K + p.bk - 1) / p.bk;
     p.swap = swap;
     p.stream_k = pl.pub.split_k > 1;
     p.stages = pl.pub.stages;
@@ -1448,8 +1485,8 @@ static ra_status build_entry(const LaunchKey& k, const DeviceInfo& di, LaunchEnt
     const int a_mn = transA ? 1 : 0, b_mn = transB ? 0 : 1;
     p.xmn = swap ? b_mn : a_mn;
     p.ymn = swap ? a_mn : b_mn;
-    RA_TRY(make_map(&e->mx, X, p.RX, K, ldx, kBM * xh, p.xmn));
-    RA_TRY(make_map(&e->my, Y, p.RY, K, ldy, pl.bn / cg, p.ymn));
+    RA_TRY(make_map(&e->mx, X, p.RX, K, ldx, kBM * xh, p.xmn, p.bk));
+    RA_TRY(make_map(&e->my, Y, p.RY, K, ldy, pl.bn / cg, p.ymn, p.bk));
     p.c_f32 = k.c_f32;
     p.epi_tma = k.c_f32 ? 0 : pl.epi_tma;      // fp32 rows are written directly: 128 contiguous bytes per thread and chunk
     p.ks = pl.pub.cluster_k;
@@ -1486,7 +1523,7 @@ ra_status gemm_launch(int transA, int transB, int M, int N, int K, float alpha, 
         const uintptr_t b0 = reinterpret_cast<uintptr_t>(B), b1 = b0 + b_elems * 2;
         if (K > 0 && ((c0 < a1 && a0 < c1) || (c0 < b1 && b0 < c1))) return RA_ERR_INVALID_ARG;
     }
-    ra_occupancy occ_v = {0, 0, 0, 1, 0, 0, 0, 0};
+    ra_occupancy occ_v = {0, 0, 0, 1, 0, 0, 0, 0, 0};
     if (occ) occ_v = *occ;
 
     if (K == 0 || alpha == 0.f) {

@@ -478,3 +478,49 @@ def test_l2_persist_same_bits_and_state(ra):
     ref, _ = oracle.gemm(0, 1, M, N, K, 1.0, A, B)
     rowA, colB = oracle.gemm_norms(0, 1, M, N, K, A, B)
     assert gemm_norm_err(got, ref, rowA, colB) <= GEMM_TOL
+
+
+@pytest.mark.parametrize("M,N,K,occ", [
+    (256, 256, 256, {}),                                     # Tiny
+    (1024, 768, 2048, dict(cta_group=2, m_blocks=2)),        # big tiles, skewed issue over 64 k-blocks of 32
+    (2048, 1024, 1024, dict(cta_group=2, m_blocks=1)),       # pair tiles
+    (64, 2048, 4096, {}),                                    # skinny (operands swapped)
+    (200, 136, 72, {}),                                      # ragged everywhere: K = 72 -> 3 k-blocks, the last 8 wide
+    (129, 67, 40, {}),
+    (1000, 3000, 520, dict(cluster_k=1)),                    # ragged multi-wave single-CTA tiles: stream-K over 32-wide units
+    (512, 512, 8192, dict(sm_budget=37)),
+])
+def test_tile_k_32_same_bits_as_64(ra, M, N, K, occ):
+    """occ.tile_k = 32 (ra.h; the tile-k axis of PAPER.md:140-144): half-size stages in 64-byte swizzle rows.  A
+    data-parallel tile accumulates the same products in the same ascending-k order whatever the stage size, so C is
+    bit-identical to tile_k = 64; stream-K plans cut K at different unit boundaries (tolerance there).  Oracle-exact on
+    integer operands in any case."""
+    occ = dict(occ, cluster_k=1)         # tile_k = 32 has no cluster split-K: compare like with like (same fp32 association)
+    lda, ldb, ldc = _up8(K), _up8(K), _up8(N)
+    A = ra_inputs.normal_bf16((M, lda), 90, ra_inputs.STREAM_A)
+    B = ra_inputs.normal_bf16((N, ldb), 90, ra_inputs.STREAM_B)
+    p64 = ra.ra_gemm_plan_query(0, 1, M, N, K, dict(occ, tile_k=64))
+    p32 = ra.ra_gemm_plan_query(0, 1, M, N, K, dict(occ, tile_k=32))
+    assert p32["tile_k"] == 32 and p64["tile_k"] == 64 and p32["clamped"] == 0, p32
+    c64, _ = run_gemm(ra, M, N, K, A, B, occ=dict(occ, tile_k=64), lda=lda, ldb=ldb, ldc=ldc)
+    c32, full = run_gemm(ra, M, N, K, A, B, occ=dict(occ, tile_k=32), lda=lda, ldb=ldb, ldc=ldc)
+    assert np.all(full[:, N:] == 0x7FC0)                                    # pad columns of C untouched
+    ref, _ = oracle.gemm(0, 1, M, N, K, 1.0, A, B, lda=lda, ldb=ldb)
+    rowA, colB = oracle.gemm_norms(0, 1, M, N, K, A, B, lda=lda, ldb=ldb)
+    assert gemm_norm_err(c32, ref, rowA, colB) <= GEMM_TOL
+    if p32["split_k"] == 1 and p64["split_k"] == 1:
+        assert c32.tobytes() == c64.tobytes()
+    Ai = ra_inputs.smallint_bf16((M, lda), 91, ra_inputs.STREAM_A)
+    Bi = ra_inputs.smallint_bf16((N, ldb), 91, ra_inputs.STREAM_B)
+    ci, _ = run_gemm(ra, M, N, K, Ai, Bi, occ=dict(occ, tile_k=32), lda=lda, ldb=ldb, ldc=ldc)
+    _, ref16 = oracle.gemm(0, 1, M, N, K, 1.0, Ai, Bi, lda=lda, ldb=ldb)
+    assert ci.tobytes() == ref16.tobytes()
+
+
+def test_tile_k_32_is_clamped_where_it_cannot_apply(ra):
+    p = ra.ra_gemm_plan_query(1, 1, 1024, 1024, 1024, dict(tile_k=32))        # MN-major A
+    assert p["tile_k"] == 64 and p["clamped"] == 1
+    with pytest.raises(ra.RaError):
+        ra.ra_gemm_plan_query(1, 1, 1024, 1024, 1024, dict(tile_k=32, allow_clamp=0))
+    with pytest.raises(ra.RaError):
+        ra.ra_gemm_plan_query(0, 1, 1024, 1024, 1024, dict(tile_k=48))
