@@ -547,6 +547,11 @@ def measure_config(ra, cfg, args, peaks, world, dev, headline: bool):
     cand_kws = [dict(mode=0, use_graph=graph)] + [dict(mode=1, use_graph=graph)] + [sug["kw"]] + cands
     runs = args.sweep_runs if sweep != "config5" else max(6, args.sweep_runs - 3)
     results, best = ra.ra_overlap_sweep(w, [ra.make_cfg(**kw) for kw in cand_kws], runs=runs)
+    sweep_argmin = best
+    # S7 picks the argmin; settings closer than the run-to-run spread of a power-capped step (~1 %, profiles/r02_l2_persist.md 3)
+    # are a tie, and a tie goes to the policy's setting (index 2) so that the timed setting is not chosen by noise
+    if sweep != "none" and results[2]["total_ms"] <= 1.01 * results[best]["total_ms"]:
+        best = 2
     best_kw = cand_kws[best]
     sweep_serial_ms = results[0]["total_ms"] / n_iters
     sweep_table = [dict(cfg_label(kw), mode=kw["mode"], ms_per_iter=r["total_ms"] / n_iters, median=r["median_ms"] / n_iters,
@@ -561,8 +566,8 @@ def measure_config(ra, cfg, args, peaks, world, dev, headline: bool):
             on, off = (results[best]["total_ms"], r["total_ms"]) if lab["priority"] == "on" else (r["total_ms"], results[best]["total_ms"])
             norm_time = on / off
     policy = {"setting": cfg_label(sug["kw"]), "predicted_ms_per_iter": sug["t_overlap_ms"], "measured_ms_per_iter": results[2]["total_ms"] / n_iters,
-              "sweep_best_ms_per_iter": results[best]["total_ms"] / n_iters,
-              "regret": results[2]["total_ms"] / results[best]["total_ms"] - 1.0, "gemm_bound": sug["gemm_bound"],
+              "sweep_best_ms_per_iter": results[sweep_argmin]["total_ms"] / n_iters, "sweep_argmin_setting": cfg_label(cand_kws[sweep_argmin]),
+              "regret": results[2]["total_ms"] / results[sweep_argmin]["total_ms"] - 1.0, "timed_setting_is": "policy (tie within 1 %)" if best == 2 and sweep_argmin != 2 else "sweep argmin", "gemm_bound": sug["gemm_bound"],
               "model_roofline_ms": sug["t_roofline_ms"], "settings_in_sweep": len(cand_kws) - 1}
     alone = kernels_alone(ra, cfg, d, peaks, n_iters, graph=graph)
     residency = residency_map(ra, w, best_kw, info["sm_count"]) if headline else None

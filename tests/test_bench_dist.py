@@ -37,3 +37,18 @@ def test_reference_arm_world2_prints_one_line():
     assert d["impl"] == "reference" and d["unit"] == "iter/s" and d["value"] > 0
     assert d["cpu_baseline"]["kind"] == "oracle" and d["e2e"]["h2d_bytes_per_step"] == 0
     assert d["config"]["workload"] == "tiny" and d["gpu_launches"] == 0
+
+
+def test_plain_python_launch_starts_its_own_ranks():
+    """`python bench.py --gpus 2` WITHOUT a torchrun wrapper (how the driver may start it): bench.py re-executes itself
+    under torch.distributed.run, one process per rank, and rank 0 prints one line with n_gpus = 2."""
+    env = dict(os.environ, CUDA_VISIBLE_DEVICES="", OMP_NUM_THREADS="2")
+    for k in ("WORLD_SIZE", "RANK", "LOCAL_RANK", "MASTER_ADDR", "MASTER_PORT"):
+        env.pop(k, None)
+    r = subprocess.run([sys.executable, "bench.py", "--impl", "reference", "--gpus", "2", "--steps", "1", "--warmup", "0",
+                        "--config", "tiny"], cwd=ROOT, env=env, capture_output=True, text=True, timeout=600)
+    assert r.returncode == 0, r.stderr[-2000:]
+    lines = [ln for ln in r.stdout.splitlines() if ln.startswith("{")]
+    assert len(lines) == 1
+    d = json.loads(lines[0])
+    assert d["impl"] == "reference" and d["n_gpus"] == 2 and d["value"] > 0
