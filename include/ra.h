@@ -362,10 +362,12 @@ ra_status ra_overlap_suggest(const ra_workload* w, const ra_peaks* peaks, ra_sug
 ra_status ra_overlap_autotune(const ra_workload* w, const ra_peaks* peaks, int runs, ra_overlap_cfg* best_cfg,
                               ra_overlap_result* best_res, int* n_tried);
 
-/* Runs cfgs[0..n) `runs` times each, interleaved round-robin so that clock drift hits all settings
- * alike; the first runs/3 passes are warm-up and the mean of the rest is stored in results[i].total_ms
- * ("the first one-third of runs are considered warm-up").  *best = argmin over
- * settings with mode == RA_MODE_OVERLAP (or over all if none).  Host pointers all. */
+/* Times cfgs[0..n): every setting is run as one block of consecutive runs, the first of them warm-up, and the mean
+ * of the remaining runs - runs/3 is stored in results[i].total_ms ("30 runs ... the first one-third of runs
+ * are considered warm-up").  The warm-up lasts runs/3 runs or, with n > 1 and if that is longer, until the setting has run
+ * for ~120 ms (at most 12 runs): a power-capped step is otherwise timed in the clock / power state the previous setting
+ * left behind (measured on cb-ar: ~100 ms at 0.80 ms per iteration after a lighter setting before it settles at
+ * 0.90-0.94).  *best = argmin over settings with mode == RA_MODE_OVERLAP (or over all if none).  Host pointers all. */
 ra_status ra_overlap_sweep(const ra_workload* w, const ra_overlap_cfg* cfgs, int n, int runs,
                            ra_overlap_result* results, int* best);
 

@@ -426,17 +426,31 @@ ra_status ra_overlap_sweep(const ra_workload* w, const ra_overlap_cfg* cfgs, int
                            int* best) {
     if (cfgs == nullptr || results == nullptr || n < 1 || runs < 1) return RA_ERR_INVALID_ARG;
     for (int i = 0; i < n; ++i) RA_TRY(ra::validate(w, &cfgs[i], &results[i]));
-    const int warm = runs / 3;   // first third of the runs is warm-up
+    // "30 runs ... the first one-third of runs are considered warm-up": every setting is run as ONE BLOCK of
+    // consecutive runs whose first part is discarded.  Blocks, not a round-robin over settings: a power-capped step is
+    // timed in the clock / power state its predecessor left behind -- measured on cb-ar: the first ~6 runs (~100 ms) after
+    // a lighter setting read 0.80 ms per iteration, the settled ones 0.90-0.94 -- so the warm-up is what makes a setting
+    // its own predecessor.  It lasts runs/3 runs or, if longer, until the setting has run for ~120 ms (at most 12 runs).
+    const int warm_min = runs / 3;
+    const int timed = runs - warm_min;
     std::vector<std::vector<float>> samples((size_t)n);
-    for (int r = 0; r < runs; ++r) {
-        for (int i = 0; i < n; ++i) {
+    for (int i = 0; i < n; ++i) {
+        int warm = warm_min;
+        for (int r = 0; r < warm + timed; ++r) {
             ra_overlap_result one = results[i];
             ra_overlap_cfg c = cfgs[i];
-            // per-kernel events only on the last pass, so they cannot perturb the timed passes
-            c.record_kernel_times = (r == runs - 1) ? cfgs[i].record_kernel_times : 0;
+            const bool last = (r == warm + timed - 1);
+            // per-kernel events only on the last run, so they cannot perturb the timed runs
+            c.record_kernel_times = last ? cfgs[i].record_kernel_times : 0;
+            if (!last) one.kernel_times = nullptr;
             RA_TRY(ra::run_once(w, &c, &one));
-            if (r >= warm && !(c.record_kernel_times && runs - warm > 1)) samples[i].push_back(one.total_ms);
-            if (r == runs - 1) {
+            if (r == 0 && n > 1 && one.total_ms > 0.f) {
+                int need = (int)(120.f / one.total_ms) + 1;
+                if (need > 12) need = 12;
+                if (need > warm) warm = need;
+            }
+            if (r >= warm && !(c.record_kernel_times && timed > 1)) samples[i].push_back(one.total_ms);
+            if (last) {
                 float* kt = results[i].kernel_times;
                 results[i] = one;
                 results[i].kernel_times = kt;
