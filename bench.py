@@ -261,6 +261,37 @@ def residency_map(ra, w, cfg_kw, n_sms):
     return out
 
 
+def library_gemm_same_box(cfg, d, n_iters):
+    """Yardstick only (never on the product path): the library GEMM (cuBLAS through torch.matmul) on the SAME box, same operands,
+    same two protocols as our kernel -- best of 10 single launches, and 6 x n_iters back to back.  MEASURED_PEAKS.json was taken on
+    whichever box the driver used; boxes of the pool differ by ~4 %, so this is the like-for-like reference."""
+    import torch
+    A = d["A"].view(torch.bfloat16)
+    B = d["B"].view(torch.bfloat16)
+    C = torch.empty((cfg.M, cfg.N), dtype=torch.bfloat16, device="cuda")
+    fn = lambda: torch.matmul(A, B.t(), out=C)
+    for _ in range(3):
+        fn()
+    torch.cuda.synchronize()
+    burst = []
+    for _ in range(10):
+        time.sleep(0.05)
+        e0, e1 = torch.cuda.Event(True), torch.cuda.Event(True)
+        e0.record(); fn(); e1.record(); torch.cuda.synchronize()
+        burst.append(e0.elapsed_time(e1))
+    runs = []
+    for r in range(6):
+        e0, e1 = torch.cuda.Event(True), torch.cuda.Event(True)
+        e0.record()
+        for _ in range(n_iters):
+            fn()
+        e1.record(); torch.cuda.synchronize()
+        runs.append(e0.elapsed_time(e1) / n_iters)
+    sus = statistics.mean(runs[2:])
+    return {"what": "torch.matmul (cuBLAS) bf16, same operands, same box", "burst_ms": min(burst), "burst_tflops": cfg.gemm_flops / min(burst) / 1e9,
+            "sustained_ms": sus, "sustained_tflops": cfg.gemm_flops / sus / 1e9}
+
+
 def kernels_alone(ra, cfg, d, peaks, n_iters, graph: int = 0):
     """Each kernel by itself (CUDA events inside the library, on the stream the kernel runs on)."""
     out = {}
@@ -284,6 +315,8 @@ def kernels_alone(ra, cfg, d, peaks, n_iters, graph: int = 0):
     out["gemm_gbs"] = cfg.gemm_bytes / g_ms / 1e6
     out["gemm_frac_of_hbm_peak"] = out["gemm_gbs"] / peaks["hbm_gbs"]
     out["gemm_plan"] = res[0]["plan"]
+    if cfg.M > 128 and cfg.M * cfg.N >= 1 << 22:
+        out["library_gemm_same_box"] = library_gemm_same_box(cfg, d, n_iters)
     w, keep = make_workload(ra, cfg, d, n_iters, gemm=False)
     # the collective alone is a bandwidth measurement: let the clocks recover from the power-capped GEMM runs first
     import torch
@@ -548,9 +581,9 @@ def measure_config(ra, cfg, args, peaks, world, dev, headline: bool):
     runs = args.sweep_runs if sweep != "config5" else max(6, args.sweep_runs - 3)
     results, best = ra.ra_overlap_sweep(w, [ra.make_cfg(**kw) for kw in cand_kws], runs=runs)
     sweep_argmin = best
-    # S7 picks the argmin; settings closer than the run-to-run spread of a power-capped step (~1 %, profiles/r02_l2_persist.md 3)
-    # are a tie, and a tie goes to the policy's setting (index 2) so that the timed setting is not chosen by noise
-    if sweep != "none" and results[2]["total_ms"] <= 1.01 * results[best]["total_ms"]:
+    # S7 picks the argmin; settings closer than the run-to-run spread of a power-capped step (1-2 %, profiles/r02_l2_persist.md 3)
+    # are a tie (2.5 %), and a tie goes to the policy's setting (index 2) so that the timed setting is not chosen by noise
+    if sweep != "none" and results[2]["total_ms"] <= 1.025 * results[best]["total_ms"]:
         best = 2
     best_kw = cand_kws[best]
     sweep_serial_ms = results[0]["total_ms"] / n_iters
@@ -567,7 +600,7 @@ def measure_config(ra, cfg, args, peaks, world, dev, headline: bool):
             norm_time = on / off
     policy = {"setting": cfg_label(sug["kw"]), "predicted_ms_per_iter": sug["t_overlap_ms"], "measured_ms_per_iter": results[2]["total_ms"] / n_iters,
               "sweep_best_ms_per_iter": results[sweep_argmin]["total_ms"] / n_iters, "sweep_argmin_setting": cfg_label(cand_kws[sweep_argmin]),
-              "regret": results[2]["total_ms"] / results[sweep_argmin]["total_ms"] - 1.0, "timed_setting_is": "policy (tie within 1 %)" if best == 2 and sweep_argmin != 2 else "sweep argmin", "gemm_bound": sug["gemm_bound"],
+              "regret": results[2]["total_ms"] / results[sweep_argmin]["total_ms"] - 1.0, "timed_setting_is": "policy (tie within 2.5 %)" if best == 2 and sweep_argmin != 2 else "sweep argmin", "gemm_bound": sug["gemm_bound"],
               "model_roofline_ms": sug["t_roofline_ms"], "settings_in_sweep": len(cand_kws) - 1}
     alone = kernels_alone(ra, cfg, d, peaks, n_iters, graph=graph)
     residency = residency_map(ra, w, best_kw, info["sm_count"]) if headline else None
@@ -675,7 +708,9 @@ def flat_summary(m, peaks):
     """One config's report lines as a single string: survives a parser that keeps only scalars."""
     a, b = m["alone"], m["best_setting"]
     gem = (f"gemm alone {a['gemm_tflops_burst']:.0f} TF/s burst={a['gemm_frac_of_bf16_peak_burst']:.3f} of bf16 peak, "
-           f"{a['gemm_tflops']:.0f} sustained={a['gemm_frac_of_bf16_peak_sustained']:.3f}" if m["compute_bound"] else
+           f"{a['gemm_tflops']:.0f} sustained={a['gemm_frac_of_bf16_peak_sustained']:.3f}"
+           + (f" (cuBLAS same box {a['library_gemm_same_box']['burst_tflops']:.0f} / {a['library_gemm_same_box']['sustained_tflops']:.0f})"
+              if "library_gemm_same_box" in a else "") if m["compute_bound"] else
            f"gemm alone {a['gemm_gbs']:.0f} GB/s={a['gemm_frac_of_hbm_peak']:.3f} of HBM peak ({a['gemm_tflops']:.0f} TF/s)")
     return (f"serial {m['serial_ms_per_iter'] * 1e3:.1f} us/iter | overlap {m['overlap_ms_per_iter'] * 1e3:.1f} | "
             f"time_ratio_same {m['time_ratio_same']:.3f} best {m['time_ratio_best']:.3f} | {gem} | "
