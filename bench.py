@@ -819,6 +819,8 @@ def _occ_from_args(args):
         occ["smem_reserve_bytes"] = args.smem_reserve_kib << 10
     if args.tile_k:
         occ["tile_k"] = args.tile_k
+    if args.static_order:
+        occ["tile_order"] = 1
     return occ
 
 
@@ -969,6 +971,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--ref-budget-s", type=float, default=90.0, help="--impl reference: CPU seconds for warmup + steps")
     ap.add_argument("--table", default="", help="write the sweep table (JSON; --mode power-table: markdown) here")
+    ap.add_argument("--static-order", action="store_true", help="--mode gemm-only: occ.tile_order = 1 (static tile assignment)")
     ap.add_argument("--tile-k", type=int, default=0, help="--mode gemm-only: occ.tile_k (32 or 64)")
     ap.add_argument("--mode", default="bench", choices=["bench", "gemm-only", "power-table", "tile-k-table"],
                     help="gemm-only / power-table: diagnostics behind profiles/ (one GPU, not the bench contract)")

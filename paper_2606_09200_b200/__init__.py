@@ -43,7 +43,7 @@ class RaError(RuntimeError):
 class Occupancy(Structure):
     _fields_ = [("smem_reserve_bytes", c_int32), ("sm_budget", c_int32), ("tiles_per_cta", c_int32),
                 ("allow_clamp", c_int32), ("cta_group", c_int32), ("m_blocks", c_int32), ("cluster_k", c_int32),
-                ("l2_persist_bytes", c_int32), ("tile_k", c_int32)]
+                ("l2_persist_bytes", c_int32), ("tile_k", c_int32), ("tile_order", c_int32)]
 
 
 class IpcHandle(Structure):
@@ -193,7 +193,7 @@ def _occ(occ) -> Occupancy | None:
     return Occupancy(int(occ.get("smem_reserve_bytes", 0)), int(occ.get("sm_budget", 0)),
                      int(occ.get("tiles_per_cta", 0)), int(occ.get("allow_clamp", 1)), int(occ.get("cta_group", 0)),
                      int(occ.get("m_blocks", 0)), int(occ.get("cluster_k", 0)), int(occ.get("l2_persist_bytes", 0)),
-                     int(occ.get("tile_k", 0)))
+                     int(occ.get("tile_k", 0)), int(occ.get("tile_order", 0)))
 
 
 def _occ_ref(occ):
@@ -427,7 +427,7 @@ def cfg_to_kw(c: OverlapCfg) -> dict:
     """OverlapCfg -> the keyword form make_cfg takes (for logging / re-creating a setting)."""
     return dict(mode=c.mode, occ=dict(smem_reserve_bytes=c.occ.smem_reserve_bytes, sm_budget=c.occ.sm_budget,
                                       tiles_per_cta=c.occ.tiles_per_cta, cta_group=c.occ.cta_group, m_blocks=c.occ.m_blocks,
-                                      cluster_k=c.occ.cluster_k, l2_persist_bytes=c.occ.l2_persist_bytes, tile_k=c.occ.tile_k),
+                                      cluster_k=c.occ.cluster_k, l2_persist_bytes=c.occ.l2_persist_bytes, tile_k=c.occ.tile_k, tile_order=c.occ.tile_order),
                 coll_sm_budget=c.coll_sm_budget, coll_smem_bytes=c.coll_smem_bytes, coll_ctas_per_sm=c.coll_ctas_per_sm,
                 coll_variant=c.coll_variant, prio_compute=c.prio_compute, prio_comm=c.prio_comm, dependent=c.dependent,
                 use_graph=c.use_graph)

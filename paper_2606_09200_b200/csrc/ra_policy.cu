@@ -65,7 +65,7 @@ ra_status ra_overlap_suggest(const ra_workload* w, const ra_peaks* peaks, ra_sug
 
     ra_suggestion s{};
     s.cfg.mode = RA_MODE_OVERLAP;
-    s.cfg.occ = {0, 0, 0, 1, 0, 0, 0, 0, 0};
+    s.cfg.occ = {0, 0, 0, 1, 0, 0, 0, 0, 0, 0};
     s.cfg.dependent = 1;
     s.cfg.prio_compute = 0;
     s.cfg.prio_comm = 0;                                  // priority off (persistent GEMM, see header)

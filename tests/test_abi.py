@@ -38,10 +38,10 @@ def test_status_strings(ra):
 
 def test_struct_layouts_match_header(ra):
     # sizes computed by hand from include/ra.h (LP64)
-    assert ctypes.sizeof(ra.Occupancy) == 36
+    assert ctypes.sizeof(ra.Occupancy) == 40
     assert ctypes.sizeof(ra.GemmPlan) == 72
     assert ctypes.sizeof(ra.Workload) == 160
-    assert ctypes.sizeof(ra.OverlapCfg) == 4 + 36 + 9 * 4
+    assert ctypes.sizeof(ra.OverlapCfg) == 4 + 40 + 9 * 4
     assert ctypes.sizeof(ra.OverlapResult) == 24 + 72 + 8
     assert ctypes.sizeof(ra.HostIO) == 7 * 8
 
@@ -325,7 +325,7 @@ def test_header_is_plain_c_and_links_from_c(ra, tmp_path):
     src.write_text(
         '#include "ra.h"\n#include <stdio.h>\n'
         "int main(void) {\n"
-        "  ra_gemm_plan p; ra_occupancy o = {0, 0, 0, 1, 0, 0, 0, 0, 0};\n"
+        "  ra_gemm_plan p; ra_occupancy o = {0, 0, 0, 1, 0, 0, 0, 0, 0, 0};\n"
         "  if (ra_gemm_plan_query(0, 1, 8192, 8192, 8192, &o, &p) != RA_OK) return 1;\n"
         '  printf("%d %d %d %s\\n", p.tile_m, p.tile_n, p.grid, ra_status_str(RA_ERR_ARCH));\n'
         "  return ra_gemm_plan_query(0, 1, 8, 8, 8, &o, (ra_gemm_plan*)0) == RA_ERR_INVALID_ARG ? 0 : 2;\n"

@@ -524,3 +524,49 @@ def test_tile_k_32_is_clamped_where_it_cannot_apply(ra):
         ra.ra_gemm_plan_query(1, 1, 1024, 1024, 1024, dict(tile_k=32, allow_clamp=0))
     with pytest.raises(ra.RaError):
         ra.ra_gemm_plan_query(0, 1, 1024, 1024, 1024, dict(tile_k=48))
+
+
+@pytest.mark.parametrize("M,N,K,occ", [
+    (4096, 4096, 2048, {}),                                    # 128 big tiles over 74 CTA pairs
+    (4096, 4096, 1024, dict(sm_budget=20)),                    # 13 tiles per pair: many claims per worker, ring wraps
+    (2048, 3000, 512, dict(cta_group=1, cluster_k=1, sm_budget=16)),   # single-CTA tiles, ragged N
+    (3000, 1000, 96, dict(cta_group=2, m_blocks=1, sm_budget=8)),      # 2 k-blocks per tile: the claim happens on the first one
+    (1536, 1536, 64, dict(cta_group=2, m_blocks=1, sm_budget=4)),      # ONE k-block per tile
+])
+def test_dynamic_tile_order_same_bits_as_static(ra, M, N, K, occ):
+    """occ.tile_order (ra.h): which worker computes a tile must not change one bit of it.  Dynamic (default) and static runs
+    are compared byte for byte, the dynamic one twice (its assignment differs from run to run), and against the oracle."""
+    plan = ra.ra_gemm_plan_query(0, 1, M, N, K, occ)
+    assert plan["split_k"] == 1 and plan["cluster_k"] == 1 and plan["n_tiles"] > plan["grid"] // plan["cta_group"], plan
+    A = ra_inputs.normal_bf16((M, K), 95, ra_inputs.STREAM_A)
+    B = ra_inputs.normal_bf16((N, K), 95, ra_inputs.STREAM_B)
+    stat, _ = run_gemm(ra, M, N, K, A, B, occ=dict(occ, tile_order=1))
+    dyn1, _ = run_gemm(ra, M, N, K, A, B, occ=occ)
+    dyn2, _ = run_gemm(ra, M, N, K, A, B, occ=dict(occ, tile_order=0))
+    assert dyn1.tobytes() == stat.tobytes() and dyn2.tobytes() == stat.tobytes()
+    ref, _ = oracle.gemm(0, 1, M, N, K, 1.0, A, B)
+    rowA, colB = oracle.gemm_norms(0, 1, M, N, K, A, B)
+    assert gemm_norm_err(dyn1, ref, rowA, colB) <= GEMM_TOL
+
+
+def test_dynamic_tile_order_back_to_back_and_concurrent_streams(ra):
+    """The claim counter and the ring live in a per-launch-cache-entry slot that a memset re-arms before every launch:
+    50 launches back to back on one stream, and two different GEMMs on two streams at once, all exact on integer operands."""
+    import torch
+    M, N, K = 2048, 2048, 512
+    occ = dict(sm_budget=12)
+    Ai = ra_inputs.smallint_bf16((M, K), 96, ra_inputs.STREAM_A)
+    Bi = ra_inputs.smallint_bf16((N, K), 96, ra_inputs.STREAM_B)
+    _, ref16 = oracle.gemm(0, 1, M, N, K, 1.0, Ai, Bi)
+    dA, dB = to_dev(Ai), to_dev(Bi)
+    c1 = torch.zeros((M, N), dtype=torch.int16, device="cuda")
+    c2 = torch.zeros((M, N), dtype=torch.int16, device="cuda")
+    ws = torch.empty(16, dtype=torch.uint8, device="cuda")
+    s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+    for i in range(50):
+        ra.ra_gemm(0, 1, M, N, K, 1.0, dA, K, dB, K, 0.0, c1, N, occ=occ, workspace=ws, stream=s1)
+        if i % 5 == 0:
+            ra.ra_gemm(0, 1, M, N, K, 1.0, dA, K, dB, K, 0.0, c2, N, occ=dict(sm_budget=20), workspace=ws, stream=s2)
+    torch.cuda.synchronize()
+    assert to_host(c1, np.uint16).reshape(M, N).tobytes() == ref16.tobytes()
+    assert to_host(c2, np.uint16).reshape(M, N).tobytes() == ref16.tobytes()
