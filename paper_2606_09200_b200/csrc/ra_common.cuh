@@ -123,15 +123,19 @@ __device__ __forceinline__ bool mbar_try_wait(uint32_t bar, uint32_t parity) {
     return ok != 0;
 }
 // Bounded wait: a protocol bug (wrong phase, lost arrive) must surface as a trapped launch
-// (cudaErrorLaunchFailure -> RA_ERR_CUDA), never as a hung GPU.  The clock is only read on the
-// slow path (after a failed probe, i.e. at most once per suspend period), so the common case costs nothing.
+// (cudaErrorLaunchFailure -> RA_ERR_CUDA), never as a hung GPU.  A suspended waiter is woken by every mbarrier event of
+// its CTA (ncu: the epilogue warps re-probe ~7 k times per kernel), so the loop body is kept to the probe itself and the
+// clock is read once per 256 failed probes.
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
     if (mbar_try_wait(bar, parity)) return;
     uint64_t t0 = 0;
+    uint32_t spins = 0;
     while (!mbar_try_wait(bar, parity)) {
-        const uint64_t now = globaltimer();
-        if (t0 == 0) t0 = now;
-        else if (now - t0 > 5000000000ull) __trap();   // 5 s
+        if ((++spins & 255u) == 0) {
+            const uint64_t now = globaltimer();
+            if (t0 == 0) t0 = now;
+            else if (now - t0 > 5000000000ull) __trap();   // 5 s
+        }
     }
 }
 
