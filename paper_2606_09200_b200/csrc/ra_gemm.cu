@@ -29,9 +29,13 @@
 //              MMAs of the other at both ends of a tile (large problems; the tile cuBLAS uses too)
 //
 // Scheduling (S3: occupancy shaping).  grid = sm_budget persistent CTAs, one
-// per SM; pipeline depth (and, when squeezed, the tile) follows from smem_reserve_bytes.  Work
-// decompositions, all static (no atomics in the schedule):
-//   data-parallel   worker c owns tiles c, c+G, c+2G, ... (grouped rasterisation for L2 reuse)
+// per SM; pipeline depth (and, when squeezed, the tile) follows from smem_reserve_bytes; tile_k = 32 halves the
+// stages; l2_persist_bytes keeps one raster group's X panel in a persisting L2 carve-out.  Work
+// decompositions (no floating-point atomics anywhere; integer atomics only hand out work):
+//   data-parallel   grouped rasterisation for L2 reuse.  Multi-wave persistent plans hand tiles out DYNAMICALLY (next unclaimed
+//                   tile of the raster, one integer atomic per tile: see g_dyn) so that workers which finish together run
+//                   neighbouring tiles in step and their loads coalesce in L2; otherwise worker c owns tiles c, c+G, c+2G, ...
+//                   Either way one worker accumulates a C element in ascending k: the assignment never changes a result.
 //   cluster split-K a 2-CTA cluster takes one tile's k-blocks half each; CTA 1 hands its accumulator to CTA 0
 //                   through distributed shared memory (no workspace; low + high half, fixed order)
 //   stream-K        the n_tiles*KB k-block units are cut into G equal contiguous ranges; a tile
