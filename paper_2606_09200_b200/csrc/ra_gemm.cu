@@ -86,8 +86,8 @@ struct GemmParams {
     int hintC;         // L2 policy of the TMA stores of C (written once, never re-read by this kernel)
     int group_x;       // rasterisation: X-tiles per group
     int dyn;           // 1: dynamic tile order (data-parallel multi-wave plans): a worker's next tile is the next unclaimed one
-    unsigned long long* dyn_ring;   // [workers][kDynRing] tagged entries (step << 32 | tile), written by the worker's scheduler thread
-    unsigned int* dyn_ctr;          // tiles claimed beyond the first `workers`
+    unsigned long long* dyn_ring;   // [workers][kDynRing] tagged entries ((generation << 12 | step) << 32 | tile), written by the worker's scheduler thread
+    unsigned int* dyn_ctr;          // [0] tiles claimed beyond the first `workers`, [1] CTAs that left the kernel, [2] generation
     int xmn, ymn;      // operand storage: 0 = K-contiguous rows (K-major), 1 = row index contiguous (MN-major)
     int epi_tma;       // 1: whole tiles leave through shared memory + TMA stores (non-swapped C only)
     int skew;          // XH == 2: k-blocks by which X block 0 leads block 1 at both ends of a tile (<= stages)
@@ -109,8 +109,12 @@ __device__ int g_gemm_max_resident;
 // coalescer together and are served by one slice read.  A static assignment (worker w owns tiles w, w + W, ...) keeps handing
 // adjacent tiles to workers that drifted apart waves ago: ncu on 8192^3 shows 1.07 GPC deliveries per L2-slice read with
 // the static order (1.25 in a one-wave problem, where everybody starts together) against cuBLAS's 1.37.
-// One launch slot per launch-cache entry: [kDynWorkers][kDynRing] ring entries + a counter, zeroed by a memset node before
-// the kernel.  The ring needs no acknowledgements: the scheduler thread (the TMA producer) is never more than `stages`
+// One launch slot per launch-cache entry: [kDynWorkers][kDynRing] ring entries + {claim counter, exit counter, generation}.
+// The slot re-arms ITSELF: ring tags carry the slot's generation, and the last CTA to leave the kernel zeroes the two
+// counters and bumps the generation, so the next launch finds a clean slot without a memset node in front of it.  (A
+// memset node was tried first and cost the overlapped step 6 %: it delays K_g^(i+1) by a few microseconds, the waiting
+// collective K_c^i takes the SMs first, and an SM that runs shared-memory-free CTAs has to drain before it can give a
+// GEMM CTA its 225 KiB carve-out -- the two kernels serialised.)  The ring needs no acknowledgements: the scheduler thread (the TMA producer) is never more than `stages`
 // (<= kMaxStages = 8) k-blocks -- hence at most 8 tiles, when a tile is a single k-block -- ahead of the MMA issuer, which is
 // never more than two tiles (two accumulators) ahead of the epilogue, and it publishes one step ahead: 11 steps of history
 // at most, so kDynRing = 16 cannot be overrun.
@@ -118,7 +122,8 @@ constexpr int kDynWorkers = 160;
 constexpr int kDynRing = 16;
 static_assert(kDynRing >= kMaxStages + 4 && (kDynRing & (kDynRing - 1)) == 0, "ring depth");
 constexpr int kDynSlots = 32;
-constexpr int kDynSlotWords = kDynWorkers * kDynRing + 8;     // u64 words per slot; the counter lives in word kDynWorkers * kDynRing
+constexpr int kDynSlotWords = kDynWorkers * kDynRing + 8;     // u64 words per slot; u32 {claims, exits, generation} start at word kDynWorkers * kDynRing
+constexpr int kDynMaxSteps = 4000;                            // steps per worker that fit the tag's 12-bit step field
 __device__ unsigned long long g_dyn[kDynSlots * kDynSlotWords];
 
 // ---- device helpers ---------------------------------------------------------------------------
@@ -345,8 +350,10 @@ struct Sched {
     int krank;              // cluster split-K: which half of a tile's k-blocks this CTA takes (else 0)
     int role;               // dynamic order: 0 = this worker's scheduler thread, 1 = a single consumer thread, 2 = a consumer warp
     int pending;            // scheduler: the tile claimed for the next step
+    unsigned gen;           // dynamic order: the slot's generation during this launch (constant until the last CTA leaves)
     __device__ Sched(const GemmParams& p_, int wid_, int nw_, int krank_ = 0, int role_ = 1)
-        : p(p_), it(0), wid(wid_), nw(nw_), krank(krank_), role(role_), pending(-1) {
+        : p(p_), it(0), wid(wid_), nw(nw_), krank(krank_), role(role_), pending(-1), gen(0) {
+        if (p.dyn) asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(gen) : "l"(p.dyn_ctr + 2) : "memory");
         if (p.stream_k) {
             const long long U = (long long)p.n_tiles * p.kb_per_tile;
             u0 = (long long)wid * U / nw;
@@ -379,7 +386,7 @@ struct Sched {
                     uint64_t t0 = 0;
                     for (;;) {
                         asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(e) : "memory");
-                        if ((unsigned)(v >> 32) == (unsigned)it) break;
+                        if ((unsigned)(v >> 32) == ((gen << 12) | (unsigned)it)) break;
                         __nanosleep(64);
                         const uint64_t now = globaltimer();
                         if (t0 == 0) t0 = now;
@@ -408,7 +415,7 @@ struct Sched {
         const unsigned c = atomicAdd(p.dyn_ctr, 1u);
         const long long t = (long long)nw + (long long)c;
         pending = t < (long long)p.n_tiles ? (int)t : p.n_tiles;
-        const unsigned long long v = ((unsigned long long)(unsigned)it << 32) | (unsigned)pending;
+        const unsigned long long v = ((unsigned long long)((gen << 12) | (unsigned)it) << 32) | (unsigned)pending;
         unsigned long long* e = p.dyn_ring + (size_t)wid * kDynRing + (it & (kDynRing - 1));
         asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" ::"l"(e), "l"(v) : "memory");
     }
@@ -1026,6 +1033,17 @@ gemm_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constant__ CU
             asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"((uint32_t)kTmemCols) : "memory");
     }
     if (threadIdx.x == 64) atomicSub(&g_gemm_resident[my_sm], 1);
+    if (p.dyn && threadIdx.x == 32) {
+        // the last CTA to get here re-arms the slot for the next launch (every thread of every CTA is past its schedule)
+        __threadfence();
+        if (atomicAdd(p.dyn_ctr + 1, 1u) == gridDim.x - 1) {
+            const unsigned g = *(volatile unsigned*)(p.dyn_ctr + 2);
+            p.dyn_ctr[0] = 0u;
+            p.dyn_ctr[1] = 0u;
+            __threadfence();
+            *(volatile unsigned*)(p.dyn_ctr + 2) = (g + 1u) & 0xFFFFFu;
+        }
+    }
     if (threadIdx.x == 0) trace_end(rec);
 }
 
@@ -1544,7 +1562,7 @@ static ra_status build_entry(const LaunchKey& k, const DeviceInfo& di, LaunchEnt
         // dynamic tile order: persistent data-parallel plans with more tiles than workers (see g_dyn)
         const int workers = pl.pub.grid / (cg * pl.pub.cluster_k);
         p.dyn = (k.occ.tile_order != 1 && !p.stream_k && pl.pub.cluster_k == 1 && k.occ.tiles_per_cta == 0 && p.n_tiles > workers &&
-                 workers <= kDynWorkers) ? 1 : 0;
+                 workers <= kDynWorkers && p.n_tiles < kDynMaxSteps) ? 1 : 0;
     }
     const void* X = swap ? k.B : k.A;
     const void* Y = swap ? k.A : k.B;
@@ -1670,7 +1688,6 @@ ra_status gemm_launch(int transA, int transB, int M, int N, int K, float alpha, 
         unsigned long long* slot = static_cast<unsigned long long*>(base) + (size_t)dyn_slot * kDynSlotWords;
         p.dyn_ring = slot;
         p.dyn_ctr = reinterpret_cast<unsigned int*>(slot + kDynWorkers * kDynRing);
-        RA_CUDA(cudaMemsetAsync(slot, 0, (size_t)kDynSlotWords * sizeof(unsigned long long), stream));
     }
     if (p.stream_k) {
         p.counters = static_cast<int*>(workspace);
