@@ -581,9 +581,24 @@ def measure_config(ra, cfg, args, peaks, world, dev, headline: bool):
     runs = args.sweep_runs if sweep != "config5" else max(6, args.sweep_runs - 3)
     results, best = ra.ra_overlap_sweep(w, [ra.make_cfg(**kw) for kw in cand_kws], runs=runs)
     sweep_argmin = best
-    # S7 picks the argmin; settings closer than the run-to-run spread of a power-capped step (1-2 %, profiles/r02_l2_persist.md 3)
-    # are a tie (2.5 %), and a tie goes to the policy's setting (index 2) so that the timed setting is not chosen by noise
-    if sweep != "none" and results[2]["total_ms"] <= 1.025 * results[best]["total_ms"]:
+    # Final: the sweep's three fastest overlap settings and the policy's pick (index 2) are timed again with the paper's own
+    # protocol -- 30 runs each, the first third warm-up -- because the minimum over ~50 settings of a noisy
+    # quantity (a power-capped step wanders by 2-3 % over tenths of a second) is biased low.  Argmin of the final; settings
+    # within 2.5 % of the policy's are a tie and the tie goes to the policy, so that the timed setting is not chosen by noise.
+    final = None
+    if sweep != "none" and len(cand_kws) > 4:
+        order = sorted((i for i, kw in enumerate(cand_kws) if kw["mode"] == 1), key=lambda i: results[i]["total_ms"])
+        finalists = list(dict.fromkeys(order[:3] + [2]))
+        fres, fbest = ra.ra_overlap_sweep(w, [ra.make_cfg(**cand_kws[i]) for i in finalists], runs=30)
+        best = finalists[fbest]
+        pol_ms = fres[finalists.index(2)]["total_ms"]
+        if pol_ms <= 1.025 * fres[fbest]["total_ms"]:
+            best = 2
+        final = {"settings": [cfg_label(cand_kws[i]) for i in finalists], "ms_per_iter": [r["total_ms"] / n_iters for r in fres],
+                 "runs": 30, "picked": finalists.index(best)}
+        for i, r in zip(finalists, fres):
+            results[i] = dict(results[i], total_ms=r["total_ms"], median_ms=r["median_ms"], min_ms=r["min_ms"])
+    elif sweep != "none" and results[2]["total_ms"] <= 1.025 * results[best]["total_ms"]:
         best = 2
     best_kw = cand_kws[best]
     sweep_serial_ms = results[0]["total_ms"] / n_iters
@@ -600,7 +615,8 @@ def measure_config(ra, cfg, args, peaks, world, dev, headline: bool):
             norm_time = on / off
     policy = {"setting": cfg_label(sug["kw"]), "predicted_ms_per_iter": sug["t_overlap_ms"], "measured_ms_per_iter": results[2]["total_ms"] / n_iters,
               "sweep_best_ms_per_iter": results[sweep_argmin]["total_ms"] / n_iters, "sweep_argmin_setting": cfg_label(cand_kws[sweep_argmin]),
-              "regret": results[2]["total_ms"] / results[sweep_argmin]["total_ms"] - 1.0, "timed_setting_is": "policy (tie within 2.5 %)" if best == 2 and sweep_argmin != 2 else "sweep argmin", "gemm_bound": sug["gemm_bound"],
+              "regret": results[2]["total_ms"] / results[best]["total_ms"] - 1.0, "final": final,
+              "timed_setting_is": "policy (tie within 2.5 %)" if best == 2 and sweep_argmin != 2 else ("policy" if best == 2 else "sweep final argmin"), "gemm_bound": sug["gemm_bound"],
               "model_roofline_ms": sug["t_roofline_ms"], "settings_in_sweep": len(cand_kws) - 1}
     alone = kernels_alone(ra, cfg, d, peaks, n_iters, graph=graph)
     residency = residency_map(ra, w, best_kw, info["sm_count"]) if headline else None
