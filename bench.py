@@ -315,7 +315,7 @@ def kernels_alone(ra, cfg, d, peaks, n_iters, graph: int = 0):
     out["gemm_gbs"] = cfg.gemm_bytes / g_ms / 1e6
     out["gemm_frac_of_hbm_peak"] = out["gemm_gbs"] / peaks["hbm_gbs"]
     out["gemm_plan"] = res[0]["plan"]
-    if cfg.M > 128 and cfg.M * cfg.N >= 1 << 22:
+    if cfg.M * cfg.N >= 1 << 20:
         out["library_gemm_same_box"] = library_gemm_same_box(cfg, d, n_iters)
     w, keep = make_workload(ra, cfg, d, n_iters, gemm=False)
     # the collective alone is a bandwidth measurement: let the clocks recover from the power-capped GEMM runs first
@@ -727,7 +727,8 @@ def flat_summary(m, peaks):
            f"{a['gemm_tflops']:.0f} sustained={a['gemm_frac_of_bf16_peak_sustained']:.3f}"
            + (f" (cuBLAS same box {a['library_gemm_same_box']['burst_tflops']:.0f} / {a['library_gemm_same_box']['sustained_tflops']:.0f})"
               if "library_gemm_same_box" in a else "") if m["compute_bound"] else
-           f"gemm alone {a['gemm_gbs']:.0f} GB/s={a['gemm_frac_of_hbm_peak']:.3f} of HBM peak ({a['gemm_tflops']:.0f} TF/s)")
+           f"gemm alone {a['gemm_gbs']:.0f} GB/s={a['gemm_frac_of_hbm_peak']:.3f} of HBM peak ({a['gemm_tflops']:.0f} TF/s"
+           + (f"; cuBLAS same box {a['library_gemm_same_box']['sustained_tflops']:.0f}" if "library_gemm_same_box" in a else "") + ")")
     return (f"serial {m['serial_ms_per_iter'] * 1e3:.1f} us/iter | overlap {m['overlap_ms_per_iter'] * 1e3:.1f} | "
             f"time_ratio_same {m['time_ratio_same']:.3f} best {m['time_ratio_best']:.3f} | {gem} | "
             f"coll alone {a['coll_gbs']:.0f} GB/s={a['coll_frac_of_hbm_peak']:.3f} of HBM peak | "

@@ -578,7 +578,7 @@ __device__ __forceinline__ void pack_out(const GemmParams& p, const uint32_t (&v
     }
 }
 
-template <int BN, int CG, int XH>
+template <int BN, int CG, int XH, int KBK>
 __global__ void __launch_bounds__(256, 2)
 gemm_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constant__ CUtensorMap mapY,
             const __grid_constant__ CUtensorMap mapC, const GemmParams p, Trace tr) {
@@ -592,26 +592,26 @@ gemm_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constant__ CU
     // what bounds the 256 x 256 pair tile (64 B/clk/SM).  The price: both accumulators belong to the current
     // tile, so the epilogue overlaps only the first k-blocks of the next tile (see the MMA issuer).
     constexpr int kYRows = BN / CG;
-    constexpr int kXHalfBytes = kBM * kBK * 2;
+    // KBK = k extent of one pipeline stage: 64 (128-byte swizzle rows) or 32 (64-byte rows; K-major operands only).  A template
+    // parameter, not a run-time one: as a run-time value it cost the weight-streaming GEMM 5 % (87.4 -> 92.0 us), whose
+    // producer thread has no slack for the extra address arithmetic per k-block.
+    static_assert(KBK == 64 || KBK == 32, "KBK");
+    constexpr int kXHalfBytes = kBM * KBK * 2;
     constexpr int kXBytes = XH * kXHalfBytes;
-    constexpr int kStageBytes = kXBytes + kYRows * kBK * 2;
+    constexpr int kStageBytes = kXBytes + kYRows * KBK * 2;
     constexpr int kTmemCols = 2 * BN;   // XH == 1: two accumulators (double buffer); XH == 2: the two X blocks of one tile
     constexpr int kTileX = kBM * XH * CG;
     constexpr uint32_t kIdesc = umma_idesc_bf16(kBM * CG, BN);
     static_assert(BN == 64 || BN == 128 || BN == 256, "BN");
     static_assert(CG == 1 || CG == 2, "CG");
     static_assert(XH == 1 || XH == 2, "XH");
-    static_assert(kStageBytes == stage_bytes(BN, CG, XH), "stage size");
-    // tile_k = 32 halves every piece of a stage (the constants above are the tile_k = 64 sizes)
-    const int bk_shift = (p.bk == 32) ? 1 : 0;
-    const uint32_t xhalf_bytes = (uint32_t)kXHalfBytes >> bk_shift, xbytes = (uint32_t)kXBytes >> bk_shift;
-    const uint32_t stage_sz = (uint32_t)kStageBytes >> bk_shift;
+    static_assert(kStageBytes == stage_bytes(BN, CG, XH) * KBK / kBK, "stage size");
 
     extern __shared__ uint8_t smem_raw[];
     // 1024-byte alignment for the 128B swizzle; the barrier block sits after the stages.  Both CTAs of a pair
     // compute identical offsets (same kernel, same dynamic-smem base), which cta_group::2 relies on.
     const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
-    const uint32_t epi_base = smem_base + p.stages * stage_sz;     // staging for TMA stores (epi_tma only)
+    const uint32_t epi_base = smem_base + p.stages * kStageBytes;     // staging for TMA stores (epi_tma only)
     const uint32_t bar_base = epi_base + (p.epi_tma ? kEpiStageBytes : 0);
     auto full_bar = [&](int s) { return bar_base + 8u * s; };
     auto empty_bar = [&](int s) { return bar_base + 8u * (kMaxStages + s); };
@@ -685,28 +685,28 @@ gemm_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constant__ CU
                 for (int kb = sg.kb0; kb < sg.kb1; ++kb) {
                     if (p.dyn && rank == 0 && kb == claim_at) sched.claim_next();
                     mbar_wait(empty_bar(stage), phase ^ 1u);           // local: MMAs reading this stage retired
-                    const uint32_t sx = smem_base + stage * stage_sz;
+                    const uint32_t sx = smem_base + stage * kStageBytes;
                     uint32_t bar;
                     if constexpr (CG == 1) {
                         bar = full_bar(stage);
-                        mbar_expect_tx(bar, stage_sz);
+                        mbar_expect_tx(bar, kStageBytes);
                     } else {
                         bar = mapa(full_bar(stage), lead);            // the leader's barrier collects both halves
-                        mbar_expect_tx_cluster(bar, stage_sz);
+                        mbar_expect_tx_cluster(bar, kStageBytes);
                     }
                     // K-major operand: one box (64 k x rows).  MN-major operand: one box (64 rows x 64 k) per 64 rows.
                     if (!p.xmn) {
-                        tma_load_2d<CG>(sx, &mapX, kb * p.bk, x0, bar, polX);
+                        tma_load_2d<CG>(sx, &mapX, kb * KBK, x0, bar, polX);
                     } else {
 #pragma unroll
                         for (int b = 0; b < kBM * XH / 64; ++b) tma_load_2d<CG>(sx + b * 8192, &mapX, x0 + 64 * b, kb * kBK, bar, polX);
                     }
                     if (!p.ymn) {
-                        tma_load_2d<CG>(sx + xbytes, &mapY, kb * p.bk, y0, bar, polY);
+                        tma_load_2d<CG>(sx + kXBytes, &mapY, kb * KBK, y0, bar, polY);
                     } else {
 #pragma unroll
                         for (int b = 0; b < kYRows / 64; ++b)
-                            tma_load_2d<CG>(sx + xbytes + b * 8192, &mapY, y0 + 64 * b, kb * kBK, bar, polY);
+                            tma_load_2d<CG>(sx + kXBytes + b * 8192, &mapY, y0 + 64 * b, kb * kBK, bar, polY);
                     }
                     if (++stage == p.stages) { stage = 0; phase ^= 1u; }
                 }
@@ -724,17 +724,17 @@ gemm_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constant__ CU
             const int kx_step = p.xmn ? (2048 >> 4) : (32 >> 4), ky_step = p.ymn ? (2048 >> 4) : (32 >> 4);
             // the four UMMA_K steps of X block h against the Y rows of one stage, into accumulator column acc_col
             auto issue_block = [&](int st, int h, uint32_t acc_col, bool first) {
-                const uint32_t sx = smem_base + st * stage_sz;
-                const uint32_t sxh = sx + h * xhalf_bytes;
-                if (bk_shift) {                    // tile_k = 32: two UMMA_K steps per stage, 64-byte swizzle (K-major operands only)
-                    const uint64_t dx = umma_desc_sw64(sxh), dy = umma_desc_sw64(sx + xbytes);
+                const uint32_t sx = smem_base + st * kStageBytes;
+                const uint32_t sxh = sx + h * kXHalfBytes;
+                if constexpr (KBK == 32) {         // two UMMA_K steps per stage, 64-byte swizzle (K-major operands only)
+                    const uint64_t dx = umma_desc_sw64(sxh), dy = umma_desc_sw64(sx + kXBytes);
 #pragma unroll
                     for (int k = 0; k < 2; ++k)
                         umma_bf16<CG>(tmem_base + acc_col, dx + (uint64_t)(2 * k), dy + (uint64_t)(2 * k), idesc, (!first || k > 0) ? 1u : 0u);
                     return;
                 }
                 const uint64_t dx = p.xmn ? umma_desc_sw128_mn(sxh) : umma_desc_sw128(sxh);
-                const uint64_t dy = p.ymn ? umma_desc_sw128_mn(sx + xbytes) : umma_desc_sw128(sx + xbytes);
+                const uint64_t dy = p.ymn ? umma_desc_sw128_mn(sx + kXBytes) : umma_desc_sw128(sx + kXBytes);
 #pragma unroll
                 for (int k = 0; k < kBK / kUmmaK; ++k) {
                     // per UMMA_K step: K-major +32 B inside the swizzle atom, MN-major +2 k-groups of 1024 B
@@ -1103,26 +1103,32 @@ static ra_status make_map(CUtensorMap* map, const void* base, int rows, int K, i
 }
 
 // ---- host: kernel instantiations, their one-time attributes, and what the hardware says about residency --------
-static const void* gemm_kernel_ptr(int bn, int cg, int xh) {
-    if (cg == 2 && xh == 2) return reinterpret_cast<const void*>(&gemm_kernel<256, 2, 2>);
-    if (cg == 2) return reinterpret_cast<const void*>(&gemm_kernel<256, 2, 1>);
+template <int KBK>
+static const void* gemm_kernel_ptr_k(int bn, int cg, int xh) {
+    if (cg == 2 && xh == 2) return reinterpret_cast<const void*>(&gemm_kernel<256, 2, 2, KBK>);
+    if (cg == 2) return reinterpret_cast<const void*>(&gemm_kernel<256, 2, 1, KBK>);
     switch (bn) {
-        case 64: return reinterpret_cast<const void*>(&gemm_kernel<64, 1, 1>);
-        case 128: return reinterpret_cast<const void*>(&gemm_kernel<128, 1, 1>);
-        case 256: return reinterpret_cast<const void*>(&gemm_kernel<256, 1, 1>);
+        case 64: return reinterpret_cast<const void*>(&gemm_kernel<64, 1, 1, KBK>);
+        case 128: return reinterpret_cast<const void*>(&gemm_kernel<128, 1, 1, KBK>);
+        case 256: return reinterpret_cast<const void*>(&gemm_kernel<256, 1, 1, KBK>);
     }
     return nullptr;
 }
-static int kernel_slot(int bn, int cg, int xh) { return cg == 2 ? (xh == 2 ? 4 : 3) : (bn == 64 ? 0 : (bn == 128 ? 1 : 2)); }
+static const void* gemm_kernel_ptr(int bn, int cg, int xh, int bk = kBK) {
+    return bk == 32 ? gemm_kernel_ptr_k<32>(bn, cg, xh) : gemm_kernel_ptr_k<64>(bn, cg, xh);
+}
+static int kernel_slot(int bn, int cg, int xh, int bk) {
+    return (bk == 32 ? 5 : 0) + (cg == 2 ? (xh == 2 ? 4 : 3) : (bn == 64 ? 0 : (bn == 128 ? 1 : 2)));
+}
 
 static std::mutex g_gemm_mu;                 // guards the attribute flags and the launch cache below
-static bool g_attr_set[64][5] = {};          // [device][instantiation]: MaxDynamicSharedMemorySize raised to the opt-in limit
+static bool g_attr_set[64][10] = {};          // [device][instantiation]: MaxDynamicSharedMemorySize raised to the opt-in limit
 
 // cudaFuncSetAttribute once per (device, instantiation), not once per launch.  Caller holds g_gemm_mu.
-static ra_status prepare_kernel(const DeviceInfo& di, int bn, int cg, int xh) {
-    const int slot = kernel_slot(bn, cg, xh);
+static ra_status prepare_kernel(const DeviceInfo& di, int bn, int cg, int xh, int bk) {
+    const int slot = kernel_slot(bn, cg, xh, bk);
     if (di.device >= 0 && di.device < 64 && g_attr_set[di.device][slot]) return RA_OK;
-    RA_CUDA(cudaFuncSetAttribute(gemm_kernel_ptr(bn, cg, xh), cudaFuncAttributeMaxDynamicSharedMemorySize, di.smem_per_block_optin));
+    RA_CUDA(cudaFuncSetAttribute(gemm_kernel_ptr(bn, cg, xh, bk), cudaFuncAttributeMaxDynamicSharedMemorySize, di.smem_per_block_optin));
     if (di.device >= 0 && di.device < 64) g_attr_set[di.device][slot] = true;
     return RA_OK;
 }
@@ -1477,12 +1483,12 @@ static ra_status make_plan(int transA, int transB, int M, int N, int K, const ra
     return RA_OK;
 }
 
-template <int BN, int CG, int XH>
+template <int BN, int CG, int XH, int KBK>
 static ra_status launch_gemm(const CUtensorMap& mx, const CUtensorMap& my, const CUtensorMap& mc, const GemmParams& p, int grid, int dyn,
                              cudaStream_t stream) {
     const int cluster = CG * p.ks;                      // CTA pair (tcgen05 cta_group::2) x split-K halves
     if (cluster == 1) {
-        gemm_kernel<BN, CG, XH><<<grid, kGemmThreads, dyn, stream>>>(mx, my, mc, p, g_trace);
+        gemm_kernel<BN, CG, XH, KBK><<<grid, kGemmThreads, dyn, stream>>>(mx, my, mc, p, g_trace);
         RA_CUDA(cudaGetLastError());
         return RA_OK;
     }
@@ -1498,7 +1504,7 @@ static ra_status launch_gemm(const CUtensorMap& mx, const CUtensorMap& my, const
     attr[0].val.clusterDim.z = 1;
     cfg.attrs = attr;
     cfg.numAttrs = 1;
-    RA_CUDA(cudaLaunchKernelEx(&cfg, gemm_kernel<BN, CG, XH>, mx, my, mc, p, g_trace));
+    RA_CUDA(cudaLaunchKernelEx(&cfg, gemm_kernel<BN, CG, XH, KBK>, mx, my, mc, p, g_trace));
     return RA_OK;
 }
 
@@ -1582,7 +1588,7 @@ static ra_status build_entry(const LaunchKey& k, const DeviceInfo& di, LaunchEnt
     e->p = p;
     {
         std::lock_guard<std::mutex> lk(g_gemm_mu);
-        RA_TRY(prepare_kernel(di, pl.bn, cg, xh));
+        RA_TRY(prepare_kernel(di, pl.bn, cg, xh, p.bk));
     }
     return RA_OK;
 }
@@ -1695,13 +1701,17 @@ ra_status gemm_launch(int transA, int transB, int M, int N, int K, float alpha, 
         RA_CUDA(cudaMemsetAsync(workspace, 0, pl.counters_bytes, stream));
     }
     const int cg = pl.pub.cta_group, xh = pl.pub.m_blocks;
-    if (cg == 2 && xh == 2) return launch_gemm<256, 2, 2>(mx, my, mc, p, pl.pub.grid, pl.pub.dyn_smem_bytes, stream);
-    if (cg == 2) return launch_gemm<256, 2, 1>(mx, my, mc, p, pl.pub.grid, pl.pub.dyn_smem_bytes, stream);
+#define RA_LAUNCH(BN_, CG_, XH_)                                                                                              \
+    return p.bk == 32 ? launch_gemm<BN_, CG_, XH_, 32>(mx, my, mc, p, pl.pub.grid, pl.pub.dyn_smem_bytes, stream)               \
+                      : launch_gemm<BN_, CG_, XH_, 64>(mx, my, mc, p, pl.pub.grid, pl.pub.dyn_smem_bytes, stream)
+    if (cg == 2 && xh == 2) RA_LAUNCH(256, 2, 2);
+    if (cg == 2) RA_LAUNCH(256, 2, 1);
     switch (pl.bn) {
-        case 64: return launch_gemm<64, 1, 1>(mx, my, mc, p, pl.pub.grid, pl.pub.dyn_smem_bytes, stream);
-        case 128: return launch_gemm<128, 1, 1>(mx, my, mc, p, pl.pub.grid, pl.pub.dyn_smem_bytes, stream);
-        case 256: return launch_gemm<256, 1, 1>(mx, my, mc, p, pl.pub.grid, pl.pub.dyn_smem_bytes, stream);
+        case 64: RA_LAUNCH(64, 1, 1);
+        case 128: RA_LAUNCH(128, 1, 1);
+        case 256: RA_LAUNCH(256, 1, 1);
     }
+#undef RA_LAUNCH
     return RA_ERR_UNSUPPORTED;
 }
 

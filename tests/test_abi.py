@@ -347,14 +347,30 @@ def test_planner_invariants_random(ra):
         smem_reserve_bytes=st.sampled_from([0, 0, 0, 32 * KB, 64 * KB, 96 * KB, 128 * KB, 160 * KB, 200 * KB]),
         sm_budget=st.sampled_from([0, 0, 0, 1, 2, 9, 33, 74, 92, 110, 128, 140, 148]),
         tiles_per_cta=st.sampled_from([0, 0, 0, 1, 2, 4]), cta_group=st.sampled_from([0, 0, 1, 2]),
-        m_blocks=st.sampled_from([0, 0, 1, 2]), cluster_k=st.sampled_from([0, 0, 1, 2, 4])))
+        m_blocks=st.sampled_from([0, 0, 1, 2]), cluster_k=st.sampled_from([0, 0, 1, 2, 4]),
+        l2_persist_bytes=st.sampled_from([0, 0, 0, 15 << 20, 47 << 20, 79 << 20]), tile_k=st.sampled_from([0, 0, 32, 64]),
+        tile_order=st.sampled_from([0, 0, 1])))
 
     @settings(max_examples=400, deadline=None)
     @given(dims, dims, dims, st.integers(0, 1), st.integers(0, 1), occs)
     def prop(M, N, K, tA, tB, occ):
         p = ra.ra_gemm_plan_query(tA, tB, M, N, K, occ)          # allow_clamp = 1: never refuses a valid shape
         budget = occ["sm_budget"] or 148
-        assert p["grid"] >= 1 and p["stages"] >= 1 and p["tile_k"] == 64
+        assert p["grid"] >= 1 and p["stages"] >= 1 and p["tile_k"] in (32, 64)
+        # tile_k = 32 only where asked for AND applicable (K-contiguous operands, no cluster split-K); never silently
+        assert (p["tile_k"] == 32) == (occ["tile_k"] == 32 and tA == 0 and tB == 1 and occ["cluster_k"] < 2), p
+        if occ["tile_k"] == 32 and p["tile_k"] == 64:
+            assert p["clamped"] == 1
+        # the raster and the L2 knob: groups are at least one tile row wide; the knob is reported only where it is used,
+        # and using it never changes the tile, the grid or the pipeline
+        assert 1 <= p["group_x"] <= max(1, -(-(N if p["swap_ab"] else M) // (p["tile_n"] if p["swap_ab"] else p["tile_m"])))
+        assert p["l2_persist_bytes"] in (0, occ["l2_persist_bytes"])
+        if occ["l2_persist_bytes"]:
+            q = ra.ra_gemm_plan_query(tA, tB, M, N, K, dict(occ, l2_persist_bytes=0))
+            assert {k: v for k, v in p.items() if k not in ("group_x", "l2_persist_bytes")} == \
+                   {k: v for k, v in q.items() if k not in ("group_x", "l2_persist_bytes")}
+        # tile_order is a run-time choice: it never changes the plan
+        assert ra.ra_gemm_plan_query(tA, tB, M, N, K, dict(occ, tile_order=1 - occ["tile_order"])) == p
         assert p["dyn_smem_bytes"] <= 227 * KB
         assert p["clamped"] or p["smem_left_per_sm"] >= occ["smem_reserve_bytes"], p
         assert p["n_tiles"] == -(-M // p["tile_m"]) * -(-N // p["tile_n"]), p
@@ -394,3 +410,6 @@ def test_l2_persist_plan(ra):
     assert ra.ra_gemm_plan_query(0, 1, 2048, 2048, 2048, dict(l2_persist_bytes=79 << 20))["l2_persist_bytes"] == 0
     with pytest.raises(ra.RaError):
         ra.ra_gemm_plan_query(0, 1, 8192, 8192, 8192, dict(l2_persist_bytes=-1))
+    for bad in (dict(tile_order=2), dict(tile_order=-1), dict(tile_k=16)):
+        with pytest.raises(ra.RaError):
+            ra.ra_gemm_plan_query(0, 1, 8192, 8192, 8192, bad)
