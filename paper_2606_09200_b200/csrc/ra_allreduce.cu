@@ -37,9 +37,11 @@ __device__ __forceinline__ void st_stream(float4* p, float4 v) {
                  : "memory");
 }
 
-template <int P>
+// ALL = true: the sum goes back to every rank buffer.  ALL = false (variant 2): to buffer 0 only, the copy engines fan it
+// out afterwards.  A template parameter: as a run-time store predicate it cost the all-buffers kernel 4 % (171 -> 178 us).
+template <int P, bool ALL>
 __global__ void __launch_bounds__(kArThreads, kArCtasPerSm)
-allreduce_kernel(const __grid_constant__ ArPtrs ptrs, size_t count, int n_write, Trace tr) {
+allreduce_kernel(const __grid_constant__ ArPtrs ptrs, size_t count, Trace tr) {
     uint64_t* rec = (threadIdx.x == 0) ? trace_begin(tr, KID_ALLREDUCE) : nullptr;
 
     const size_t nvec = count >> 2;
@@ -68,11 +70,8 @@ allreduce_kernel(const __grid_constant__ ArPtrs ptrs, size_t count, int n_write,
                 }
             }
         }
-        // n_write = P: the sum goes back to every rank buffer; n_write = 1 (variant 2): to buffer 0 only, the copy
-        // engines fan it out afterwards
 #pragma unroll
-        for (int r = 0; r < P; ++r)
-            if (r < n_write) st_stream(reinterpret_cast<float4*>(ptrs.p[r]) + v, s);
+        for (int r = 0; r < (ALL ? P : 1); ++r) st_stream(reinterpret_cast<float4*>(ptrs.p[r]) + v, s);
     }
     // ragged tail: count % 4 scalars
     if (blockIdx.x == 0) {
@@ -82,8 +81,7 @@ allreduce_kernel(const __grid_constant__ ArPtrs ptrs, size_t count, int n_write,
 #pragma unroll
             for (int r = 1; r < P; ++r) s = __fadd_rn(s, ptrs.p[r][e]);
 #pragma unroll
-            for (int r = 0; r < P; ++r)
-                if (r < n_write) ptrs.p[r][e] = s;
+            for (int r = 0; r < (ALL ? P : 1); ++r) ptrs.p[r][e] = s;
         }
     }
     if (threadIdx.x == 0) trace_end(rec);
@@ -196,8 +194,9 @@ allreduce_tma_kernel(const __grid_constant__ ArTmaParams p, Trace tr) {
 }
 
 template <int P>
-static cudaError_t launch_ar(const ArPtrs& ptrs, size_t count, int n_write, int grid, cudaStream_t stream) {
-    allreduce_kernel<P><<<grid, kArThreads, 0, stream>>>(ptrs, count, n_write, g_trace);
+static cudaError_t launch_ar(const ArPtrs& ptrs, size_t count, bool all, int grid, cudaStream_t stream) {
+    if (all) allreduce_kernel<P, true><<<grid, kArThreads, 0, stream>>>(ptrs, count, g_trace);
+    else allreduce_kernel<P, false><<<grid, kArThreads, 0, stream>>>(ptrs, count, g_trace);
     return cudaGetLastError();
 }
 
@@ -269,7 +268,7 @@ ra_status allreduce_launch(float* const* bufs, int P, size_t count, int sm_budge
 
     cudaError_t e;
     switch (P) {
-#define RA_AR_CASE(n) case n: e = launch_ar<n>(ptrs, count, variant == 2 ? 1 : n, (int)grid, stream); break;
+#define RA_AR_CASE(n) case n: e = launch_ar<n>(ptrs, count, variant != 2, (int)grid, stream); break;
         RA_AR_CASE(1) RA_AR_CASE(2) RA_AR_CASE(3) RA_AR_CASE(4) RA_AR_CASE(5) RA_AR_CASE(6) RA_AR_CASE(7) RA_AR_CASE(8)
         RA_AR_CASE(9) RA_AR_CASE(10) RA_AR_CASE(11) RA_AR_CASE(12) RA_AR_CASE(13) RA_AR_CASE(14) RA_AR_CASE(15)
         RA_AR_CASE(16)
