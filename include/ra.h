@@ -113,8 +113,8 @@ typedef struct {
                                  finish together start neighbouring tiles together and their loads of the shared operand
                                  rows coalesce in L2 (8192^3: 11 % fewer L2-slice reads, 2 % faster; profiles/r02_tile_order.md).
                                  1 = static: worker w owns tiles w, w + W, w + 2W, ...  Either way every C element is
-                                 accumulated in the same ascending-k order, so results are bit-identical.  Stream-K,
-                                 cluster split-K, bounded-work and single-wave plans are always static. */
+                                 accumulated in the same ascending-k order, so results are bit-identical.  Single-CTA tiles,
+                                 stream-K, cluster split-K, bounded-work and single-wave plans are always static. */
 } ra_occupancy;
 
 /* What S3 decided -- for tests, logs and the sweep tables. */

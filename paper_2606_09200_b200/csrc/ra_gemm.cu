@@ -342,6 +342,7 @@ struct Seg {
     int tile, kb0, kb1;
     long long start_unit;   // stream-K: first unit of this segment
 };
+template <bool DYN>
 struct Sched {
     const GemmParams& p;
     long long u0, u1, cur;  // stream-K unit range of this worker
@@ -353,7 +354,7 @@ struct Sched {
     unsigned gen;           // dynamic order: the slot's generation during this launch (constant until the last CTA leaves)
     __device__ Sched(const GemmParams& p_, int wid_, int nw_, int krank_ = 0, int role_ = 1)
         : p(p_), it(0), wid(wid_), nw(nw_), krank(krank_), role(role_), pending(-1), gen(0) {
-        if (p.dyn) asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(gen) : "l"(p.dyn_ctr + 2) : "memory");
+        if constexpr (DYN) asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(gen) : "l"(p.dyn_ctr + 2) : "memory");
         if (p.stream_k) {
             const long long U = (long long)p.n_tiles * p.kb_per_tile;
             u0 = (long long)wid * U / nw;
@@ -376,7 +377,7 @@ struct Sched {
             return true;
         }
         long long t = (long long)wid + (long long)it * nw;
-        if (p.dyn && it > 0) {
+        if constexpr (DYN) if (it > 0) {
             if (role == 0) {
                 t = pending;                   // claim_next() ran during the previous tile
             } else {
@@ -578,7 +579,9 @@ __device__ __forceinline__ void pack_out(const GemmParams& p, const uint32_t (&v
     }
 }
 
-template <int BN, int CG, int XH, int KBK>
+// DYN = dynamic tile order (see g_dyn).  A template parameter: compiled into every instantiation as a run-time branch it cost
+// the single-wave shapes, which never take it, 5-10 % (2048^3: 18.5 -> 20.5 us).  Instantiated for CTA-pair tiles only.
+template <int BN, int CG, int XH, int KBK, bool DYN>
 __global__ void __launch_bounds__(256, 2)
 gemm_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constant__ CUtensorMap mapY,
             const __grid_constant__ CUtensorMap mapC, const GemmParams p, Trace tr) {
@@ -672,7 +675,7 @@ gemm_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constant__ CU
         // ================= TMA producer (one per CTA) =================
         if (lane == 0) {
             const uint64_t polX = make_policy(p.hintX), polY = make_policy(p.hintY);
-            Sched sched(p, wid, nw, krank, rank == 0 ? 0 : 1);      // the pair leader's producer is the worker's scheduler thread
+            Sched<DYN> sched(p, wid, nw, krank, rank == 0 ? 0 : 1);      // the pair leader's producer is the worker's scheduler thread
             Seg sg;
             int stage = 0;
             uint32_t phase = 0;
@@ -683,7 +686,7 @@ gemm_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constant__ CU
                 const int y0 = ty * BN + (int)rank * kYRows;
                 const int claim_at = sg.kb0 + min(p.stages, sg.kb1 - sg.kb0 - 1);   // pipeline full: the claim's round trip is hidden
                 for (int kb = sg.kb0; kb < sg.kb1; ++kb) {
-                    if (p.dyn && rank == 0 && kb == claim_at) sched.claim_next();
+                    if constexpr (DYN) if (rank == 0 && kb == claim_at) sched.claim_next();
                     mbar_wait(empty_bar(stage), phase ^ 1u);           // local: MMAs reading this stage retired
                     const uint32_t sx = smem_base + stage * kStageBytes;
                     uint32_t bar;
@@ -715,7 +718,7 @@ gemm_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constant__ CU
     } else if (warp == 1) {
         // ================= MMA issuer (leader CTA only) =================
         if (lane == 0 && rank == 0) {
-            Sched sched(p, wid, nw, krank);
+            Sched<DYN> sched(p, wid, nw, krank);
             Seg sg;
             int stage = 0;
             uint32_t phase = 0;
@@ -806,7 +809,7 @@ gemm_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constant__ CU
         // residency count-in (after the set-up barrier, so the atomic's round trip delays nothing: this warp's next
         // action is the wait for the first accumulator)
         if (et == 0) atomicMax(&g_gemm_max_resident, atomicAdd(&g_gemm_resident[my_sm], 1) + 1);
-        Sched sched(p, wid, nw, krank, 2);
+        Sched<DYN> sched(p, wid, nw, krank, 2);
         Seg sg;
         int acc_it = 0;
         uint32_t sbuf_it = 0;                               // staging-buffer rotation (per warp)
@@ -1033,7 +1036,7 @@ gemm_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constant__ CU
             asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"((uint32_t)kTmemCols) : "memory");
     }
     if (threadIdx.x == 64) atomicSub(&g_gemm_resident[my_sm], 1);
-    if (p.dyn && threadIdx.x == 32) {
+    if constexpr (DYN) if (threadIdx.x == 32) {
         // the last CTA to get here re-arms the slot for the next launch (every thread of every CTA is past its schedule)
         __threadfence();
         if (atomicAdd(p.dyn_ctr + 1, 1u) == gridDim.x - 1) {
@@ -1104,31 +1107,31 @@ static ra_status make_map(CUtensorMap* map, const void* base, int rows, int K, i
 
 // ---- host: kernel instantiations, their one-time attributes, and what the hardware says about residency --------
 template <int KBK>
-static const void* gemm_kernel_ptr_k(int bn, int cg, int xh) {
-    if (cg == 2 && xh == 2) return reinterpret_cast<const void*>(&gemm_kernel<256, 2, 2, KBK>);
-    if (cg == 2) return reinterpret_cast<const void*>(&gemm_kernel<256, 2, 1, KBK>);
+static const void* gemm_kernel_ptr_k(int bn, int cg, int xh, int dyn) {
+    if (cg == 2 && xh == 2) return dyn ? reinterpret_cast<const void*>(&gemm_kernel<256, 2, 2, KBK, true>) : reinterpret_cast<const void*>(&gemm_kernel<256, 2, 2, KBK, false>);
+    if (cg == 2) return dyn ? reinterpret_cast<const void*>(&gemm_kernel<256, 2, 1, KBK, true>) : reinterpret_cast<const void*>(&gemm_kernel<256, 2, 1, KBK, false>);
     switch (bn) {
-        case 64: return reinterpret_cast<const void*>(&gemm_kernel<64, 1, 1, KBK>);
-        case 128: return reinterpret_cast<const void*>(&gemm_kernel<128, 1, 1, KBK>);
-        case 256: return reinterpret_cast<const void*>(&gemm_kernel<256, 1, 1, KBK>);
+        case 64: return reinterpret_cast<const void*>(&gemm_kernel<64, 1, 1, KBK, false>);
+        case 128: return reinterpret_cast<const void*>(&gemm_kernel<128, 1, 1, KBK, false>);
+        case 256: return reinterpret_cast<const void*>(&gemm_kernel<256, 1, 1, KBK, false>);
     }
     return nullptr;
 }
-static const void* gemm_kernel_ptr(int bn, int cg, int xh, int bk = kBK) {
-    return bk == 32 ? gemm_kernel_ptr_k<32>(bn, cg, xh) : gemm_kernel_ptr_k<64>(bn, cg, xh);
+static const void* gemm_kernel_ptr(int bn, int cg, int xh, int bk = kBK, int dyn = 0) {
+    return bk == 32 ? gemm_kernel_ptr_k<32>(bn, cg, xh, dyn) : gemm_kernel_ptr_k<64>(bn, cg, xh, dyn);
 }
-static int kernel_slot(int bn, int cg, int xh, int bk) {
-    return (bk == 32 ? 5 : 0) + (cg == 2 ? (xh == 2 ? 4 : 3) : (bn == 64 ? 0 : (bn == 128 ? 1 : 2)));
+static int kernel_slot(int bn, int cg, int xh, int bk, int dyn) {
+    return (dyn ? 10 : 0) + (bk == 32 ? 5 : 0) + (cg == 2 ? (xh == 2 ? 4 : 3) : (bn == 64 ? 0 : (bn == 128 ? 1 : 2)));
 }
 
 static std::mutex g_gemm_mu;                 // guards the attribute flags and the launch cache below
-static bool g_attr_set[64][10] = {};          // [device][instantiation]: MaxDynamicSharedMemorySize raised to the opt-in limit
+static bool g_attr_set[64][20] = {};          // [device][instantiation]: MaxDynamicSharedMemorySize raised to the opt-in limit
 
 // cudaFuncSetAttribute once per (device, instantiation), not once per launch.  Caller holds g_gemm_mu.
-static ra_status prepare_kernel(const DeviceInfo& di, int bn, int cg, int xh, int bk) {
-    const int slot = kernel_slot(bn, cg, xh, bk);
+static ra_status prepare_kernel(const DeviceInfo& di, int bn, int cg, int xh, int bk, int dyn) {
+    const int slot = kernel_slot(bn, cg, xh, bk, dyn);
     if (di.device >= 0 && di.device < 64 && g_attr_set[di.device][slot]) return RA_OK;
-    RA_CUDA(cudaFuncSetAttribute(gemm_kernel_ptr(bn, cg, xh, bk), cudaFuncAttributeMaxDynamicSharedMemorySize, di.smem_per_block_optin));
+    RA_CUDA(cudaFuncSetAttribute(gemm_kernel_ptr(bn, cg, xh, bk, dyn), cudaFuncAttributeMaxDynamicSharedMemorySize, di.smem_per_block_optin));
     if (di.device >= 0 && di.device < 64) g_attr_set[di.device][slot] = true;
     return RA_OK;
 }
@@ -1483,12 +1486,12 @@ static ra_status make_plan(int transA, int transB, int M, int N, int K, const ra
     return RA_OK;
 }
 
-template <int BN, int CG, int XH, int KBK>
+template <int BN, int CG, int XH, int KBK, bool DYN>
 static ra_status launch_gemm(const CUtensorMap& mx, const CUtensorMap& my, const CUtensorMap& mc, const GemmParams& p, int grid, int dyn,
                              cudaStream_t stream) {
     const int cluster = CG * p.ks;                      // CTA pair (tcgen05 cta_group::2) x split-K halves
     if (cluster == 1) {
-        gemm_kernel<BN, CG, XH, KBK><<<grid, kGemmThreads, dyn, stream>>>(mx, my, mc, p, g_trace);
+        gemm_kernel<BN, CG, XH, KBK, DYN><<<grid, kGemmThreads, dyn, stream>>>(mx, my, mc, p, g_trace);
         RA_CUDA(cudaGetLastError());
         return RA_OK;
     }
@@ -1504,7 +1507,7 @@ static ra_status launch_gemm(const CUtensorMap& mx, const CUtensorMap& my, const
     attr[0].val.clusterDim.z = 1;
     cfg.attrs = attr;
     cfg.numAttrs = 1;
-    RA_CUDA(cudaLaunchKernelEx(&cfg, gemm_kernel<BN, CG, XH, KBK>, mx, my, mc, p, g_trace));
+    RA_CUDA(cudaLaunchKernelEx(&cfg, gemm_kernel<BN, CG, XH, KBK, DYN>, mx, my, mc, p, g_trace));
     return RA_OK;
 }
 
@@ -1567,7 +1570,7 @@ static ra_status build_entry(const LaunchKey& k, const DeviceInfo& di, LaunchEnt
     {
         // dynamic tile order: persistent data-parallel plans with more tiles than workers (see g_dyn)
         const int workers = pl.pub.grid / (cg * pl.pub.cluster_k);
-        p.dyn = (k.occ.tile_order != 1 && !p.stream_k && pl.pub.cluster_k == 1 && k.occ.tiles_per_cta == 0 && p.n_tiles > workers &&
+        p.dyn = (cg == 2 && k.occ.tile_order != 1 && !p.stream_k && pl.pub.cluster_k == 1 && k.occ.tiles_per_cta == 0 && p.n_tiles > workers &&
                  workers <= kDynWorkers && p.n_tiles < kDynMaxSteps) ? 1 : 0;
     }
     const void* X = swap ? k.B : k.A;
@@ -1588,7 +1591,7 @@ static ra_status build_entry(const LaunchKey& k, const DeviceInfo& di, LaunchEnt
     e->p = p;
     {
         std::lock_guard<std::mutex> lk(g_gemm_mu);
-        RA_TRY(prepare_kernel(di, pl.bn, cg, xh, p.bk));
+        RA_TRY(prepare_kernel(di, pl.bn, cg, xh, p.bk, p.dyn));
     }
     return RA_OK;
 }
@@ -1701,15 +1704,21 @@ ra_status gemm_launch(int transA, int transB, int M, int N, int K, float alpha, 
         RA_CUDA(cudaMemsetAsync(workspace, 0, pl.counters_bytes, stream));
     }
     const int cg = pl.pub.cta_group, xh = pl.pub.m_blocks;
-#define RA_LAUNCH(BN_, CG_, XH_)                                                                                              \
-    return p.bk == 32 ? launch_gemm<BN_, CG_, XH_, 32>(mx, my, mc, p, pl.pub.grid, pl.pub.dyn_smem_bytes, stream)               \
-                      : launch_gemm<BN_, CG_, XH_, 64>(mx, my, mc, p, pl.pub.grid, pl.pub.dyn_smem_bytes, stream)
-    if (cg == 2 && xh == 2) RA_LAUNCH(256, 2, 2);
-    if (cg == 2) RA_LAUNCH(256, 2, 1);
+#define RA_LAUNCH(BN_, CG_, XH_, DYN_)                                                                                        \
+    return p.bk == 32 ? launch_gemm<BN_, CG_, XH_, 32, DYN_>(mx, my, mc, p, pl.pub.grid, pl.pub.dyn_smem_bytes, stream)         \
+                      : launch_gemm<BN_, CG_, XH_, 64, DYN_>(mx, my, mc, p, pl.pub.grid, pl.pub.dyn_smem_bytes, stream)
+    if (cg == 2 && xh == 2) {
+        if (p.dyn) RA_LAUNCH(256, 2, 2, true);
+        RA_LAUNCH(256, 2, 2, false);
+    }
+    if (cg == 2) {
+        if (p.dyn) RA_LAUNCH(256, 2, 1, true);
+        RA_LAUNCH(256, 2, 1, false);
+    }
     switch (pl.bn) {
-        case 64: RA_LAUNCH(64, 1, 1);
-        case 128: RA_LAUNCH(128, 1, 1);
-        case 256: RA_LAUNCH(256, 1, 1);
+        case 64: RA_LAUNCH(64, 1, 1, false);
+        case 128: RA_LAUNCH(128, 1, 1, false);
+        case 256: RA_LAUNCH(256, 1, 1, false);
     }
 #undef RA_LAUNCH
     return RA_ERR_UNSUPPORTED;

@@ -529,7 +529,7 @@ def test_tile_k_32_is_clamped_where_it_cannot_apply(ra):
 @pytest.mark.parametrize("M,N,K,occ", [
     (4096, 4096, 2048, {}),                                    # 128 big tiles over 74 CTA pairs
     (4096, 4096, 1024, dict(sm_budget=20)),                    # 13 tiles per pair: many claims per worker, ring wraps
-    (2048, 3000, 512, dict(cta_group=1, cluster_k=1, sm_budget=16)),   # single-CTA tiles, ragged N
+    (2048, 3000, 512, dict(cta_group=1, cluster_k=1, sm_budget=16)),   # single-CTA tiles, ragged N: always static (the knob is a no-op)
     (3000, 1000, 96, dict(cta_group=2, m_blocks=1, sm_budget=8)),      # 2 k-blocks per tile: the claim happens on the first one
     (1536, 1536, 64, dict(cta_group=2, m_blocks=1, sm_budget=4)),      # ONE k-block per tile
 ])
