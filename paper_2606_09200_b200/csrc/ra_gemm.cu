@@ -1692,8 +1692,12 @@ ra_status gemm_launch(int transA, int transB, int M, int N, int K, float alpha, 
     p.beta = beta;
     if (p.dyn) {
         static_assert(kLaunchCacheEntries <= (size_t)kDynSlots, "one g_dyn slot per launch-cache entry");
-        void* base = nullptr;
-        RA_CUDA(cudaGetSymbolAddress(&base, g_dyn));
+        static void* g_dyn_base[64] = {};          // per device: the symbol's address never changes
+        void* base = (key.device >= 0 && key.device < 64) ? g_dyn_base[key.device] : nullptr;
+        if (base == nullptr) {
+            RA_CUDA(cudaGetSymbolAddress(&base, g_dyn));
+            if (key.device >= 0 && key.device < 64) g_dyn_base[key.device] = base;
+        }
         unsigned long long* slot = static_cast<unsigned long long*>(base) + (size_t)dyn_slot * kDynSlotWords;
         p.dyn_ring = slot;
         p.dyn_ctr = reinterpret_cast<unsigned int*>(slot + kDynWorkers * kDynRing);
