@@ -394,7 +394,8 @@ ra_status ra_overlap_sweep(const ra_workload* w, const ra_overlap_cfg* cfgs, int
  * ra_ipc_export   HOST out-pointer; dev_ptr a DEVICE pointer of this process (not itself an IPC mapping).
  * ra_ipc_open     maps a peer's handle into this process (peer access is enabled lazily by the driver) and returns the
  *                 DEVICE pointer that corresponds to the exported one.  Open each handle once per process.
- * ra_ipc_close    unmaps a pointer ra_ipc_open returned (RA_ERR_INVALID_ARG for any other pointer).
+ * ra_ipc_close    unmaps a pointer ra_ipc_open returned (RA_ERR_INVALID_ARG for any other pointer); ra_shutdown unmaps
+ *                 whatever is still open.
  * ra_peer_slice   host-only: the floats [begin, end) of a count-float buffer that rank `rank` of P reduces; the slices
  *                 partition [0, count), boundaries are multiples of 4 floats (16-byte vectors).
  * ra_allreduce_peer  bufs: HOST array of the P DEVICE pointers IN RANK ORDER (own buffer at index rank, the rest opened

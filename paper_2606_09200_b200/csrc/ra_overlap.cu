@@ -29,6 +29,7 @@ ra_status alltoall_validate(const void* send, const void* recv, int P, size_t ch
                             int ctas_per_sm, int variant);
 
 void gemm_cache_clear();
+void peer_close_all();
 
 // ---- cached host objects ----------------------------------------------------------------------
 struct Cache {
@@ -476,6 +477,7 @@ ra_status ra_overlap_sweep(const ra_workload* w, const ra_overlap_cfg* cfgs, int
 }
 
 void ra_shutdown(void) {
+    ra::peer_close_all();
     ra::gemm_cache_clear();
     (void)ra::l2_persist_ensure(0);
     std::lock_guard<std::mutex> lk(ra::g_cache.mu);

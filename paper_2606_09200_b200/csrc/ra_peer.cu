@@ -64,6 +64,14 @@ static ra_status address_range(const void* p, uintptr_t* base, size_t* size) {
 static std::mutex g_ipc_mu;
 static std::unordered_map<uintptr_t, uintptr_t> g_ipc_open;   // pointer handed out -> mapping base (what cudaIpcCloseMemHandle wants)
 
+// ra_shutdown: unmap whatever the caller left open
+void peer_close_all() {
+    std::lock_guard<std::mutex> lk(g_ipc_mu);
+    for (auto& kv : g_ipc_open) (void)cudaIpcCloseMemHandle(reinterpret_cast<void*>(kv.second));
+    g_ipc_open.clear();
+    (void)cudaGetLastError();
+}
+
 }  // namespace ra
 
 extern "C" {
