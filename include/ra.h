@@ -422,7 +422,7 @@ ra_status ra_alltoall_peer(const void* send, void* const* recv, int P, int rank,
                            void* stream);
 
 /* Sets the current device's persisting-L2 carve-out to min(bytes, device maximum) and reports what was granted (host
- * out-pointer, may be NULL; the driver rounds up to eighths of the L2, 15.8 MiB steps on B200); bytes = 0 takes it back and turns the lines it held into normal ones.  This is the state
+ * out-pointer, may be NULL; the driver rounds up to sixteenths of the L2, 7.9 MiB steps on B200); bytes = 0 takes it back and turns the lines it held into normal ones.  This is the state
  * ra_occupancy.l2_persist_bytes manages for the GEMM (see there); the call exists so that a caller who ran ra_gemm with
  * the knob can give the L2 back before launching something else.  One driver call when the value changes, none
  * otherwise; not to be called while a stream of the device is being captured.  RA_ERR_INVALID_ARG for bytes < 0. */

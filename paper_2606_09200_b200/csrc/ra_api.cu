@@ -46,7 +46,7 @@ ra_status require_sm100(const DeviceInfo& di) { return di.cc_major == 10 ? RA_OK
 // reserve: the library tracks what it last set per device and only calls the driver on a change.
 static std::mutex g_l2_mutex;
 static long long g_l2_state[64];     // what was asked for (after clamping to the device maximum)
-static long long g_l2_granted[64];   // what the driver made of it (it rounds up to eighths of the L2: 15.8 MiB steps on B200)
+static long long g_l2_granted[64];   // what the driver made of it (it rounds up to sixteenths of the L2: 7.9 MiB steps on B200)
 static bool g_l2_known[64] = {};
 
 ra_status l2_persist_ensure(long long bytes, long long* granted) {

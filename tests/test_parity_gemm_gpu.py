@@ -463,7 +463,7 @@ def test_l2_persist_same_bits_and_state(ra):
     got, _ = run_gemm(ra, M, N, K, A, B, occ=occ)
     assert got.tobytes() == base.tobytes()
     set_to = _persisting_l2_limit()                 # ra_gemm leaves the carve-out set (the next GEMM wants it too);
-    assert 24 << 20 <= set_to < 40 << 20            # the driver rounds up to eighths of the L2 (15.8 MiB on B200)
+    assert 24 << 20 <= set_to < 40 << 20            # the driver rounds up to sixteenths of the L2 (7.9 MiB on B200)
     assert ra.ra_l2_persist(0) == 0
     assert _persisting_l2_limit() == 0
     # a knob-free GEMM after a persisting one takes the carve-out back by itself
