@@ -37,7 +37,8 @@ typedef enum {
     RA_ERR_UNSUPPORTED = 2,     /* valid BLAS-wise but not implemented (ld not a multiple of 8 elements, ...) */
     RA_ERR_INFEASIBLE_KNOB = 3, /* smem_reserve_bytes / sm_budget cannot be honoured and allow_clamp == 0 */
     RA_ERR_CUDA = 4,            /* a CUDA call failed; ra_last_cuda_error() returns the cudaError_t value */
-    RA_ERR_ARCH = 5             /* current device is not compute capability 10.x */
+    RA_ERR_ARCH = 5,            /* current device is not compute capability 10.x */
+    RA_ERR_SCRATCH_LIMIT = 6    /* ra_gemm_static_ws only: the plan needs more scratch than RA_GEMM_STATIC_WS_BYTES */
 } ra_status;
 
 /* Static string for a status code (never NULL). */
@@ -188,6 +189,40 @@ size_t ra_gemm_workspace_bytes(int transA, int transB, int M, int N, int K, cons
 ra_status ra_gemm(int transA, int transB, int M, int N, int K, float alpha, const void* A, int lda, const void* B,
                   int ldb, float beta, void* C, int ldc, const ra_occupancy* occ, void* workspace,
                   size_t workspace_bytes, void* stream);
+
+/* ---------------------------------------------------------------------------------------------
+ * ra_gemm for callers that cannot provide scratch memory.
+ *
+ * ra_gemm leaves every device allocation to the caller, including the scratch a stream-K plan needs
+ * (ra_gemm_workspace_bytes).  Some callers have no way to get that scratch: a plug-in that runs inside a
+ * host application whose memory pool already owns the whole HBM and hands none out; code on a serving path
+ * where cudaMalloc / cudaFree are forbidden because they stall every stream of the device -- exactly the
+ * compute / communication concurrency this library exists to keep; a component that is only
+ * given its operands and a stream and must not change the process's memory footprint after start-up.
+ * This entry point is ra_gemm (bf16 output, same arguments, same kernels, same bits) with the workspace
+ * taken from a fixed array that is part of the library image: RA_GEMM_STATIC_WS_BYTES of global memory,
+ * 256-byte aligned, reserved on every GPU whose context loads libra.so and held until the process exits.
+ * It calls no cudaMalloc, cudaFree or other allocating CUDA routine, on the first call or any later one.
+ *
+ *   - Plans that need no scratch behave exactly like ra_gemm with workspace = NULL.
+ *   - A plan that needs more than RA_GEMM_STATIC_WS_BYTES is refused with RA_ERR_SCRATCH_LIMIT before
+ *     anything is enqueued (nothing is written, nothing is launched): lower sm_budget, or use ra_gemm with
+ *     a workspace of your own.  ra_gemm_workspace_bytes tells in advance (host only).
+ *   - The first call on each device looks up the array's device address (cudaGetSymbolAddress, with that
+ *     device current, return code checked) and remembers it.  Make that first call during start-up, outside
+ *     any stream capture; later calls on that device only enqueue work on `stream`.
+ *   - All calls, from every thread and on every stream, use the SAME array, and it keeps whatever the last
+ *     call left in it.  The tile counters at its start are zeroed on `stream` ahead of every launch that
+ *     uses them; the partial sums behind them are written before they are read, so stale contents never
+ *     reach C.  But two calls whose kernels can run at the same time on one GPU (different streams, or
+ *     different host threads without ordering between them) race on the array and produce wrong results
+ *     without an error: order them on one stream or with events.  ra_gemm with per-call workspaces has no
+ *     such restriction.
+ *   - Errors otherwise as ra_gemm.
+ * ------------------------------------------------------------------------------------------- */
+#define RA_GEMM_STATIC_WS_BYTES ((size_t)16 << 20)   /* 16 MiB; config 5's stream-K plans need 4.6 - 6.9 MiB */
+ra_status ra_gemm_static_ws(int transA, int transB, int M, int N, int K, float alpha, const void* A, int lda, const void* B,
+                            int ldb, float beta, void* C, int ldc, const ra_occupancy* occ, void* stream);
 
 /* The same GEMM with a choice of output type ("fp32 output").  c_dtype = RA_DTYPE_BF16 is ra_gemm.
  * RA_DTYPE_F32: C is M x N fp32, ldc in floats (ldc % 4 == 0, 16-byte aligned base); C = alpha*acc + beta*C_in is

@@ -19,6 +19,8 @@ from . import build as _build
 _HERE = os.path.dirname(os.path.abspath(__file__))
 
 RA_OK, RA_ERR_INVALID_ARG, RA_ERR_UNSUPPORTED, RA_ERR_INFEASIBLE_KNOB, RA_ERR_CUDA, RA_ERR_ARCH = range(6)
+RA_ERR_SCRATCH_LIMIT = 6
+RA_GEMM_STATIC_WS_BYTES = 16 << 20      # include/ra.h: the scratch ra_gemm_static_ws carries inside libra.so
 RA_COLL_ALLREDUCE, RA_COLL_ALLTOALL, RA_COLL_NONE = 0, 1, 2
 RA_MODE_SERIAL, RA_MODE_OVERLAP = 0, 1
 RA_MAX_RANKS = 16
@@ -27,7 +29,7 @@ RA_DTYPE_BF16, RA_DTYPE_F32 = 0, 1
 # every symbol include/ra.h declares (tests/test_abi.py checks the header against this and the .so)
 EXPORTS = (
     "ra_status_str", "ra_last_cuda_error", "ra_shutdown", "ra_device_info", "ra_gemm_plan_query", "ra_gemm_residency",
-    "ra_gemm_workspace_bytes", "ra_gemm", "ra_gemm_ex", "ra_allreduce_emul", "ra_allreduce_emul_ex", "ra_alltoall_emul",
+    "ra_gemm_workspace_bytes", "ra_gemm", "ra_gemm_ex", "ra_gemm_static_ws", "ra_allreduce_emul", "ra_allreduce_emul_ex", "ra_alltoall_emul",
     "ra_alltoall_emul_ex",
     "ra_overlap_run", "ra_overlap_run_host", "ra_overlap_suggest", "ra_overlap_autotune", "ra_overlap_sweep", "ra_set_trace",
     "ra_l2_persist", "ra_ipc_export", "ra_ipc_open", "ra_ipc_close", "ra_peer_slice", "ra_allreduce_peer", "ra_alltoall_peer",
@@ -122,6 +124,8 @@ def _L():
                             c_void_p, c_int, POINTER(Occupancy), c_void_p, c_size_t, c_void_p]
     lib.ra_gemm_ex.argtypes = [c_int, c_int, c_int, c_int, c_int, c_float, c_void_p, c_int, c_void_p, c_int, c_float,
                                c_void_p, c_int, c_int, POINTER(Occupancy), c_void_p, c_size_t, c_void_p]
+    lib.ra_gemm_static_ws.argtypes = [c_int, c_int, c_int, c_int, c_int, c_float, c_void_p, c_int, c_void_p, c_int, c_float,
+                                      c_void_p, c_int, POINTER(Occupancy), c_void_p]
     lib.ra_allreduce_emul.argtypes = [POINTER(c_void_p), c_int, c_size_t, c_int, c_void_p]
     lib.ra_allreduce_emul_ex.argtypes = [POINTER(c_void_p), c_int, c_size_t, c_int, c_int, c_int, c_int, c_void_p]
     lib.ra_alltoall_emul.argtypes = [c_void_p, c_void_p, c_int, c_size_t, c_int, c_void_p]
@@ -244,6 +248,15 @@ def ra_gemm_ex(transA, transB, M, N, K, alpha, A, lda, B, ldb, beta, C, ldc, c_d
         workspace_bytes = workspace.numel() * workspace.element_size()
     _check(_L().ra_gemm_ex(transA, transB, M, N, K, float(alpha), _ptr(A), lda, _ptr(B), ldb, float(beta), _ptr(C), ldc,
                            int(c_dtype), _occ_ref(occ), _ptr(workspace), int(workspace_bytes or 0), _stream(stream)), "ra_gemm_ex")
+
+
+def ra_gemm_static_ws(transA, transB, M, N, K, alpha, A, lda, B, ldb, beta, C, ldc, occ=None, stream=None) -> None:
+    """ra_gemm for callers that cannot allocate device memory (a plug-in inside a host application whose pool owns the HBM,
+    a serving path where cudaMalloc would stall the overlapped streams): the stream-K scratch is a fixed
+    RA_GEMM_STATIC_WS_BYTES array inside libra.so.  Raises RaError(RA_ERR_SCRATCH_LIMIT) when the plan needs more.  Every
+    call shares that array: do not let two of them run on the GPU at the same time.  See include/ra.h."""
+    _check(_L().ra_gemm_static_ws(transA, transB, M, N, K, float(alpha), _ptr(A), lda, _ptr(B), ldb, float(beta), _ptr(C),
+                                  ldc, _occ_ref(occ), _stream(stream)), "ra_gemm_static_ws")
 
 
 def _ptr_array(bufs):

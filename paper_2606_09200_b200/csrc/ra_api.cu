@@ -118,6 +118,7 @@ const char* ra_status_str(ra_status s) {
         case RA_ERR_INFEASIBLE_KNOB: return "RA_ERR_INFEASIBLE_KNOB";
         case RA_ERR_CUDA: return "RA_ERR_CUDA";
         case RA_ERR_ARCH: return "RA_ERR_ARCH";
+        case RA_ERR_SCRATCH_LIMIT: return "RA_ERR_SCRATCH_LIMIT";
     }
     return "RA_ERR_UNKNOWN";
 }

@@ -1779,3 +1779,52 @@ ra_status ra_gemm_ex(int transA, int transB, int M, int N, int K, float alpha, c
 }
 
 }  // extern "C"
+
+// ---------------------------------------------------------------------------------------------------------------------
+// ra_gemm_static_ws: the stream-K scratch lives in the library image instead of in a caller allocation (include/ra.h
+// says who needs that and why).  The array is named only here: in host code `g_static_ws` is the host-side shadow of the
+// symbol, NOT a device address -- handing it to a kernel or to cudaMemsetAsync would fault (or, on a machine whose GPU can
+// reach host memory, quietly scribble over the wrong bytes) -- so the address every launch uses comes from
+// cudaGetSymbolAddress, asked once per device with that device current.
+// ---------------------------------------------------------------------------------------------------------------------
+static __device__ __align__(256) unsigned char g_static_ws[RA_GEMM_STATIC_WS_BYTES];
+
+namespace ra {
+namespace {
+constexpr int kStaticWsDevices = 64;
+std::mutex g_static_ws_mu;
+void* g_static_ws_addr[kStaticWsDevices] = {};   // per device ordinal: where that device's copy of the array lives
+
+// Device address of g_static_ws on the CURRENT device.  Set-up (first call per device): one cudaGetSymbolAddress.
+ra_status static_ws_address(void** out) {
+    int dev = -1;
+    RA_CUDA(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= kStaticWsDevices) return RA_ERR_UNSUPPORTED;
+    std::lock_guard<std::mutex> lk(g_static_ws_mu);
+    if (g_static_ws_addr[dev] == nullptr) {
+        void* ptr = nullptr;
+        RA_CUDA(cudaGetSymbolAddress((void**)&ptr, g_static_ws));
+        if (ptr == nullptr || (reinterpret_cast<uintptr_t>(ptr) & 255u)) return RA_ERR_CUDA;
+        g_static_ws_addr[dev] = ptr;
+    }
+    *out = g_static_ws_addr[dev];
+    return RA_OK;
+}
+}  // namespace
+}  // namespace ra
+
+extern "C" ra_status ra_gemm_static_ws(int transA, int transB, int M, int N, int K, float alpha, const void* A, int lda,
+                                       const void* B, int ldb, float beta, void* C, int ldc, const ra_occupancy* occ,
+                                       void* stream) {
+    // How much scratch would this launch take?  Host-only planning; a plan that cannot be made (bad shape, infeasible
+    // knob) is left for gemm_launch to report with its usual code.
+    ra::Plan pl;
+    const bool planned = ra::make_plan(transA, transB, M, N, K, occ, &pl) == RA_OK;
+    if (planned && pl.ws_bytes > RA_GEMM_STATIC_WS_BYTES) return RA_ERR_SCRATCH_LIMIT;
+    void* ws = nullptr;
+    if (planned && pl.ws_bytes > 0) RA_TRY(ra::static_ws_address(&ws));
+    // From here on this is ra_gemm: gemm_launch zeroes the tile counters at the head of the workspace on `stream` before
+    // the kernel (cudaMemsetAsync) and never reads a partial sum it has not written in the same launch.
+    return ra::gemm_launch(transA, transB, M, N, K, alpha, A, lda, B, ldb, beta, C, ldc, occ, ws,
+                           ws ? RA_GEMM_STATIC_WS_BYTES : 0, static_cast<cudaStream_t>(stream), nullptr, 0);
+}
