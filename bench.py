@@ -26,6 +26,7 @@ from __future__ import annotations
 
 import argparse
 import json
+import math
 import os
 import statistics
 import subprocess
@@ -740,6 +741,115 @@ def flat_summary(m, peaks):
             f"gemm_ctas_per_sm_seen {m['gemm_max_ctas_on_one_sm']}")
 
 
+LINE_LIMIT = 2900   # bytes: the whole line fits in the last 3 kB of stdout, whichever way a reader cuts it
+
+
+def _finite(x):
+    """NaN / Inf -> None, recursively: the line must be strict JSON (json.dumps(..., allow_nan=False))."""
+    if isinstance(x, float):
+        return x if math.isfinite(x) else None
+    if isinstance(x, dict):
+        return {k: _finite(v) for k, v in x.items()}
+    if isinstance(x, (list, tuple)):
+        return [_finite(v) for v in x]
+    return x
+
+
+def _r(x, n=4):
+    return None if x is None or not math.isfinite(x) else float(f"{x:.{n}g}") if abs(x) < 1e15 else x
+
+
+def short_summary(m):
+    """One config in ~200 bytes: serial / overlapped us per iteration, their ratio, each kernel alone as a fraction of its
+    peak (GEMM: burst bf16 peak if compute-bound, HBM peak otherwise), overlapped time over the combined roofline."""
+    a, b = m["alone"], m["best_setting"]
+    g = a["gemm_frac_of_bf16_peak_burst"] if m["compute_bound"] else a["gemm_frac_of_hbm_peak"]
+    return (f"ser {m['serial_ms_per_iter'] * 1e3:.1f} ov {m['overlap_ms_per_iter'] * 1e3:.1f} us r {m['time_ratio_same']:.3f}; "
+            f"gemm {g:.3f} {'tensor' if m['compute_bound'] else 'hbm'}; coll {a['coll_frac_of_hbm_peak']:.3f} hbm; "
+            f"ov/roof {m['overlap_vs_roofline']['sustained']:.3f}s {m['overlap_vs_roofline']['burst']:.3f}b; "
+            f"res{b['smem_reserve_bytes'] // 1024}K sm{b['sm_budget']} prio-{b['priority']} cv{b['coll_variant']}")
+
+
+def contract_line(cfg, m, per_config, peaks, cpu, world, steps, warmup, sweep, total_bench_s=None, detail_path=""):
+    """The ONE stdout line of the bench contract (small: the contract keys, `roofline`, `cpu_baseline`, `e2e`, `clocks`, the
+    serial / overlap scalars and one short string per config) and the detail document (everything measured) that goes to
+    --detail.  `m` is measure_config's result for the headline workload, `per_config` the other workloads' results."""
+    flops, gbytes, cbytes = cfg.gemm_flops, cfg.gemm_bytes, cfg.coll_bytes
+    alone, over_ms, gemm_in_step_ms = m["alone"], m["overlap_ms_per_iter"], m["gemm_in_step_ms"]
+    # dominant kernel = the GEMM: 0.8 of the step's kernel time on cb-*, the HBM stream on mb-*; launch_ms = CUDA events
+    # around every K_g launch, on the compute stream, in the instrumented pass of the same K steps after the timed region
+    if m["compute_bound"]:
+        ach = flops / gemm_in_step_ms / 1e9
+        roof = {"kernel": "ra::gemm_kernel", "bound": "tensor", "achieved": ach, "peak": peaks["bf16_tflops_sustained"], "unit": "TFLOP/s",
+                "frac": ach / peaks["bf16_tflops_sustained"], "traffic": None, "peak_kind": f"{peaks['source']}, sustained (kernel timed inside a long step)",
+                "launch_ms": gemm_in_step_ms, "frac_of_burst_peak": ach / peaks["bf16_tflops"],
+                "alone_burst": {"achieved": alone["gemm_tflops_burst"], "peak": peaks["bf16_tflops"], "frac": alone["gemm_frac_of_bf16_peak_burst"]}}
+    else:
+        ach = gbytes / gemm_in_step_ms / 1e6
+        roof = {"kernel": "ra::gemm_kernel", "bound": "hbm", "achieved": ach, "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": ach / peaks["hbm_gbs"],
+                "traffic": None, "peak_kind": peaks["source"], "launch_ms": gemm_in_step_ms,
+                "alone": {"achieved": alone["gemm_gbs"], "peak": peaks["hbm_gbs"], "frac": alone["gemm_frac_of_hbm_peak"]}}
+    roof["algorithmic_bytes"] = gbytes
+    tpath = os.path.join(ROOT, "profiles", "traffic.json")   # dram bytes per launch from the committed ncu --set full capture
+    if os.path.exists(tpath):
+        with open(tpath) as f:
+            t = json.load(f).get(cfg.name, {})
+        # the capture that matches the timed setting: with or without the L2 carve-out (profiles/r02_l2_persist.md)
+        persist = m["best_setting"].get("l2_persist_bytes", 0) >= 79 << 20
+        roof["traffic"] = t.get("gemm_dram_bytes_l2_persist_79MiB" if persist else "gemm_dram_bytes")
+        roof["traffic_source"] = "profiles/traffic.json (one ncu capture, another box; not this run)"
+    # both kernels share HBM inside the overlapped step, so a kernel's in-step rate understates the memory system's use:
+    # the whole iteration's algorithmic bytes over its time is the figure to hold against the HBM peak
+    step_gbs = (gbytes + cbytes) / over_ms / 1e6
+    combined_step = {"bound": "hbm", "achieved": step_gbs, "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": step_gbs / peaks["hbm_gbs"],
+                     "bytes_per_iter": gbytes + cbytes}
+
+    b = m["best_setting"]
+    config = {"workload": cfg.name, "gemm": [cfg.M, cfg.N, cfg.K], "collective": cfg.coll, "P": cfg.P, "coll_bytes_moved": cbytes,
+              "n_iters_per_step": m["n_iters_per_step"], "l2": "inputs_exceed_l2 (no flush needed)", "multi_gpu": "replicas only",
+              "sweep": sweep, "setting": {k: b[k] for k in ("smem_reserve_bytes", "sm_budget", "priority", "coll_sm_budget", "coll_variant", "use_graph") if k in b},
+              "configs_in_this_run": [cfg.name] + list(per_config), "detail": detail_path or None}
+    config["cfg." + cfg.name] = short_summary(m)
+    for name, pm in per_config.items():
+        config["cfg." + name] = short_summary(pm)
+    e2e = m.get("e2e")
+    line = {
+        "metric": METRIC, "value": m["value"], "unit": UNIT, "n_gpus": world, "steps": steps, "warmup": warmup,
+        "ms_per_step": m["ms_per_step"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16",
+        "data": "synthetic", "gpu_launches": m["gpu_launches"], "config": config,
+        "serial_ms_per_iter": _r(m["serial_ms_per_iter"]), "overlap_ms_per_iter": _r(over_ms), "time_ratio": _r(m["time_ratio_same"]),
+        "time_ratio_vs_kernels_alone": _r(m["time_ratio_best"]), "norm_time_priority": _r(m["norm_time_priority"]),
+        "overlap_rate": _r(m["overlap_rate"]), "coll_alone_frac_of_hbm_peak": _r(alone["coll_frac_of_hbm_peak"]),
+        "combined_roofline_ms": {k: _r(v) for k, v in m["combined_roofline_ms"].items()},
+        "overlap_vs_roofline": {k: _r(v) for k, v in m["overlap_vs_roofline"].items()},
+        "wall_ms_timed_region": _r(m["wall_ms_timed_region"], 6), "paper_context": "paper: up to 25.5% less time, priority vs baseline overlap, A40 (PAPER.md:7,122): context, not the target",
+        "roofline": {k: (_r(v, 6) if isinstance(v, float) and abs(v) < 1e6 else v) for k, v in roof.items()},
+        "cpu_baseline": None if cpu is None else {"value": cpu["value"], "unit": cpu["unit"], "cores": cpu["cores"], "kind": cpu["kind"],
+                                                  "sample": cpu["sample"][:160]},
+        "e2e": None if e2e is None else {k: e2e[k] for k in ("value", "unit", "h2d_bytes_per_step", "d2h_bytes_per_step")},
+        "clocks": {k: m["clocks"].get(k) for k in ("sm_mhz", "sm_max_mhz", "reasons")},
+    }
+    line["roofline"]["alone_burst" if m["compute_bound"] else "alone"] = {k: _r(v, 5) for k, v in roof["alone_burst" if m["compute_bound"] else "alone"].items()}
+    line = _finite(line)
+    # never let the line outgrow a 3 kB tail: the optional parts go first (they are all in the detail file)
+    for drop in ("paper_context", "cfgs", "time_ratio_vs_kernels_alone", "combined_roofline_ms"):
+        if len(dumps_line(line)) <= LINE_LIMIT:
+            break
+        if drop == "cfgs":
+            for k in [k for k in line["config"] if k.startswith("cfg.")]:
+                del line["config"][k]
+        else:
+            line.pop(drop, None)
+    detail = {"line": line, "headline": m, "per_config": per_config, "roofline": dict(roof, combined_step=combined_step),
+              "cpu_baseline": cpu, "peaks": peaks, "total_bench_s": total_bench_s, "paper_context": PAPER_CONTEXT,
+              "cfg_long": dict({cfg.name: flat_summary(m, peaks)}, **{n: flat_summary(pm, peaks) for n, pm in per_config.items()})}
+    return line, detail
+
+
+def dumps_line(line) -> str:
+    return json.dumps(line, allow_nan=False, separators=(", ", ": "))
+
+
 def run_ours(args, cfg):
     import torch
     if not torch.cuda.is_available():
@@ -760,67 +870,19 @@ def run_ours(args, cfg):
     if rank != 0:
         return
 
-    # ---- rooflines (dominant kernel = the GEMM: 0.8 of the step's kernel time on cb-*, the HBM stream on mb-*) ----
-    flops, gbytes, cbytes = cfg.gemm_flops, cfg.gemm_bytes, cfg.coll_bytes
-    alone, over_ms, gemm_in_step_ms = m["alone"], m["overlap_ms_per_iter"], m["gemm_in_step_ms"]
-    src = "CUDA events around every K_g launch, on the compute stream, instrumented pass of the same K steps right after the timed region"
-    if m["compute_bound"]:
-        ach = flops / gemm_in_step_ms / 1e9
-        roof = {"kernel": "ra::gemm_kernel", "bound": "tensor", "achieved": ach, "peak": peaks["bf16_tflops_sustained"], "unit": "TFLOP/s",
-                "frac": ach / peaks["bf16_tflops_sustained"], "traffic": None, "peak_source": f"{peaks['source']} (sustained: kernel timed inside a long overlapped step)",
-                "launch_ms": gemm_in_step_ms, "launch_ms_source": src, "frac_of_burst_peak": ach / peaks["bf16_tflops"],
-                "alone": {"achieved": alone["gemm_tflops_burst"], "peak": peaks["bf16_tflops"], "frac": alone["gemm_frac_of_bf16_peak_burst"], "peak_kind": "burst (best of 10 single launches)"}}
-    else:
-        ach = gbytes / gemm_in_step_ms / 1e6
-        roof = {"kernel": "ra::gemm_kernel", "bound": "hbm", "achieved": ach, "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": ach / peaks["hbm_gbs"],
-                "traffic": None, "peak_source": peaks["source"], "launch_ms": gemm_in_step_ms, "launch_ms_source": src,
-                "alone": {"achieved": alone["gemm_gbs"], "peak": peaks["hbm_gbs"], "frac": alone["gemm_frac_of_hbm_peak"]}}
-    # both kernels share HBM inside the overlapped step, so a kernel's in-step rate understates the memory system's use:
-    # the whole iteration's algorithmic bytes over its time is the figure to hold against the HBM peak
-    step_gbs = (gbytes + cbytes) / over_ms / 1e6
-    roof["combined_step"] = {"bound": "hbm", "achieved": step_gbs, "peak": peaks["hbm_gbs"], "unit": "GB/s",
-                             "frac": step_gbs / peaks["hbm_gbs"], "bytes_per_iter": gbytes + cbytes}
-    tpath = os.path.join(ROOT, "profiles", "traffic.json")   # dram bytes per launch from the committed ncu capture
-    if os.path.exists(tpath):
-        with open(tpath) as f:
-            t = json.load(f).get(cfg.name, {})
-            # the capture that matches the timed setting: with or without the L2 carve-out (profiles/r02_l2_persist.md)
-            persist = m["best_setting"].get("l2_persist_bytes", 0) >= 79 << 20
-            roof["traffic"] = t.get("gemm_dram_bytes_l2_persist_79MiB" if persist else "gemm_dram_bytes")
-    roof["algorithmic_bytes"] = gbytes
-
     cpu = None
     if args.gpus == 1 and not args.no_cpu_baseline:
         t_iter, desc, cores, kind = cpu_oracle_full(cfg)
         cpu = {"value": 1.0 / t_iter, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc, "seconds_per_iter": t_iter,
                "timed": kind}
-
-    config = {"workload": cfg.name, "gemm": [cfg.M, cfg.N, cfg.K], "layout": "transA=0,transB=1 (K-contiguous)", "collective": cfg.coll,
-              "P": cfg.P, "coll_bytes_moved": cbytes, "n_iters_per_step": m["n_iters_per_step"], "l2": "inputs_exceed_l2 (no flush needed)",
-              "multi_gpu": "replicas only", "best_setting": m["best_setting"], "plan": m["plan"], "sweep": args.sweep,
-              "timed_region": "K steps at the picked setting, no per-kernel events; allreduce buffers refilled from pristine copies before every run",
-              "configs_in_this_run": [cfg.name] + list(per_config)}
-    config["cfg." + cfg.name] = flat_summary(m, peaks)
-    for name, pm in per_config.items():
-        config["cfg." + name] = flat_summary(pm, peaks)
-
-    line = {
-        "metric": METRIC, "value": m["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
-        "ms_per_step": m["ms_per_step"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16",
-        "data": "synthetic", "config": config,
-        "overlap_ms_per_iter": over_ms, "serial_ms_per_iter": m["serial_ms_per_iter"], "time_ratio_best": m["time_ratio_best"],
-        "time_ratio_same": m["time_ratio_same"], "norm_time_priority": m["norm_time_priority"], "overlap_rate": m["overlap_rate"],
-        "sweep_serial_ms_per_iter": m["sweep_serial_ms_per_iter"],
-        "gemm_in_step_ms": gemm_in_step_ms, "coll_in_step_ms": m["coll_in_step_ms"], "instrumented_ms_per_iter": m["instrumented_ms_per_iter"],
-        "alone": alone, "policy": m["policy"], "residency": m.get("residency"), "peaks": peaks,
-        "per_config": per_config, "total_bench_s": time.perf_counter() - t_start,
-        "paper_context": PAPER_CONTEXT,
-        # the keys a reader of the last 1.5 kB of this line should find there
-        "wall_ms_timed_region": m["wall_ms_timed_region"], "gemm_max_ctas_on_one_sm": m["gemm_max_ctas_on_one_sm"],
-        "combined_roofline_ms": m["combined_roofline_ms"], "overlap_vs_roofline": m["overlap_vs_roofline"],
-        "roofline": roof, "cpu_baseline": cpu, "e2e": m["e2e"], "gpu_launches": m["gpu_launches"], "clocks": m["clocks"],
-    }
-    print(json.dumps(line), flush=True)
+    line, detail = contract_line(cfg, m, per_config, peaks, cpu, world, args.steps, max(args.warmup, 3), args.sweep,
+                                 total_bench_s=time.perf_counter() - t_start, detail_path=args.detail)
+    if args.detail:
+        os.makedirs(os.path.dirname(os.path.abspath(args.detail)), exist_ok=True)
+        with open(args.detail, "w") as f:
+            json.dump(_finite(detail), f, indent=1, allow_nan=False)
+        print(f"bench.py: per-config results, sweep, policy, residency and peaks are in {args.detail}", file=sys.stderr, flush=True)
+    print(dumps_line(line), flush=True)
 
 
 # ------------------------------------------------------------------------------------------------
@@ -986,6 +1048,9 @@ def main():
     ap.add_argument("--per-config", default="all", choices=["all", "none"],
                     help="at N=1 also run the other four BASELINE.json configs (default) or only --config")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--detail", default=os.path.join("gpurun_out", "bench_detail.json"),
+                    help="everything the run measured (per-config results, sweep, policy, residency, peaks) goes to this JSON "
+                         "file; stdout carries only the short contract line ('' = do not write it)")
     ap.add_argument("--ref-budget-s", type=float, default=90.0, help="--impl reference: CPU seconds for warmup + steps")
     ap.add_argument("--table", default="", help="write the sweep table (JSON; --mode power-table: markdown) here")
     ap.add_argument("--static-order", action="store_true", help="--mode gemm-only: occ.tile_order = 1 (static tile assignment)")
