@@ -123,6 +123,63 @@ def test_full_size_integer_exact(ra, index):
     torch.cuda.empty_cache()
 
 
+KIB = 1024
+
+
+def test_config5_corners_integer_exact(ra):
+    """The memory-bound shape (64 x 16384 x 16384) at the twelve corners of config 5's grid -- smem_reserve_bytes
+    {0, 64, 128, 200} KiB x sm_budget {74, 110, 148} -- through ra_overlap_run with the config's alltoall on the other
+    stream, all 2^20 entries compared with the oracle bit for bit on small-integer operands (PAPER.md:28 defines the
+    result; shaping occupancy must not change it).  Under the 1e-2 normalised bound a lost 64-wide k-block
+    moves an entry by ~2e-3 and passes; here it cannot.  The plan families are asserted, so the pin cannot quietly move
+    to another path: budgets 74 / 110 are stream-K (split_k > 1, grid = budget), 128 / 200 KiB are one-stage pipelines."""
+    import torch
+    cfg = ra_inputs.CONFIGS[4]
+    M, N, K = cfg.M, cfg.N, cfg.K
+    assert (M, N, K) == (64, 16384, 16384) and cfg.coll == "alltoall"
+    A = ra_inputs.smallint_bf16((M, K), cfg.seed + 200, ra_inputs.STREAM_A)
+    B = ra_inputs.smallint_bf16((N, K), cfg.seed + 200, ra_inputs.STREAM_B)
+    assert 4 * K < 1 << 24
+    _, ref16 = oracle.gemm(0, 1, M, N, K, 1.0, A, B)
+    assert len(np.unique(ref16)) > 100                                     # not a degenerate reference
+    dA, dB = to_dev(A), to_dev(B)
+    send = ra_inputs.alltoall_payload(cfg)
+    ref_b = oracle.alltoall(send, cfg.P, cfg.chunk_bytes)
+    da = to_dev(send)
+    db = torch.zeros_like(da)
+    hi = ra.ra_device_info()["prio_greatest"]
+    seen = set()
+    for reserve in (0, 64 * KIB, 128 * KIB, 200 * KIB):
+        for budget in (74, 110, 148):
+            for tile_k in ((64, 32) if reserve in (0, 128 * KIB) else (64,)):
+                occ = dict(smem_reserve_bytes=reserve, sm_budget=budget, tile_k=tile_k)
+                plan = ra.ra_gemm_plan_query(0, 1, M, N, K, occ)
+                if budget < 148:
+                    assert plan["split_k"] > 1 and plan["grid"] == budget, plan
+                else:
+                    assert plan["split_k"] == 1, plan
+                if reserve >= 128 * KIB and tile_k == 64:
+                    assert plan["stages"] == 1, plan
+                seen.add((plan["split_k"] > 1, plan["stages"], plan["tile_k"]))
+                dC = torch.full((M, N), 0x7FC0, dtype=torch.int16, device="cuda")
+                ws = torch.empty(max(ra.ra_gemm_workspace_bytes(0, 1, M, N, K, occ), 16), dtype=torch.uint8, device="cuda")
+                w, keep = ra.make_workload(gemm=dict(M=M, N=N, K=K, A=dA, B=dB, C=dC, workspace=ws),
+                                           alltoall=dict(a=da, b=db, P=cfg.P, chunk_bytes=cfg.chunk_bytes), n_iters=N_ITERS)
+                res = ra.ra_overlap_run(w, ra.make_cfg(mode=1, prio_compute=0, prio_comm=hi if budget != 110 else 0, occ=occ))
+                torch.cuda.synchronize()
+                assert res["plan"]["split_k"] == plan["split_k"] and res["plan"]["stages"] == plan["stages"]
+                got = to_host(dC, np.uint16).reshape(M, N)
+                bad = np.argwhere(got != ref16)
+                assert bad.size == 0, (f"{len(bad)} of {M * N} entries differ, first at {bad[0].tolist()}: "
+                                       f"gpu {got[tuple(bad[0])]:#06x} ref {ref16[tuple(bad[0])]:#06x}", plan, occ)
+                del dC, w, ws
+    assert len(seen) >= 6, seen                                            # stream-K and data-parallel, deep and one-stage, both tile_k
+    assert np.array_equal(to_host(db, np.uint64), ref_b.view(np.uint64))   # the collective that ran beside them
+    assert np.array_equal(to_host(da, np.uint64), send.view(np.uint64))
+    torch.cuda.empty_cache()
+
+
+
 @pytest.mark.parametrize("index", [1, 2, 3, 4, 5, 6, 7, 8])
 def test_full_size_config(ra, index):
     import torch
