@@ -98,7 +98,12 @@ typedef struct {
                                  like the shared-memory reserve.  ra_gemm sets the carve-out when it
                                  differs from what the library last set (one driver call, not inside a stream capture)
                                  and leaves it set; ra_overlap_run / _sweep / _autotune / _run_host set it for the run and
-                                 take it back before returning; ra_l2_persist(0) and ra_shutdown take it back too.
+                                 take it back before returning; ra_l2_persist(0) takes it back too, and ra_shutdown puts back whatever
+                                 carve-out the context had before the library first touched it.  With the knob at 0 the
+                                 library still clears a carve-out it finds on first use (a foreign set-aside costs the
+                                 collectives ~4 %), but only as best effort: if the driver refuses, the call carries on.
+                                 Nothing is changed while `stream` is being captured.  Requests above the device maximum
+                                 are clamped in the plan (ra_gemm_plan.l2_persist_bytes reports the clamped value).
                                  Ignored (reported as 0 in the plan) by swapped, stream-K, cluster split-K and
                                  single-wave plans.  Does not change results (same per-element k order). */
     int32_t tile_k;           /* 0 / 64 = default: 64 bf16 of K per pipeline stage (128-byte swizzle rows).  32: half-size
@@ -115,7 +120,12 @@ typedef struct {
                                  rows coalesce in L2 (8192^3: 11 % fewer L2-slice reads, 2 % faster; profiles/r02_tile_order.md).
                                  1 = static: worker w owns tiles w, w + W, w + 2W, ...  Either way every C element is
                                  accumulated in the same ascending-k order, so results are bit-identical.  Single-CTA tiles,
-                                 stream-K, cluster split-K, bounded-work and single-wave plans are always static. */
+                                 stream-K, cluster split-K, bounded-work and single-wave plans are always static.
+                                 Concurrency: every dynamic-order launch IN FLIGHT owns one of 32 device-side launch slots
+                                 (claim counter + ring), tracked with an event recorded behind the launch, so the same call
+                                 on several streams or from several host threads is safe.  A launch that finds all slots in
+                                 flight, or whose stream is being captured into a CUDA graph (the graph would hold the slot
+                                 for as long as it lives), silently runs the static order instead -- same bits. */
 } ra_occupancy;
 
 /* What S3 decided -- for tests, logs and the sweep tables. */
@@ -183,6 +193,8 @@ size_t ra_gemm_workspace_bytes(int transA, int transB, int M, int N, int K, cons
  * propagate), as in BLAS.
  * workspace: device pointer, 16-byte aligned, at least ra_gemm_workspace_bytes(...) bytes (may be
  * NULL when that is 0).  Its contents are scratch; it must not be shared by two GEMMs in flight.
+ * Thread-safety: calls on distinct streams from distinct host threads are safe (also with identical arguments) as
+ * long as they do not share a workspace or write overlapping C.
  * Results are bit-reproducible run to run for a fixed (shape, plan): stream-K partial sums are
  * combined in ascending-k order, never with floating-point atomics.
  * ------------------------------------------------------------------------------------------- */
@@ -428,9 +440,12 @@ ra_status ra_overlap_sweep(const ra_workload* w, const ra_overlap_cfg* cfgs, int
  *                 can be shared) and the bytes that follow it.  Plain bytes: ship it over any transport.
  * ra_ipc_export   HOST out-pointer; dev_ptr a DEVICE pointer of this process (not itself an IPC mapping).
  * ra_ipc_open     maps a peer's handle into this process (peer access is enabled lazily by the driver) and returns the
- *                 DEVICE pointer that corresponds to the exported one.  Open each handle once per process.
- * ra_ipc_close    unmaps a pointer ra_ipc_open returned (RA_ERR_INVALID_ARG for any other pointer); ra_shutdown unmaps
- *                 whatever is still open.
+ *                 DEVICE pointer that corresponds to the exported one.  Opening the same handle again returns the same
+ *                 pointer and takes another reference: pair every ra_ipc_open with one ra_ipc_close.  NOTE: the handle
+ *                 covers the whole ALLOCATION that holds the exported pointer (a caching allocator's segment, say), so a
+ *                 peer can reach everything in it; export from dedicated allocations if that matters.
+ * ra_ipc_close    drops one reference on a pointer ra_ipc_open returned (RA_ERR_INVALID_ARG for any other pointer) and
+ *                 unmaps it with the last one; ra_shutdown unmaps whatever is still open.
  * ra_peer_slice   host-only: the floats [begin, end) of a count-float buffer that rank `rank` of P reduces; the slices
  *                 partition [0, count), boundaries are multiples of 4 floats (16-byte vectors).
  * ra_allreduce_peer  bufs: HOST array of the P DEVICE pointers IN RANK ORDER (own buffer at index rank, the rest opened
@@ -439,7 +454,8 @@ ra_status ra_overlap_sweep(const ra_workload* w, const ra_overlap_cfg* cfgs, int
  *                 has run, every buffer equals the oracle's allreduce bit for bit.  variant as ra_allreduce_emul_ex.
  * ra_alltoall_peer   send: this rank's P chunks (DEVICE); recv: HOST array of the P ranks' receive buffers (DEVICE
  *                 pointers in rank order, P chunks each).  Pushes chunk j into slot `rank` of recv[j]:
- *                 recv_j[rank] = send_rank[j].  variant as ra_alltoall_emul_ex (2 = copy engines, peer-to-peer).
+ *                 recv_j[rank] = send_rank[j].  variant as ra_alltoall_emul_ex (2 = copy engines, peer-to-peer).  The receive
+ *                 buffers must be pairwise disjoint and disjoint from send (else RA_ERR_INVALID_ARG).
  * Errors as the emulation calls; 1 <= P <= RA_MAX_RANKS, 0 <= rank < P.
  * ------------------------------------------------------------------------------------------- */
 typedef struct {

@@ -48,6 +48,7 @@ static std::mutex g_l2_mutex;
 static long long g_l2_state[64];     // what was asked for (after clamping to the device maximum)
 static long long g_l2_granted[64];   // what the driver made of it (it rounds up to sixteenths of the L2: 7.9 MiB steps on B200)
 static bool g_l2_known[64] = {};
+static long long g_l2_found[64];     // what the context had when the library first looked (given back by l2_persist_restore)
 
 ra_status l2_persist_ensure(long long bytes, long long* granted) {
     if (bytes < 0) return RA_ERR_INVALID_ARG;
@@ -62,6 +63,7 @@ ra_status l2_persist_ensure(long long bytes, long long* granted) {
         size_t cur = 0;
         RA_CUDA(cudaDeviceGetLimit(&cur, cudaLimitPersistingL2CacheSize));
         g_l2_granted[dev] = (long long)cur;
+        g_l2_found[dev] = (long long)cur;
         g_l2_state[dev] = cur == 0 ? 0 : -1;
         g_l2_known[dev] = true;
     }
@@ -71,21 +73,71 @@ ra_status l2_persist_ensure(long long bytes, long long* granted) {
     if (want != g_l2_state[dev]) {
         // Shrinking: persisting lines are given up FIRST -- the driver was seen to leave the limit at what is still in use
         // (3/16 of the L2 after a 24 MiB panel) when asked to go to 0 with lines resident.
-        if (want < g_l2_state[dev] || g_l2_state[dev] < 0) RA_CUDA(cudaCtxResetPersistingL2Cache());
-        RA_CUDA(cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, (size_t)want));
-        size_t got = 0;
-        RA_CUDA(cudaDeviceGetLimit(&got, cudaLimitPersistingL2CacheSize));
-        if (want == 0 && got != 0) {                       // in-flight work re-marked lines in between: drain and retry once
-            RA_CUDA(cudaDeviceSynchronize());
-            RA_CUDA(cudaCtxResetPersistingL2Cache());
-            RA_CUDA(cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, 0));
-            RA_CUDA(cudaDeviceGetLimit(&got, cudaLimitPersistingL2CacheSize));
+        const auto apply = [&](size_t* got) -> cudaError_t {
+            cudaError_t e = cudaSuccess;
+            if (want < g_l2_state[dev] || g_l2_state[dev] < 0) e = cudaCtxResetPersistingL2Cache();
+            if (e == cudaSuccess) e = cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, (size_t)want);
+            if (e == cudaSuccess) e = cudaDeviceGetLimit(got, cudaLimitPersistingL2CacheSize);
+            if (e == cudaSuccess && want == 0 && *got != 0) {  // in-flight work re-marked lines in between: drain and retry once
+                e = cudaDeviceSynchronize();
+                if (e == cudaSuccess) e = cudaCtxResetPersistingL2Cache();
+                if (e == cudaSuccess) e = cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, 0);
+                if (e == cudaSuccess) e = cudaDeviceGetLimit(got, cudaLimitPersistingL2CacheSize);
+            }
+            return e;
+        };
+        size_t got = (size_t)g_l2_granted[dev];
+        const cudaError_t e = apply(&got);
+        if (e != cudaSuccess) {
+            if (want > 0) RA_CUDA(e);          // the caller asked for a carve-out and cannot have it: that is an error
+            // want == 0 is housekeeping with the feature OFF (every collective and every plain GEMM passes through here): where
+            // the driver will not let this process change the limit (a set-aside fixed from outside, MPS) nothing the caller
+            // asked for has failed.  Best effort: forget the error, remember that it was tried, carry on.
+            (void)cudaGetLastError();
+            got = (size_t)g_l2_granted[dev];
         }
         g_l2_state[dev] = want;
         g_l2_granted[dev] = (long long)got;
     }
     if (granted) *granted = g_l2_granted[dev];
     return RA_OK;
+}
+
+// ra_gemm's form: the same, except that nothing happens while `stream` is being captured (cudaDeviceSetLimit cannot be
+// captured; the GEMM then runs with whatever carve-out is in place -- same results, the evict_last hints just do not stick)
+// and that the common case -- the state already is what is asked for -- costs one mutex and no driver call.
+ra_status l2_persist_ensure_on(long long bytes, cudaStream_t stream) {
+    if (bytes < 0) return RA_ERR_INVALID_ARG;
+    int dev = -1;
+    RA_CUDA(cudaGetDevice(&dev));
+    if (dev >= 0 && dev < 64) {
+        std::lock_guard<std::mutex> lk(g_l2_mutex);
+        if (g_l2_known[dev] && g_l2_state[dev] == bytes) return RA_OK;
+    }
+    cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+    if (cudaStreamIsCapturing(stream, &cs) != cudaSuccess || cs != cudaStreamCaptureStatusNone) {
+        (void)cudaGetLastError();
+        return RA_OK;
+    }
+    return l2_persist_ensure(bytes);
+}
+
+// ra_shutdown: the current device's carve-out goes back to what the context had before the library first touched it (an
+// application that set one for its own access-policy windows gets it back), and the library forgets the device's state.
+void l2_persist_restore() {
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) {
+        (void)cudaGetLastError();
+        return;
+    }
+    std::lock_guard<std::mutex> lk(g_l2_mutex);
+    if (!g_l2_known[dev]) return;
+    if (g_l2_granted[dev] != g_l2_found[dev]) {
+        bool ok = cudaCtxResetPersistingL2Cache() == cudaSuccess;
+        ok = ok && cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, (size_t)g_l2_found[dev]) == cudaSuccess;
+        if (!ok) (void)cudaGetLastError();
+    }
+    g_l2_known[dev] = false;
 }
 
 // First use of a collective on a device: take back a carve-out the context came up with (see above).  A no-op once the

@@ -42,6 +42,10 @@ ra_status require_sm100(const DeviceInfo& di);
 // last set (then no driver call is made); bytes = 0 also resets the persisting lines.  Must not be called while a
 // stream of the device is being captured unless it is a no-op.
 ra_status l2_persist_ensure(long long bytes, long long* granted = nullptr);
+// The same for a launch on `stream`: skipped (RA_OK) while that stream is being captured; no driver call when nothing changes.
+ra_status l2_persist_ensure_on(long long bytes, cudaStream_t stream);
+// Gives the current device's carve-out back as the library found it and forgets the device (ra_shutdown).
+void l2_persist_restore();
 // Collectives call this before their first launch on a device: takes back a carve-out the context came up with.
 ra_status l2_persist_first_use(cudaStream_t stream);
 

@@ -109,7 +109,7 @@ __device__ int g_gemm_max_resident;
 // coalescer together and are served by one slice read.  A static assignment (worker w owns tiles w, w + W, ...) keeps handing
 // adjacent tiles to workers that drifted apart waves ago: ncu on 8192^3 shows 1.07 GPC deliveries per L2-slice read with
 // the static order (1.25 in a one-wave problem, where everybody starts together) against cuBLAS's 1.37.
-// One launch slot per launch-cache entry: [kDynWorkers][kDynRing] ring entries + {claim counter, exit counter, generation}.
+// One launch slot per launch in flight (see dyn_slot_acquire): [kDynWorkers][kDynRing] ring entries + {claim counter, exit counter, generation}.
 // The slot re-arms ITSELF: ring tags carry the slot's generation, and the last CTA to leave the kernel zeroes the two
 // counters and bumps the generation, so the next launch finds a clean slot without a memset node in front of it.  (A
 // memset node was tried first and cost the overlapped step 6 %: it delays K_g^(i+1) by a few microseconds, the waiting
@@ -1180,6 +1180,20 @@ static ra_status validate_shape(int transA, int transB, int M, int N, int K) {
     return RA_OK;
 }
 
+// cudaDevAttrMaxPersistingL2CacheSize of the current device, or B200's figure (79 MiB) where no device can be asked
+// (the planner also runs host-only).  Asked once.
+static long long max_persisting_l2() {
+    static const long long v = [] {
+        int dev = -1, bytes = 0;
+        if (cudaGetDevice(&dev) == cudaSuccess &&
+            cudaDeviceGetAttribute(&bytes, cudaDevAttrMaxPersistingL2CacheSize, dev) == cudaSuccess && bytes > 0)
+            return (long long)bytes;
+        (void)cudaGetLastError();
+        return (long long)79 << 20;
+    }();
+    return v;
+}
+
 static ra_status make_plan(int transA, int transB, int M, int N, int K, const ra_occupancy* occ_in, Plan* out) {
     RA_TRY(validate_shape(transA, transB, M, N, K));
     ra_occupancy occ = {0, 0, 0, 1, 0, 0, 0, 0, 0, 0};
@@ -1350,7 +1364,7 @@ static ra_status make_plan(int transA, int transB, int M, int N, int K, const ra
     int grid, stream_k = 0, ctas_per_sm = n_acc, ks = 1;
     // Residency (A22 / A23): the plan's accounting -- smem_left_per_sm >= reserve -- assumes ONE GEMM CTA per SM.  That is
     // guaranteed by the footprint itself when a second CTA cannot fit: the request is padded past half of an SM's
-    // shared memory whenever the hardware (cudaOccupancyMaxActiveBlocksPerMultiprocessor) would otherwise admit two
+    // shared memory whenever the hardware (resident_ctas(): registers, threads, shared memory -- NOT the occupancy API, see there) would otherwise admit two
     // and the padding still honours the reserve -- the paper's direction: more shared memory per block, fewer
     // resident blocks.
     const int half = (smem_per_sm - 2 * reserved) / 2 + 16;
@@ -1460,14 +1474,17 @@ static ra_status make_plan(int transA, int transB, int M, int N, int K, const ra
         // panel still keeps part of it.
         const long long xtile_bytes = (long long)tile_x * K * 2;
         if (occ.l2_persist_bytes > 0 && !swap && !stream_k && ks == 1 && tiles_x * tiles_y > workers && xtile_bytes > 0) {
-            const int fit = (int)(occ.l2_persist_bytes / xtile_bytes);
+            // what can actually persist: the request clamped to the device's maximum carve-out (the raster group is sized
+            // from this, and the plan reports it, so a 1 GiB request does not widen the group past what L2 can hold)
+            const long long l2_bytes = occ.l2_persist_bytes < max_persisting_l2() ? occ.l2_persist_bytes : max_persisting_l2();
+            const int fit = (int)(l2_bytes / xtile_bytes);
             if (fit > gx) {
                 gx = fit < tiles_x ? fit : tiles_x;
                 const int groups = (tiles_x + gx - 1) / gx;
                 gx = (tiles_x + groups - 1) / groups;         // equal groups: 16 tile rows at 9 that fit -> 8 + 8, not 9 + 7
             }
             pl.hint_x = 2;
-            g.l2_persist_bytes = occ.l2_persist_bytes;
+            g.l2_persist_bytes = (int32_t)l2_bytes;
         }
         if (gx > tiles_x) gx = (int)tiles_x;
         g.group_x = gx < 1 ? 1 : gx;
@@ -1533,9 +1550,13 @@ static std::mutex g_launch_mu;
 static std::vector<LaunchEntry> g_launch_cache;
 static uint64_t g_launch_stamp = 0;
 
+static void dyn_slots_clear();
 void gemm_cache_clear() {
-    std::lock_guard<std::mutex> lk(g_launch_mu);
-    g_launch_cache.clear();
+    {
+        std::lock_guard<std::mutex> lk(g_launch_mu);
+        g_launch_cache.clear();
+    }
+    dyn_slots_clear();     // ra_shutdown: the caller has no launch in flight any more
 }
 
 // Builds plan, parameters and tensor maps for one key (the slow path of a launch).
@@ -1592,8 +1613,84 @@ static ra_status build_entry(const LaunchKey& k, const DeviceInfo& di, LaunchEnt
     {
         std::lock_guard<std::mutex> lk(g_gemm_mu);
         RA_TRY(prepare_kernel(di, pl.bn, cg, xh, p.bk, p.dyn));
+        if (p.dyn) RA_TRY(prepare_kernel(di, pl.bn, cg, xh, p.bk, 0));   // the static twin: taken when no launch slot is free
     }
     return RA_OK;
+}
+
+// ---- dynamic tile order: one g_dyn slot per launch IN FLIGHT ---------------------------------------------------------
+// A slot (claim counter, exit counter, generation, ring) belongs to ONE running kernel: two kernels drawing from one claim
+// counter would each skip the tiles the other claimed.  Launches are asynchronous, so "who still uses slot i" is answered by
+// an event recorded behind every dynamic-order launch: a slot is handed out only if it was never used or its last launch
+// has completed (cudaEventQuery), whatever stream, host thread or cache entry that launch came from.  When all kDynSlots are
+// in flight, or the stream is being captured (a graph would keep the slot's address for as long as it lives), or the
+// caller may not create an event (ra_gemm_static_ws), the launch takes the STATIC-order instantiation of the same plan --
+// same tiles, same per-element k order, same bits (tests), a few per cent slower on multi-wave shapes.
+struct DynSlot {
+    cudaEvent_t done = nullptr;   // recorded behind the last launch that used the slot
+    int device = -1;              // the device `done` was created on
+    int state = 0;                // 0 = free, 1 = claimed (its launch is being enqueued), 2 = in flight until `done` completes
+};
+static DynSlot g_dyn_slot[kDynSlots];
+static int g_dyn_cursor = 0;
+static std::mutex g_dyn_mu;
+static thread_local bool t_no_new_events = false;
+
+static int dyn_slot_acquire(int device) {
+    std::lock_guard<std::mutex> lk(g_dyn_mu);
+    for (int n = 0; n < kDynSlots; ++n) {
+        const int i = (g_dyn_cursor + n) % kDynSlots;
+        DynSlot& sl = g_dyn_slot[i];
+        if (sl.state == 1) continue;
+        if (sl.state == 2) {
+            if (cudaEventQuery(sl.done) != cudaSuccess) {
+                (void)cudaGetLastError();          // cudaErrorNotReady (still running) or a dead context: not ours to take
+                continue;
+            }
+            sl.state = 0;
+        }
+        if (sl.done != nullptr && sl.device != device) {   // an event records only on streams of its own device
+            if (t_no_new_events) continue;
+            (void)cudaEventDestroy(sl.done);
+            sl.done = nullptr;
+        }
+        if (sl.done == nullptr) {
+            if (t_no_new_events) continue;
+            if (cudaEventCreateWithFlags(&sl.done, cudaEventDisableTiming) != cudaSuccess) {
+                (void)cudaGetLastError();
+                sl.done = nullptr;
+                return -1;
+            }
+            sl.device = device;
+        }
+        sl.state = 1;
+        g_dyn_cursor = (i + 1) % kDynSlots;
+        return i;
+    }
+    return -1;
+}
+
+// After the launch: launched = the kernel was enqueued on `stream`.
+static void dyn_slot_release(int i, bool launched, cudaStream_t stream) {
+    std::lock_guard<std::mutex> lk(g_dyn_mu);
+    DynSlot& sl = g_dyn_slot[i];
+    if (launched && cudaEventRecord(sl.done, stream) == cudaSuccess) {
+        sl.state = 2;
+        return;
+    }
+    (void)cudaGetLastError();
+    // No way to tell when that kernel ends: wait for it here rather than hand its slot to somebody else.
+    if (launched) (void)cudaStreamSynchronize(stream);
+    sl.state = 0;
+}
+
+static void dyn_slots_clear() {
+    std::lock_guard<std::mutex> lk(g_dyn_mu);
+    for (DynSlot& sl : g_dyn_slot) {
+        if (sl.done != nullptr) (void)cudaEventDestroy(sl.done);
+        sl = DynSlot{};
+    }
+    (void)cudaGetLastError();
 }
 
 ra_status gemm_launch(int transA, int transB, int M, int N, int K, float alpha, const void* A, int lda, const void* B,
@@ -1635,8 +1732,6 @@ ra_status gemm_launch(int transA, int transB, int M, int N, int K, float alpha, 
         return RA_OK;
     }
 
-    RA_TRY(l2_persist_ensure(occ_v.l2_persist_bytes));   // no driver call unless the carve-out has to change
-
     LaunchKey key;
     memset(&key, 0, sizeof(key));                  // padding bytes too: keys are compared with memcmp
     key.transA = transA; key.transB = transB; key.M = M; key.N = N; key.K = K;
@@ -1649,7 +1744,6 @@ ra_status gemm_launch(int transA, int transB, int M, int N, int K, float alpha, 
     GemmParams p;
     CUtensorMap mx, my, mc;
     bool hit = false;
-    int dyn_slot = 0;                              // = the entry's index in the cache: one g_dyn slot per cached launch
     {
         std::lock_guard<std::mutex> lk(g_launch_mu);
         for (size_t i = 0; i < g_launch_cache.size(); ++i) {
@@ -1657,7 +1751,6 @@ ra_status gemm_launch(int transA, int transB, int M, int N, int K, float alpha, 
             if (memcmp(&e.key, &key, sizeof(key)) == 0) {
                 e.stamp = ++g_launch_stamp;
                 pl = e.pl; p = e.p; mx = e.mx; my = e.my; mc = e.mc;
-                dyn_slot = (int)i;
                 hit = true;
                 break;
             }
@@ -1674,13 +1767,11 @@ ra_status gemm_launch(int transA, int transB, int M, int N, int K, float alpha, 
         e.stamp = ++g_launch_stamp;
         if (g_launch_cache.size() < kLaunchCacheEntries) {
             g_launch_cache.push_back(e);
-            dyn_slot = (int)g_launch_cache.size() - 1;
         } else {
             size_t lru = 0;
             for (size_t i = 1; i < g_launch_cache.size(); ++i)
                 if (g_launch_cache[i].stamp < g_launch_cache[lru].stamp) lru = i;
             g_launch_cache[lru] = e;
-            dyn_slot = (int)lru;
         }
     }
     if (pl.ws_bytes > 0) {
@@ -1688,14 +1779,26 @@ ra_status gemm_launch(int transA, int transB, int M, int N, int K, float alpha, 
             return RA_ERR_INVALID_ARG;
     }
     if (plan_out) *plan_out = pl.pub;
+    // the carve-out the PLAN uses (0 when it ignores the knob); no driver call unless it has to change, none under capture
+    RA_TRY(l2_persist_ensure_on(pl.pub.l2_persist_bytes, stream));
     p.alpha = alpha;
     p.beta = beta;
+    int dyn_slot = -1;
     if (p.dyn) {
-        static_assert(kLaunchCacheEntries <= (size_t)kDynSlots, "one g_dyn slot per launch-cache entry");
+        cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+        if (cudaStreamIsCapturing(stream, &cs) != cudaSuccess) (void)cudaGetLastError();
+        else if (cs == cudaStreamCaptureStatusNone) dyn_slot = dyn_slot_acquire(key.device);
+        if (dyn_slot < 0) p.dyn = 0;               // no slot to be had: the static order of the same plan
+    }
+    if (p.dyn) {
         static void* g_dyn_base[64] = {};          // per device: the symbol's address never changes
         void* base = (key.device >= 0 && key.device < 64) ? g_dyn_base[key.device] : nullptr;
         if (base == nullptr) {
-            RA_CUDA(cudaGetSymbolAddress(&base, g_dyn));
+            const cudaError_t e = cudaGetSymbolAddress(&base, g_dyn);
+            if (e != cudaSuccess) {
+                dyn_slot_release(dyn_slot, false, stream);
+                RA_CUDA(e);
+            }
             if (key.device >= 0 && key.device < 64) g_dyn_base[key.device] = base;
         }
         unsigned long long* slot = static_cast<unsigned long long*>(base) + (size_t)dyn_slot * kDynSlotWords;
@@ -1708,24 +1811,26 @@ ra_status gemm_launch(int transA, int transB, int M, int N, int K, float alpha, 
         RA_CUDA(cudaMemsetAsync(workspace, 0, pl.counters_bytes, stream));
     }
     const int cg = pl.pub.cta_group, xh = pl.pub.m_blocks;
+    ra_status st = RA_ERR_UNSUPPORTED;
 #define RA_LAUNCH(BN_, CG_, XH_, DYN_)                                                                                        \
-    return p.bk == 32 ? launch_gemm<BN_, CG_, XH_, 32, DYN_>(mx, my, mc, p, pl.pub.grid, pl.pub.dyn_smem_bytes, stream)         \
-                      : launch_gemm<BN_, CG_, XH_, 64, DYN_>(mx, my, mc, p, pl.pub.grid, pl.pub.dyn_smem_bytes, stream)
+    st = p.bk == 32 ? launch_gemm<BN_, CG_, XH_, 32, DYN_>(mx, my, mc, p, pl.pub.grid, pl.pub.dyn_smem_bytes, stream)           \
+                    : launch_gemm<BN_, CG_, XH_, 64, DYN_>(mx, my, mc, p, pl.pub.grid, pl.pub.dyn_smem_bytes, stream)
     if (cg == 2 && xh == 2) {
         if (p.dyn) RA_LAUNCH(256, 2, 2, true);
-        RA_LAUNCH(256, 2, 2, false);
-    }
-    if (cg == 2) {
+        else RA_LAUNCH(256, 2, 2, false);
+    } else if (cg == 2) {
         if (p.dyn) RA_LAUNCH(256, 2, 1, true);
-        RA_LAUNCH(256, 2, 1, false);
-    }
-    switch (pl.bn) {
-        case 64: RA_LAUNCH(64, 1, 1, false);
-        case 128: RA_LAUNCH(128, 1, 1, false);
-        case 256: RA_LAUNCH(256, 1, 1, false);
+        else RA_LAUNCH(256, 2, 1, false);
+    } else {
+        switch (pl.bn) {
+            case 64: RA_LAUNCH(64, 1, 1, false); break;
+            case 128: RA_LAUNCH(128, 1, 1, false); break;
+            case 256: RA_LAUNCH(256, 1, 1, false); break;
+        }
     }
 #undef RA_LAUNCH
-    return RA_ERR_UNSUPPORTED;
+    if (dyn_slot >= 0) dyn_slot_release(dyn_slot, st == RA_OK, stream);
+    return st;
 }
 
 }  // namespace ra
@@ -1825,6 +1930,11 @@ extern "C" ra_status ra_gemm_static_ws(int transA, int transB, int M, int N, int
     if (planned && pl.ws_bytes > 0) RA_TRY(ra::static_ws_address(&ws));
     // From here on this is ra_gemm: gemm_launch zeroes the tile counters at the head of the workspace on `stream` before
     // the kernel (cudaMemsetAsync) and never reads a partial sum it has not written in the same launch.
-    return ra::gemm_launch(transA, transB, M, N, K, alpha, A, lda, B, ldb, beta, C, ldc, occ, ws,
-                           ws ? RA_GEMM_STATIC_WS_BYTES : 0, static_cast<cudaStream_t>(stream), nullptr, 0);
+    // Dynamic-order plans need an event per launch slot; this path creates none (it reuses slots whose event a plain ra_gemm
+    // call made earlier, else it runs the static tile order: same bits).
+    ra::t_no_new_events = true;
+    const ra_status st = ra::gemm_launch(transA, transB, M, N, K, alpha, A, lda, B, ldb, beta, C, ldc, occ, ws,
+                                         ws ? RA_GEMM_STATIC_WS_BYTES : 0, static_cast<cudaStream_t>(stream), nullptr, 0);
+    ra::t_no_new_events = false;
+    return st;
 }

@@ -284,10 +284,20 @@ static ra_status run_once_locked(const ra_workload* w, const ra_overlap_cfg* cfg
 
 // The GEMM's L2 carve-out (occ.l2_persist_bytes) is set for the duration of one run and taken back afterwards: it is
 // device-wide, and a collective launched later on its own must not inherit it.
+static ra_status plan_l2_persist(const ra_workload* w, const ra_overlap_cfg* cfg, long long* bytes) {
+    *bytes = 0;
+    if (!(w->M > 0 && w->N > 0) || cfg->occ.l2_persist_bytes <= 0) return RA_OK;
+    ra_gemm_plan plan;
+    RA_TRY(ra_gemm_plan_query(w->transA, w->transB, w->M, w->N, w->K, &cfg->occ, &plan));
+    *bytes = plan.l2_persist_bytes;
+    return RA_OK;
+}
+
 static ra_status run_once(const ra_workload* w, const ra_overlap_cfg* cfg, ra_overlap_result* res) {
     std::lock_guard<std::mutex> lk(g_cache.mu);
-    const long long want = (w->M > 0 && w->N > 0) ? cfg->occ.l2_persist_bytes : 0;
-    if (want < 0) return RA_ERR_INVALID_ARG;
+    if (cfg->occ.l2_persist_bytes < 0) return RA_ERR_INVALID_ARG;
+    long long want = 0;                       // what the PLAN uses: swapped, stream-K, split-K and single-wave plans ignore the knob
+    RA_TRY(plan_l2_persist(w, cfg, &want));
     RA_TRY(l2_persist_ensure(want));          // want = 0 too: a carve-out found on the device is the collective's loss
     ra_status st = run_once_locked(w, cfg, res);
     if (want > 0) {
@@ -407,8 +417,9 @@ ra_status ra_overlap_run_host(const ra_workload* dev0, const ra_workload* dev1, 
     }
     if (dev0->kind == RA_COLL_ALLTOALL && io->a2a_in == nullptr) return RA_ERR_INVALID_ARG;
     const ra_workload* sets[2] = {dev0, dev1};
-    const long long want = has_gemm ? cfg->occ.l2_persist_bytes : 0;
-    if (want < 0) return RA_ERR_INVALID_ARG;
+    if (cfg->occ.l2_persist_bytes < 0) return RA_ERR_INVALID_ARG;
+    long long want = 0;
+    RA_TRY(ra::plan_l2_persist(dev0, cfg, &want));
     RA_TRY(ra::l2_persist_ensure(want));
     ra_status st = ra::run_host(sets, dev1 ? 2 : 1, io, cfg, n_steps, res);
     if (want > 0) {
@@ -437,7 +448,22 @@ ra_status ra_overlap_sweep(const ra_workload* w, const ra_overlap_cfg* cfgs, int
     std::vector<std::vector<float>> samples((size_t)n);
     for (int i = 0; i < n; ++i) {
         int warm = warm_min;
-        for (int r = 0; r < warm + timed; ++r) {
+        int r0 = 0;
+        if (n > 1) {
+            // Run 0 of a setting that is compared with others is always a warm-up run, never instrumented, and decides
+            // how long the warm-up lasts -- BEFORE `last` is evaluated below, so that runs == 1 cannot make run 0 both
+            // the probe and the (instrumented) last run.
+            ra_overlap_result one = results[i];
+            ra_overlap_cfg c = cfgs[i];
+            c.record_kernel_times = 0;
+            one.kernel_times = nullptr;
+            RA_TRY(ra::run_once(w, &c, &one));
+            int need = one.total_ms > 0.f ? (int)(120.f / one.total_ms) + 1 : 1;
+            if (need > 12) need = 12;
+            if (need > warm) warm = need;
+            r0 = 1;
+        }
+        for (int r = r0; r < warm + timed; ++r) {
             ra_overlap_result one = results[i];
             ra_overlap_cfg c = cfgs[i];
             const bool last = (r == warm + timed - 1);
@@ -445,11 +471,6 @@ ra_status ra_overlap_sweep(const ra_workload* w, const ra_overlap_cfg* cfgs, int
             c.record_kernel_times = last ? cfgs[i].record_kernel_times : 0;
             if (!last) one.kernel_times = nullptr;
             RA_TRY(ra::run_once(w, &c, &one));
-            if (r == 0 && n > 1 && one.total_ms > 0.f) {
-                int need = (int)(120.f / one.total_ms) + 1;
-                if (need > 12) need = 12;
-                if (need > warm) warm = need;
-            }
             if (r >= warm && !(c.record_kernel_times && timed > 1)) samples[i].push_back(one.total_ms);
             if (last) {
                 float* kt = results[i].kernel_times;
@@ -479,7 +500,7 @@ ra_status ra_overlap_sweep(const ra_workload* w, const ra_overlap_cfg* cfgs, int
 void ra_shutdown(void) {
     ra::peer_close_all();
     ra::gemm_cache_clear();
-    (void)ra::l2_persist_ensure(0);
+    ra::l2_persist_restore();
     std::lock_guard<std::mutex> lk(ra::g_cache.mu);
     for (auto& kv : ra::g_cache.streams) cudaStreamDestroy(kv.second);
     ra::g_cache.streams.clear();

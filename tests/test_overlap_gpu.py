@@ -139,6 +139,25 @@ def test_sweep_picks_argmin_and_reports_stats(ra):
     assert len(results[3]["kernel_times"]) == 4
 
 
+def test_sweep_with_a_single_run_per_setting(ra):
+    """runs = 1 with several settings: run 0 of every setting is the untimed warm-up probe, and exactly one later run is
+    the instrumented last one -- its per-kernel times are what the result carries (they used to be overwritten)."""
+    import torch
+    M, N, K = 1024, 1024, 1024
+    A, B, g, dC = _gemm_side(ra, M, N, K, 6)
+    bufs = [torch.zeros(1 << 20, device="cuda") for _ in range(4)]
+    w, keep = ra.make_workload(gemm=g, allreduce=bufs, n_iters=4)
+    cfgs = [ra.make_cfg(mode=0, record_kernel_times=1), ra.make_cfg(mode=1, record_kernel_times=1)]
+    results, best = ra.ra_overlap_sweep(w, cfgs, runs=1)
+    assert best == 1
+    for r in results:
+        assert r["total_ms"] > 0 and r["min_ms"] == r["median_ms"] == r["total_ms"]      # one sample
+        assert len(r["kernel_times"]) == 4 and r["gemm_ms_sum"] > 0 and r["coll_ms_sum"] > 0
+        assert r["gemm_ms_sum"] <= r["total_ms"] * 1.05
+    single, b1 = ra.ra_overlap_sweep(w, cfgs[1:], runs=1)       # n == 1: no probe, the one run is the result
+    assert b1 == 0 and single[0]["total_ms"] > 0
+
+
 def test_trace_records_residency(ra):
     """Per-SM residency evidence: persistent GEMM CTAs sit on distinct SMs; records are well-formed."""
     import torch
@@ -359,7 +378,8 @@ def test_reserve_is_honoured_with_a_collective_running(ra, reserve_kb, budget, c
     """For every reserve x budget of the config-5 sweep, with a collective co-running on the other stream: no SM ever
     hosts more GEMM CTAs at once than the plan accounts for (the %smid trace AND the kernel's own per-SM counter say
     so), hence the plan's smem_left_per_sm >= smem_reserve_bytes is what each SM really had left; the plan's
-    hw_ctas_per_sm is what cudaOccupancyMaxActiveBlocksPerMultiprocessor answers for the launched footprint; it is 1
+    hw_ctas_per_sm is the library's own resource arithmetic for the launched footprint (registers, threads, shared
+    memory per SM; include/ra.h says why not cudaOccupancyMaxActiveBlocksPerMultiprocessor); it is 1
     (guaranteed by padding) whenever the reserve leaves room for the padding, and otherwise the accounting assumes the
     two CTAs the hardware admits -- round 1 assumed one, and this test caught two on an SM at 160 KiB x 74."""
     import torch

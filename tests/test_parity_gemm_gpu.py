@@ -487,7 +487,7 @@ def test_l2_persist_same_bits_and_state(ra):
     (64, 2048, 4096, {}),                                    # skinny (operands swapped)
     (200, 136, 72, {}),                                      # ragged everywhere: K = 72 -> 3 k-blocks, the last 8 wide
     (129, 67, 40, {}),
-    (1000, 3000, 520, dict(cluster_k=1)),                    # ragged multi-wave single-CTA tiles: stream-K over 32-wide units
+    (1000, 3000, 520, dict(cluster_k=1)),                    # ragged K (520 = 16 units of 32 + 8) on a data-parallel pair-tile plan
     (512, 512, 8192, dict(sm_budget=37)),
 ])
 def test_tile_k_32_same_bits_as_64(ra, M, N, K, occ):
@@ -515,6 +515,41 @@ def test_tile_k_32_same_bits_as_64(ra, M, N, K, occ):
     ci, _ = run_gemm(ra, M, N, K, Ai, Bi, occ=dict(occ, tile_k=32), lda=lda, ldb=ldb, ldc=ldc)
     _, ref16 = oracle.gemm(0, 1, M, N, K, 1.0, Ai, Bi, lda=lda, ldb=ldb)
     assert ci.tobytes() == ref16.tobytes()
+
+
+@pytest.mark.parametrize("tile_k", [64, 32])
+@pytest.mark.parametrize("M,N,K,occ", [
+    (64, 4096, 8192, dict(cluster_k=1)),                          # swapped skinny path, 32 tiles over 148 CTAs
+    (64, 4096, 8192, dict(cluster_k=1, sm_budget=74, smem_reserve_bytes=128 * 1024)),   # shallow pipeline
+    (48, 2048, 4104, dict(cluster_k=1, sm_budget=40)),            # ragged M and K (4104 = 64 * 64 + 8)
+    (200, 10000, 1024, dict()),                                   # non-swapped: 80 tiles of 128 x 256 over 148 CTAs
+    (1000, 2000, 1032, dict(cta_group=1, cluster_k=1, sm_budget=37)),   # ragged everywhere, fix-up stores at the C edge
+])
+def test_stream_k_integer_exact(ra, M, N, K, occ, tile_k):
+    """The stream-K fix-up (the last part to arrive sums all parts' fp32 partials in ascending-k order) against the
+    oracle, bit for bit: with operands in {-2..2} every partial sum is an exact integer, so a lost, doubled or misplaced
+    k-range shows in the bits.  The plan is asserted to BE stream-K (split_k > 1) at the tile_k asked for -- the cases
+    that used to carry this label planned data-parallel.  PAPER.md:28 (the definition), PAPER.md:47 (occupancy shaping
+    leaves the kernel's result alone)."""
+    occ = dict(occ, tile_k=tile_k)
+    if tile_k == 32 and not ra.ra_gemm_plan_query(0, 1, M, N, K, occ)["split_k"] > 1:
+        pytest.skip("tile_k = 32 turns this shape into a data-parallel plan")
+    plan = ra.ra_gemm_plan_query(0, 1, M, N, K, occ)
+    assert plan["split_k"] > 1 and plan["tile_k"] == tile_k and plan["cluster_k"] == 1, plan
+    assert ra.ra_gemm_workspace_bytes(0, 1, M, N, K, occ) > 0
+    lda, ldb, ldc = _up8(K), _up8(K), _up8(N)
+    A = ra_inputs.smallint_bf16((M, lda), 95, ra_inputs.STREAM_A)
+    B = ra_inputs.smallint_bf16((N, ldb), 95, ra_inputs.STREAM_B)
+    _, ref16 = oracle.gemm(0, 1, M, N, K, 1.0, A, B, lda=lda, ldb=ldb)
+    got, full = run_gemm(ra, M, N, K, A, B, occ=occ, lda=lda, ldb=ldb, ldc=ldc)
+    assert np.all(full[:, N:] == 0x7FC0)
+    bad = np.argwhere(got != ref16)
+    assert bad.size == 0, (f"{len(bad)} of {M * N} entries differ, first at {bad[0].tolist()}", plan)
+    # alpha / beta through the same fix-up path: C = 2 * acc - Cin is still exact in fp32 and mostly exact in bf16 (RNE otherwise)
+    Cin = ra_inputs.smallint_bf16((M, ldc), 96, ra_inputs.STREAM_C)
+    _, ref16b = oracle.gemm(0, 1, M, N, K, 2.0, A, B, -1.0, Cin, lda=lda, ldb=ldb, ldc=ldc)
+    got2, _ = run_gemm(ra, M, N, K, A, B, alpha=2.0, beta=-1.0, Cin=Cin, occ=occ, lda=lda, ldb=ldb, ldc=ldc)
+    assert got2.tobytes() == ref16b.tobytes()
 
 
 def test_tile_k_32_is_clamped_where_it_cannot_apply(ra):
@@ -550,8 +585,9 @@ def test_dynamic_tile_order_same_bits_as_static(ra, M, N, K, occ):
 
 
 def test_dynamic_tile_order_back_to_back_and_concurrent_streams(ra):
-    """The claim counter and the ring live in a per-launch-cache-entry slot that a memset re-arms before every launch:
-    50 launches back to back on one stream, and two different GEMMs on two streams at once, all exact on integer operands."""
+    """The claim counter and the ring live in a launch slot that re-arms itself (the last CTA out zeroes the counters and
+    bumps the generation the ring tags carry; no memset in front of the kernel): 50 launches back to back on one stream,
+    and two different GEMMs on two streams at once, all exact on integer operands."""
     import torch
     M, N, K = 2048, 2048, 512
     occ = dict(sm_budget=12)
@@ -570,3 +606,55 @@ def test_dynamic_tile_order_back_to_back_and_concurrent_streams(ra):
     torch.cuda.synchronize()
     assert to_host(c1, np.uint16).reshape(M, N).tobytes() == ref16.tobytes()
     assert to_host(c2, np.uint16).reshape(M, N).tobytes() == ref16.tobytes()
+
+
+def test_dynamic_tile_order_same_key_on_two_streams(ra):
+    """include/ra.h, tile_order: every launch in flight has a claim counter of its own.  The SAME call (pointers, shape,
+    knobs -- one launch-cache entry) 50 times on each of two streams at once: with one shared counter each kernel would
+    skip the tiles the other claimed and leave the poison in C.  Both streams write the same values to the same C, so
+    any interleaving of correct launches gives the oracle's bits (integer operands: exact)."""
+    import torch
+    M, N, K = 2048, 2048, 512
+    occ = dict(sm_budget=24)                       # 12 workers x 512 x 256 tiles, 32 tiles: dynamic order, room for both kernels
+    plan = ra.ra_gemm_plan_query(0, 1, M, N, K, occ)
+    assert plan["cta_group"] == 2 and plan["split_k"] == 1 and plan["n_tiles"] > plan["grid"] // 2, plan
+    Ai = ra_inputs.smallint_bf16((M, K), 97, ra_inputs.STREAM_A)
+    Bi = ra_inputs.smallint_bf16((N, K), 97, ra_inputs.STREAM_B)
+    _, ref16 = oracle.gemm(0, 1, M, N, K, 1.0, Ai, Bi)
+    dA, dB = to_dev(Ai), to_dev(Bi)
+    ws = torch.empty(16, dtype=torch.uint8, device="cuda")
+    s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+    for rep in range(3):
+        dC = torch.full((M, N), 0x7FC0, dtype=torch.int16, device="cuda")
+        torch.cuda.synchronize()
+        for i in range(50):
+            ra.ra_gemm(0, 1, M, N, K, 1.0, dA, K, dB, K, 0.0, dC, N, occ=occ, workspace=ws, stream=s1)
+            ra.ra_gemm(0, 1, M, N, K, 1.0, dA, K, dB, K, 0.0, dC, N, occ=occ, workspace=ws, stream=s2)
+        torch.cuda.synchronize()
+        assert to_host(dC, np.uint16).reshape(M, N).tobytes() == ref16.tobytes(), rep
+
+
+def test_dynamic_tile_order_more_keys_in_flight_than_cache_entries(ra):
+    """40 distinct calls (40 output buffers -> 40 launch-cache keys) cycled three times through the 32-entry cache over
+    four streams without a synchronisation in between: evictions happen while earlier launches are still running.  A
+    launch slot is handed out only once its previous launch has completed (else the launch takes the static order), so
+    every C must equal the oracle's bits."""
+    import torch
+    M, N, K = 1536, 2048, 512
+    occ = dict(sm_budget=16)
+    plan = ra.ra_gemm_plan_query(0, 1, M, N, K, occ)
+    assert plan["cta_group"] == 2 and plan["n_tiles"] > plan["grid"] // 2, plan
+    Ai = ra_inputs.smallint_bf16((M, K), 98, ra_inputs.STREAM_A)
+    Bi = ra_inputs.smallint_bf16((N, K), 98, ra_inputs.STREAM_B)
+    _, ref16 = oracle.gemm(0, 1, M, N, K, 1.0, Ai, Bi)
+    dA, dB = to_dev(Ai), to_dev(Bi)
+    ws = torch.empty(16, dtype=torch.uint8, device="cuda")
+    cs = [torch.full((M, N), 0x7FC0, dtype=torch.int16, device="cuda") for _ in range(40)]
+    streams = [torch.cuda.Stream() for _ in range(4)]
+    torch.cuda.synchronize()
+    for rnd in range(3):
+        for i, c in enumerate(cs):
+            ra.ra_gemm(0, 1, M, N, K, 1.0, dA, K, dB, K, 0.0, c, N, occ=occ, workspace=ws, stream=streams[(i + rnd) % 4])
+    torch.cuda.synchronize()
+    for i, c in enumerate(cs):
+        assert to_host(c, np.uint16).reshape(M, N).tobytes() == ref16.tobytes(), i
