@@ -620,7 +620,13 @@ def measure_config(ra, cfg, args, peaks, world, dev, headline: bool):
               "timed_setting_is": "policy (tie within 2.5 %)" if best == 2 and sweep_argmin != 2 else ("policy" if best == 2 else "sweep final argmin"), "gemm_bound": sug["gemm_bound"],
               "model_roofline_ms": sug["t_roofline_ms"], "settings_in_sweep": len(cand_kws) - 1}
     alone = kernels_alone(ra, cfg, d, peaks, n_iters, graph=graph)
-    residency = residency_map(ra, w, best_kw, info["sm_count"]) if headline else None
+    residency = residency_map(ra, w, best_kw, info["sm_count"])
+    residency_ring = None
+    if cfg.coll == "alltoall" and cfg.M * cfg.N >= 1 << 20:
+        # the collective whose co-residency DEPENDS on the reserve: one TMA-ring alltoall CTA per SM (64 KiB ring) living inside
+        # the shared memory a 72 KiB smem_reserve_bytes makes the GEMM leave free
+        residency_ring = residency_map(ra, w, dict(mode=1, occ=dict(smem_reserve_bytes=72 * 1024), coll_variant=0, coll_smem_bytes=64 * 1024,
+                                                   coll_ctas_per_sm=1, prio_compute=0, prio_comm=info["prio_greatest"]), info["sm_count"])
 
     # ---- timed region: exactly K steps of the overlapped hot path at exactly the picked setting ----
     best_cfg = ra.make_cfg(**best_kw)
@@ -686,6 +692,8 @@ def measure_config(ra, cfg, args, peaks, world, dev, headline: bool):
         out["sweep_marginals"] = sweep_marginals(cand_kws, results, n_iters)
     if residency is not None:
         out["residency"] = residency
+    if residency_ring is not None:
+        out["residency_tma_ring_in_72k_reserve"] = residency_ring
     if args.table and headline:
         with open(args.table, "w") as f:
             json.dump(sweep_table, f, indent=1)

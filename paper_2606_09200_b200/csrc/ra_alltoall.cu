@@ -213,6 +213,10 @@ ra_status alltoall_peer_launch(const void* send, void* const* recv, int P, int r
         if (recv[j] == nullptr || (reinterpret_cast<uintptr_t>(recv[j]) & 15u)) return RA_ERR_INVALID_ARG;
         const uintptr_t r0 = reinterpret_cast<uintptr_t>(recv[j]), r1 = r0 + (size_t)P * chunk_bytes;
         if (chunk_bytes > 0 && s0 < r1 && r0 < s1) return RA_ERR_INVALID_ARG;            // send must not alias a receive buffer
+        for (int i = 0; i < j; ++i) {                                                     // nor two ranks share one
+            const uintptr_t q0 = reinterpret_cast<uintptr_t>(recv[i]), q1 = q0 + (size_t)P * chunk_bytes;
+            if (chunk_bytes > 0 && q0 < r1 && r0 < q1) return RA_ERR_INVALID_ARG;
+        }
     }
     if (variant == 0 && chunk_bytes > 0) {
         const int smem = smem_bytes_per_cta ? smem_bytes_per_cta : kA2aDefaultSmem;

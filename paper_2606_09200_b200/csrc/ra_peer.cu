@@ -62,12 +62,16 @@ static ra_status address_range(const void* p, uintptr_t* base, size_t* size) {
 }
 
 static std::mutex g_ipc_mu;
-static std::unordered_map<uintptr_t, uintptr_t> g_ipc_open;   // pointer handed out -> mapping base (what cudaIpcCloseMemHandle wants)
+// pointer handed out -> {mapping base (what cudaIpcCloseMemHandle wants), how many ra_ipc_open calls returned it}.  Opening one
+// handle twice gives the same pointer and takes a second reference inside the driver: every open is paired with one close.
+struct IpcOpen { uintptr_t base; int count; };
+static std::unordered_map<uintptr_t, IpcOpen> g_ipc_open;
 
 // ra_shutdown: unmap whatever the caller left open
 void peer_close_all() {
     std::lock_guard<std::mutex> lk(g_ipc_mu);
-    for (auto& kv : g_ipc_open) (void)cudaIpcCloseMemHandle(reinterpret_cast<void*>(kv.second));
+    for (auto& kv : g_ipc_open)
+        for (int i = 0; i < kv.second.count; ++i) (void)cudaIpcCloseMemHandle(reinterpret_cast<void*>(kv.second.base));
     g_ipc_open.clear();
     (void)cudaGetLastError();
 }
@@ -105,7 +109,9 @@ ra_status ra_ipc_open(const ra_ipc_handle* h, void** dev_ptr) {
     void* p = static_cast<uint8_t*>(base) + h->offset;
     {
         std::lock_guard<std::mutex> lk(ra::g_ipc_mu);
-        ra::g_ipc_open[reinterpret_cast<uintptr_t>(p)] = reinterpret_cast<uintptr_t>(base);
+        ra::IpcOpen& e = ra::g_ipc_open[reinterpret_cast<uintptr_t>(p)];      // value-initialised {0, 0} when new
+        e.base = reinterpret_cast<uintptr_t>(base);
+        e.count += 1;
     }
     *dev_ptr = p;
     return RA_OK;
@@ -117,8 +123,8 @@ ra_status ra_ipc_close(void* dev_ptr) {
         std::lock_guard<std::mutex> lk(ra::g_ipc_mu);
         auto it = ra::g_ipc_open.find(reinterpret_cast<uintptr_t>(dev_ptr));
         if (it == ra::g_ipc_open.end()) return RA_ERR_INVALID_ARG;
-        base = it->second;
-        ra::g_ipc_open.erase(it);
+        base = it->second.base;
+        if (--it->second.count <= 0) ra::g_ipc_open.erase(it);
     }
     RA_CUDA(cudaIpcCloseMemHandle(reinterpret_cast<void*>(base)));
     return RA_OK;

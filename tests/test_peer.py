@@ -40,6 +40,22 @@ def test_slice_argument_errors(ra):
             ra.ra_peer_slice(100, P, r)
 
 
+def test_alltoall_peer_rejects_aliased_buffers(ra):
+    """Argument errors are found before any CUDA call (so this runs without a device): two ranks sharing one receive
+    buffer, or a receive buffer overlapping the send buffer, is RA_ERR_INVALID_ARG."""
+    chunk = 4096
+    send, r0, r1 = 0x10000000, 0x20000000, 0x30000000
+    for recv in ([r0, r0], [r0, r0 + chunk], [r0, send + chunk]):
+        with pytest.raises(ra.RaError) as e:
+            ra.ra_alltoall_peer(send, recv, 0, chunk, stream=0)
+        assert e.value.status == ra.RA_ERR_INVALID_ARG, recv
+    import torch
+    if not torch.cuda.is_available():                              # (made-up addresses: never let them reach a real GPU)
+        with pytest.raises(ra.RaError) as e:                       # disjoint buffers get past validation ...
+            ra.ra_alltoall_peer(send, [r0, r1], 0, chunk, stream=0)
+        assert e.value.status in (ra.RA_ERR_CUDA, ra.RA_ERR_ARCH)   # ... and stop at "no device", not at the arguments
+
+
 def test_peer_calls_fail_loudly_without_device(ra):
     import torch
     if torch.cuda.is_available():

@@ -24,7 +24,7 @@ def ra():
 
 
 @pytest.mark.parametrize("P,count", [(1, 4099), (2, 1 << 20), (4, (1 << 18) + 37), (8, 1 << 21), (3, 5), (16, 70001)])
-@pytest.mark.parametrize("variant", [0, 1])
+@pytest.mark.parametrize("variant", [0, 1, 2])
 def test_allreduce_peer_sequential_ranks(ra, P, count, variant):
     import torch
     host = [ra_inputs.uniform_f32(count, 900 + P, ra_inputs.STREAM_AR + r) for r in range(P)]
