@@ -256,6 +256,8 @@ ra_status allreduce_launch(float* const* bufs, int P, size_t count, int sm_budge
         if (grid == 0) grid = 1;                                   // count < 4: only the scalar tail
         if (dyn > 48 * 1024)
             RA_CUDA(cudaFuncSetAttribute(allreduce_tma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, max_dyn));
+            // same split as the GEMM asks for, so that either kernel can join the other on an SM (see prepare_kernel in ra_gemm.cu)
+            RA_CUDA(cudaFuncSetAttribute(allreduce_tma_kernel, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
         allreduce_tma_kernel<<<(unsigned)grid, kArTmaThreads, dyn, stream>>>(tp, g_trace);
         RA_CUDA(cudaGetLastError());
         return RA_OK;

@@ -264,6 +264,8 @@ static ra_status launch_kernels(A2aParams p, uint64_t n_chunks, const DeviceInfo
         if (grid > p.n_units) grid = p.n_units;
         if (dyn > 48 * 1024)
             RA_CUDA(cudaFuncSetAttribute(alltoall_tma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, max_dyn));
+            // same split as the GEMM asks for, so that either kernel can join the other on an SM (see prepare_kernel in ra_gemm.cu)
+            RA_CUDA(cudaFuncSetAttribute(alltoall_tma_kernel, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
         alltoall_tma_kernel<<<(unsigned)grid, kA2aThreads, dyn, stream>>>(p, g_trace);
     } else {
         p.slice_bytes = 64 * 1024;

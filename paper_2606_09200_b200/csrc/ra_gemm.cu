@@ -1132,6 +1132,11 @@ static ra_status prepare_kernel(const DeviceInfo& di, int bn, int cg, int xh, in
     const int slot = kernel_slot(bn, cg, xh, bk, dyn);
     if (di.device >= 0 && di.device < 64 && g_attr_set[di.device][slot]) return RA_OK;
     RA_CUDA(cudaFuncSetAttribute(gemm_kernel_ptr(bn, cg, xh, bk, dyn), cudaFuncAttributeMaxDynamicSharedMemorySize, di.smem_per_block_optin));
+    // The SM's shared-memory / L1 split is configured for the kernel that lands on it and is not changed while CTAs are
+    // resident.  A GEMM CTA that was shrunk to honour smem_reserve_bytes must therefore ask for the FULL split, or the
+    // memory it leaves free does not exist as shared memory and the collective's ring cannot move in beside it
+    // (profiles/r03_residency.md: 0.000 co-residency before this).  The GEMM reads through TMA, not L1: nothing is lost.
+    RA_CUDA(cudaFuncSetAttribute(gemm_kernel_ptr(bn, cg, xh, bk, dyn), cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
     if (di.device >= 0 && di.device < 64) g_attr_set[di.device][slot] = true;
     return RA_OK;
 }
